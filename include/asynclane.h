@@ -1,0 +1,179 @@
+/*
+ * asynclane.h -- C ABI of the B200 (sm_100a) lane-batched denoising step of AsyncLane
+ * (arxiv 2606.08411).  Citations "P:L<n>" are lines of the paper text.
+ *
+ * One scheduler iteration (Alg.1 UPDATELANES) runs, per shared-prefix group, one batched
+ * model call (Eq.11).  This library is the data-parallel part of that call:
+ *
+ *   al_lane_attention     shared-prefix lane-batched bidirectional attention   (Eq.2-3)
+ *   al_kv_refresh         compact cache refresh: in-place K/V row scatter       (Eq.12)
+ *   al_confidence_select  softmax confidence / argmax / threshold unmask select (Eq.8)
+ *
+ * Conventions
+ *  - Every pointer named *_dev (and q/k/v/caches/logits/outputs/workspace) is a DEVICE pointer owned
+ *    by the caller; the library never allocates or frees device memory on the hot path and keeps no
+ *    reference after the call returns.  `al_handle` owns only small host-side state (device id, SM
+ *    count, tensor-map encoder entry point).
+ *  - Every hot call only ENQUEUES work on `cuda_stream` (a cudaStream_t passed as void*): no device
+ *    synchronisation, no host read of device descriptors; all calls are CUDA-graph capturable.
+ *  - Every call returns an al_status; nothing throws.  On error nothing has been launched, except
+ *    AL_ERR_CUDA which reports a failed launch.  `al_last_error()` gives a thread-local message.
+ *  - Sizes of 0 lanes / 0 positions / 0 rows are valid no-ops returning AL_OK.
+ *  - 16-byte alignment is required of q, k_new, v_new, caches, out, k_src, v_src, logits rows
+ *    (row_stride * element size % 16 == 0 for the vector path; otherwise a scalar path is used)
+ *    and of the workspace.
+ */
+#ifndef ASYNCLANE_H_
+#define ASYNCLANE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  AL_OK = 0,
+  AL_ERR_INVALID_ARG = 1, /* null pointer, negative size, misaligned pointer, bad enum            */
+  AL_ERR_UNSUPPORTED = 2, /* valid request this build has no kernel for (e.g. head_dim, dtype)    */
+  AL_ERR_WORKSPACE = 3,   /* workspace_bytes smaller than al_*_workspace_bytes() for these bounds */
+  AL_ERR_CUDA = 4         /* a CUDA runtime / driver call failed; see al_last_error()             */
+} al_status;
+
+typedef enum { AL_F32 = 0, AL_BF16 = 1 } al_dtype;
+
+typedef struct al_handle al_handle; /* opaque */
+
+/*
+ * Lane descriptor: one per active lane l = (r_l, s_l, b_l, z_l, t_l) of Eq.1, reduced to
+ * what the kernels need.  The array lives in DEVICE memory so that a captured graph can be
+ * replayed with new lanes.  Six int32, 24 bytes, no padding.
+ */
+typedef struct {
+  int32_t group_id;    /* lanes of one shared-prefix group G_t share one prefix KV         */
+  int32_t kv_base_row; /* "prefix offset": first row of this lane's sequence in the cache pool      */
+  int32_t prefix_len;  /* visible cache rows [kv_base_row, kv_base_row+prefix_len) = P+s_l  */
+  int32_t q_start;     /* "lane start": first row of the lane in packed Q/K_new/V_new/O/logits      */
+  int32_t q_len;       /* "lane length": b_l + w_l rows of u_l (Eq.2)                         */
+  int32_t flags;       /* bit0: refine lane => EOS suppressed in confidence_select          */
+} al_lane_desc;
+
+#define AL_LANE_FLAG_REFINE 1
+
+typedef struct {
+  int32_t n_q_heads;  /* H_q                                                            */
+  int32_t n_kv_heads; /* H_kv, divides H_q; q-head h reads kv-head h / (H_q/H_kv)        */
+  int32_t head_dim;   /* d: bf16 tensor-core path needs 128 (64 also built); f32: <= 256 */
+  int32_t dtype;      /* al_dtype of q, k_new, v_new, caches and out                     */
+  int64_t cache_rows; /* capacity in rows of ONE kv-head plane of the cache pool         */
+  float scale;        /* softmax scale; 0 => 1/sqrt(head_dim) (paper silent)             */
+  int32_t reserved;   /* must be 0                                                       */
+} al_attn_shape;
+
+/* ---- life cycle ------------------------------------------------------------------------------- */
+
+/* Creates a handle bound to CUDA device `device` (queries SM count, resolves the tensor-map encoder).
+ * Fails with AL_ERR_CUDA when no usable device exists: there is no CPU fallback. */
+al_status al_create(al_handle** out_handle, int device);
+al_status al_destroy(al_handle* handle);
+/* Thread-local, never NULL, valid until the next failing call on this thread. */
+const char* al_last_error(void);
+/* "asynclane-b200 <version> sm_100a" */
+const char* al_version(void);
+/* Number of SMs of the handle's device (grid sizing information for callers / bench). */
+int32_t al_sm_count(const al_handle* handle);
+
+/* ---- (a) shared-prefix lane-batched attention ------------------------------------------------- */
+
+/*
+ * For every lane l, q-head h (kv-head g = h / n_rep) and local row i in [0, q_len):
+ *   keys/values = cache rows kv_base_row + j, j in [0, prefix_len)      (plane g of k_cache/v_cache)
+ *              ++ k_new/v_new rows q_start + j', j' in [0, q_len)        (the lane's own rows)
+ *   out[q_start+i][h][:] = softmax_j(scale * <q_i, k_j>) . v_j           (bidirectional, no causal mask)
+ *   lse[q_start+i][h]    = log sum_j exp(scale * <q_i, k_j>)             (optional)
+ * Lanes never see each other ("updated independently using its own prefix state"); lanes with
+ * equal group_id address the same cache rows, which the kernel reads from HBM once per group and
+ * kv-head, not once per lane.
+ *
+ * Layouts (row-major, innermost last):
+ *   q, out        [T][H_q][d]        T = total packed rows (sum of q_len)
+ *   k_new, v_new  [T][H_kv][d]
+ *   k_cache, v_cache [H_kv][cache_rows][d]     (never written by this call)
+ *   lse_or_null   float [T][H_q]
+ * Host-side bounds: n_lanes (exact), total_q_rows = T (exact), max_prefix_len >= every prefix_len.
+ * Preconditions on lanes_dev (not checked on the hot path; see al_validate_lanes): lanes are disjoint
+ * in [q_start, q_start+q_len), 0 <= kv_base_row, kv_base_row+prefix_len <= cache_rows, q_len >= 1.
+ * Lanes of one group that are adjacent in the array and contiguous in q_start are stacked into
+ * common 128-row tensor-core tiles.
+ * Rows of Q not covered by any lane are not written in `out`.
+ */
+size_t al_lane_attention_workspace_bytes(const al_attn_shape* shape, int32_t n_lanes,
+                                         int32_t total_q_rows, int32_t max_prefix_len);
+al_status al_lane_attention(al_handle* handle, const al_attn_shape* shape, const void* q,
+                            const void* k_new, const void* v_new, const void* k_cache,
+                            const void* v_cache, const al_lane_desc* lanes_dev, int32_t n_lanes,
+                            int32_t total_q_rows, int32_t max_prefix_len, void* out,
+                            float* lse_or_null, void* workspace, size_t workspace_bytes,
+                            void* cuda_stream);
+
+/* ---- (b) compact cache refresh ---------------------------------------------------------------- */
+
+/*
+ * For r in [0, n_pos), layer in [0, n_layers), kv-head g:
+ *   k_cache[layer][g][kv_base_row + pos[r]][:] = k_src[layer][r][g][:]     (same for V)
+ * Bit copy; every other byte of the caches is untouched.  Layouts: caches [H_kv][cache_rows][d] per
+ * layer, layers `layer_stride_cache` ELEMENTS apart; src [R][H_kv][d] per layer, layers
+ * `layer_stride_src` elements apart.  Precondition: pos strictly increasing (unique), each
+ * kv_base_row + pos[r] in [0, cache_rows).  Duplicates make the result order-dependent.
+ * head_dim * element size must be a multiple of 16.
+ */
+al_status al_kv_refresh(al_handle* handle, const al_attn_shape* shape, void* k_cache, void* v_cache,
+                        const void* k_src, const void* v_src, const int32_t* pos_dev, int32_t n_pos,
+                        int32_t kv_base_row, int32_t n_layers, int64_t layer_stride_cache,
+                        int64_t layer_stride_src, void* cuda_stream);
+
+/* ---- (c) confidence / argmax / threshold select ----------------------------------------------- */
+
+#define AL_SELECT_FORCE_TOP1 1
+
+/*
+ * Per row i of logits [n_rows][vocab] (row_stride elements between rows):
+ *   x = logits row (refine-lane rows with eos_id >= 0: x[eos_id] = -inf)
+ *   argmax_out[i] = first index attaining max x;  conf_out[i] = 1 / sum_v exp(x_v - max x)
+ *   commit_out[i] = (tokens_in[i] == mask_id) && conf_out[i] >= threshold
+ *   flags & AL_SELECT_FORCE_TOP1: a lane with masked rows but no commit commits its masked row of
+ *     largest confidence (lowest row on ties).  Without lanes, all rows form one generate lane.
+ *   tokens_out[i] = commit ? argmax : tokens_in[i]     (tokens_out may alias tokens_in)
+ * conf is computed in fp32 from the dtype-rounded logits.  Rows must hold at least one finite value.
+ */
+size_t al_confidence_select_workspace_bytes(int32_t n_rows, int32_t vocab);
+al_status al_confidence_select(al_handle* handle, const void* logits, int32_t logits_dtype,
+                               int32_t n_rows, int32_t vocab, int64_t row_stride,
+                               const int32_t* tokens_in_dev, int32_t mask_id, int32_t eos_id,
+                               float threshold, const al_lane_desc* lanes_dev_or_null,
+                               int32_t n_lanes, int32_t flags, float* conf_out, int32_t* argmax_out,
+                               uint8_t* commit_out, int32_t* tokens_out, void* workspace,
+                               size_t workspace_bytes, void* cuda_stream);
+
+/* ---- debug / self-test (synchronising; never on the hot path) --------------------------------- */
+
+/* Copies the descriptors to the host and checks the preconditions listed above.  Synchronises. */
+al_status al_validate_lanes(al_handle* handle, const al_attn_shape* shape,
+                            const al_lane_desc* lanes_dev, int32_t n_lanes, int32_t total_q_rows);
+
+/*
+ * tcgen05 encoding self-test: one 128x128x128 bf16 tile pipeline through the same TMA maps, shared
+ * memory descriptors, instruction descriptors and TMEM paths as the attention kernel:
+ *   s_out[128][128] (f32) = A . B^T                (A, B: [128][128] bf16, K-major)
+ *   o_out[128][128] (f32) = bf16(s_out * p_scale) . V   (V: [128 keys][128] bf16, P fed from TMEM)
+ * Synchronises.  All pointers are device pointers.
+ */
+al_status al_selftest_umma(al_handle* handle, const void* a_bf16, const void* b_bf16,
+                           const void* v_bf16, float p_scale, float* s_out, float* o_out,
+                           void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ASYNCLANE_H_ */

@@ -1,0 +1,180 @@
+"""ctypes binding of libasynclane.so -- argument marshalling only.
+
+Same names as the C ABI (include/asynclane.h).  Arguments are torch CUDA tensors (used purely as
+device memory) or raw ints; every step of the path runs in the library's kernels.  There is no CPU
+fallback: loading fails loudly if the library is missing, and al_create fails without a B200.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+AL_OK, AL_ERR_INVALID_ARG, AL_ERR_UNSUPPORTED, AL_ERR_WORKSPACE, AL_ERR_CUDA = range(5)
+AL_F32, AL_BF16 = 0, 1
+AL_LANE_FLAG_REFINE = 1
+AL_SELECT_FORCE_TOP1 = 1
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libasynclane.so")
+
+EXPORTS = [
+    "al_create", "al_destroy", "al_last_error", "al_version", "al_sm_count",
+    "al_lane_attention_workspace_bytes", "al_lane_attention", "al_kv_refresh",
+    "al_confidence_select_workspace_bytes", "al_confidence_select", "al_validate_lanes",
+    "al_selftest_umma",
+]
+
+
+class AlError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"asynclane status {status}: {message}")
+        self.status = status
+
+
+class al_attn_shape(ctypes.Structure):
+    _fields_ = [("n_q_heads", ctypes.c_int32), ("n_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+                ("dtype", ctypes.c_int32), ("cache_rows", ctypes.c_int64), ("scale", ctypes.c_float),
+                ("reserved", ctypes.c_int32)]
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
+    """dlopen libasynclane.so (building it in-tree first if absent) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        if not build_if_missing:
+            raise FileNotFoundError(f"{LIB_PATH} missing: run `python -m paper_2606_08411_b200.build`")
+        from . import build as _build
+        _build.build()
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64, f32, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_size_t
+    shp = ctypes.POINTER(al_attn_shape)
+    lib.al_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int]
+    lib.al_destroy.argtypes = [vp]
+    lib.al_last_error.restype = ctypes.c_char_p
+    lib.al_version.restype = ctypes.c_char_p
+    lib.al_sm_count.argtypes = [vp]
+    lib.al_sm_count.restype = i32
+    lib.al_lane_attention_workspace_bytes.argtypes = [shp, i32, i32, i32]
+    lib.al_lane_attention_workspace_bytes.restype = sz
+    lib.al_lane_attention.argtypes = [vp, shp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, sz, vp]
+    lib.al_kv_refresh.argtypes = [vp, shp, vp, vp, vp, vp, vp, i32, i32, i32, i64, i64, vp]
+    lib.al_confidence_select_workspace_bytes.argtypes = [i32, i32]
+    lib.al_confidence_select_workspace_bytes.restype = sz
+    lib.al_confidence_select.argtypes = [vp, vp, i32, i32, i32, i64, vp, i32, i32, f32, vp, i32, i32,
+                                         vp, vp, vp, vp, vp, sz, vp]
+    lib.al_validate_lanes.argtypes = [vp, shp, vp, i32, i32]
+    lib.al_selftest_umma.argtypes = [vp, vp, vp, vp, f32, vp, vp, vp]
+    for name in EXPORTS:
+        fn = getattr(lib, name)
+        if name not in ("al_last_error", "al_version", "al_sm_count", "al_lane_attention_workspace_bytes",
+                        "al_confidence_select_workspace_bytes"):
+            fn.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _check(status: int) -> None:
+    if status != AL_OK:
+        raise AlError(status, load_library().al_last_error().decode())
+
+
+def _ptr(t) -> Optional[int]:
+    """Device pointer of a torch CUDA tensor (None passes NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise TypeError("asynclane: expected a CUDA tensor (the library has no CPU path)")
+    if not t.is_contiguous():
+        raise ValueError("asynclane: tensors must be contiguous")
+    return t.data_ptr()
+
+
+def _dtype_code(t) -> int:
+    import torch
+    if t.dtype == torch.bfloat16:
+        return AL_BF16
+    if t.dtype == torch.float32:
+        return AL_F32
+    raise TypeError(f"asynclane: unsupported dtype {t.dtype}")
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+class Handle:
+    """Owns an al_handle; methods carry the names of the C entry points."""
+
+    def __init__(self, device: int = 0):
+        self._lib = load_library()
+        h = ctypes.c_void_p()
+        _check(self._lib.al_create(ctypes.byref(h), device))
+        self._h = h
+        self.device = device
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            self._lib.al_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def sm_count(self) -> int:
+        return int(self._lib.al_sm_count(self._h))
+
+    @staticmethod
+    def make_shape(n_q_heads: int, n_kv_heads: int, head_dim: int, dtype: int, cache_rows: int,
+                   scale: float = 0.0) -> al_attn_shape:
+        return al_attn_shape(n_q_heads, n_kv_heads, head_dim, dtype, cache_rows, scale, 0)
+
+    def al_lane_attention_workspace_bytes(self, shape: al_attn_shape, n_lanes: int, total_q_rows: int,
+                                          max_prefix_len: int) -> int:
+        return int(self._lib.al_lane_attention_workspace_bytes(ctypes.byref(shape), n_lanes, total_q_rows,
+                                                               max_prefix_len))
+
+    def al_lane_attention(self, shape, q, k_new, v_new, k_cache, v_cache, lanes_dev, n_lanes, total_q_rows,
+                          max_prefix_len, out, lse=None, workspace=None, stream=None) -> None:
+        ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+        _check(self._lib.al_lane_attention(self._h, ctypes.byref(shape), _ptr(q), _ptr(k_new), _ptr(v_new),
+                                           _ptr(k_cache), _ptr(v_cache), _ptr(lanes_dev), n_lanes, total_q_rows,
+                                           max_prefix_len, _ptr(out), _ptr(lse), _ptr(workspace), ws_bytes,
+                                           _stream_ptr(stream)))
+
+    def al_kv_refresh(self, shape, k_cache, v_cache, k_src, v_src, pos_dev, n_pos, kv_base_row=0, n_layers=1,
+                      layer_stride_cache=0, layer_stride_src=0, stream=None) -> None:
+        _check(self._lib.al_kv_refresh(self._h, ctypes.byref(shape), _ptr(k_cache), _ptr(v_cache), _ptr(k_src),
+                                       _ptr(v_src), _ptr(pos_dev), n_pos, kv_base_row, n_layers,
+                                       layer_stride_cache, layer_stride_src, _stream_ptr(stream)))
+
+    def al_confidence_select_workspace_bytes(self, n_rows: int, vocab: int) -> int:
+        return int(self._lib.al_confidence_select_workspace_bytes(n_rows, vocab))
+
+    def al_confidence_select(self, logits, n_rows, vocab, row_stride, tokens_in, mask_id, eos_id, threshold,
+                             lanes_dev, n_lanes, flags, conf_out, argmax_out, commit_out, tokens_out,
+                             workspace, stream=None) -> None:
+        ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+        _check(self._lib.al_confidence_select(self._h, _ptr(logits), _dtype_code(logits), n_rows, vocab,
+                                              row_stride, _ptr(tokens_in), mask_id, eos_id, threshold,
+                                              _ptr(lanes_dev), n_lanes, flags, _ptr(conf_out), _ptr(argmax_out),
+                                              _ptr(commit_out), _ptr(tokens_out), _ptr(workspace), ws_bytes,
+                                              _stream_ptr(stream)))
+
+    def al_validate_lanes(self, shape, lanes_dev, n_lanes, total_q_rows) -> None:
+        _check(self._lib.al_validate_lanes(self._h, ctypes.byref(shape), _ptr(lanes_dev), n_lanes, total_q_rows))
+
+    def al_selftest_umma(self, a, b, v, p_scale, s_out, o_out, stream=None) -> None:
+        _check(self._lib.al_selftest_umma(self._h, _ptr(a), _ptr(b), _ptr(v), p_scale, _ptr(s_out), _ptr(o_out),
+                                          _stream_ptr(stream)))

@@ -1,0 +1,98 @@
+// al_kv_refresh -- compact cache refresh scatter (Eq.12).
+//
+// cache[layer][g][kv_base_row + pos[r]][:] = src[layer][r][g][:] for K and V, as a pure bit copy in
+// 16-byte vectors.  HBM-bound stream: algorithmic bytes = 2 planes x (read + write) x R x H_kv x
+// row_bytes x layers (+ 4R for pos).  Source reads are fully contiguous; destination writes are
+// contiguous runs of row_bytes (256 B for d=128 bf16).  Each thread moves UNROLL vectors of K and
+// of V with all loads issued before the stores (memory-level parallelism), streaming cache hints on
+// the read side (source rows are read exactly once).
+#include "al_internal.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kUnroll = 4;
+
+__device__ __forceinline__ int4 ld_stream(const int4* p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+// vecs_per_row = row_bytes/16; one "item" = one 16-byte vector of one (layer, r, g) row.
+__global__ void __launch_bounds__(kThreads)
+kv_refresh_kernel(int4* __restrict__ k_cache, int4* __restrict__ v_cache,
+                  const int4* __restrict__ k_src, const int4* __restrict__ v_src,
+                  const int32_t* __restrict__ pos, int n_pos, int kv_base_row, int n_kv_heads,
+                  long long cache_rows, int vecs_per_row, long long layer_stride_cache_vecs,
+                  long long layer_stride_src_vecs, long long items_per_layer, long long total_items) {
+  const long long stride = (long long)gridDim.x * kThreads;
+  long long i0 = (long long)blockIdx.x * kThreads + threadIdx.x;
+  for (; i0 < total_items; i0 += stride * kUnroll) {
+    int4 kv[kUnroll], vv[kUnroll];
+    long long dst[kUnroll];
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u) {
+      const long long i = i0 + u * stride;
+      dst[u] = -1;
+      if (i < total_items) {
+        const long long layer = i / items_per_layer;
+        const long long rem = i - layer * items_per_layer;      // (r * H_kv + g) * vecs_per_row + c
+        const int c = (int)(rem % vecs_per_row);
+        const long long rg = rem / vecs_per_row;
+        const int g = (int)(rg % n_kv_heads);
+        const int r = (int)(rg / n_kv_heads);
+        const long long s = layer * layer_stride_src_vecs + rem;
+        kv[u] = ld_stream(k_src + s);
+        vv[u] = ld_stream(v_src + s);
+        const long long row = (long long)g * cache_rows + kv_base_row + __ldg(pos + r);
+        dst[u] = layer * layer_stride_cache_vecs + row * vecs_per_row + c;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u)
+      if (dst[u] >= 0) {
+        k_cache[dst[u]] = kv[u];
+        v_cache[dst[u]] = vv[u];
+      }
+  }
+}
+
+}  // namespace
+
+extern "C" al_status al_kv_refresh(al_handle* h, const al_attn_shape* s, void* k_cache, void* v_cache,
+                                   const void* k_src, const void* v_src, const int32_t* pos_dev,
+                                   int32_t n_pos, int32_t kv_base_row, int32_t n_layers,
+                                   int64_t layer_stride_cache, int64_t layer_stride_src, void* stream) {
+  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: handle is NULL");
+  al_status st = al_check_shape(s, "al_kv_refresh");
+  if (st != AL_OK) return st;
+  if (n_pos < 0 || n_layers < 0 || kv_base_row < 0 || layer_stride_cache < 0 || layer_stride_src < 0)
+    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: negative size");
+  if (n_pos == 0 || n_layers == 0) return AL_OK;
+  if (!k_cache || !v_cache || !k_src || !v_src || !pos_dev) AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: NULL pointer");
+  const int esz = al_esize(s->dtype);
+  const long long row_bytes = (long long)s->head_dim * esz;
+  if (row_bytes % 16 != 0) AL_FAIL(AL_ERR_UNSUPPORTED, "al_kv_refresh: head_dim*esize = %lld not a multiple of 16", row_bytes);
+  if (!al_aligned16(k_cache) || !al_aligned16(v_cache) || !al_aligned16(k_src) || !al_aligned16(v_src))
+    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: pointers must be 16-byte aligned");
+  if ((layer_stride_cache * esz) % 16 != 0 || (layer_stride_src * esz) % 16 != 0)
+    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: layer strides must be multiples of 16 bytes");
+  if (n_layers > 1 && (layer_stride_cache < (int64_t)s->n_kv_heads * s->cache_rows * s->head_dim ||
+                       layer_stride_src < (int64_t)n_pos * s->n_kv_heads * s->head_dim))
+    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: layer strides smaller than one layer");
+  const int vpr = (int)(row_bytes / 16);
+  const long long items_per_layer = (long long)n_pos * s->n_kv_heads * vpr;
+  const long long total = items_per_layer * n_layers;
+  long long blocks = (total + (long long)kThreads * kUnroll - 1) / ((long long)kThreads * kUnroll);
+  const long long cap = (long long)h->sm_count * 16;       // grid-stride beyond 16 CTAs per SM
+  if (blocks > cap) blocks = cap;
+  kv_refresh_kernel<<<(unsigned)blocks, kThreads, 0, static_cast<cudaStream_t>(stream)>>>(
+      (int4*)k_cache, (int4*)v_cache, (const int4*)k_src, (const int4*)v_src, pos_dev, n_pos,
+      kv_base_row, s->n_kv_heads, (long long)s->cache_rows, vpr, layer_stride_cache * esz / 16,
+      layer_stride_src * esz / 16, items_per_layer, total);
+  AL_CUDA_OK(cudaGetLastError());
+  return AL_OK;
+}

@@ -1,0 +1,102 @@
+"""Device-resident buffers for one lane-batched denoising step and the three C-ABI calls that make
+up the hot path: per layer al_lane_attention, then al_kv_refresh (all layers in one
+launch), then al_confidence_select.  Only marshalling and buffer ownership live here; torch is used
+for device memory, streams and CUDA graphs.
+"""
+from __future__ import annotations
+
+from typing import Optional
+
+import numpy as np
+import torch
+
+from . import binding as B
+from .workloads import LaneStepWorkload, bf16_bits
+
+
+def to_device(x: np.ndarray, dtype: str, device) -> torch.Tensor:
+    """float32 array whose values are representable in `dtype` -> device tensor of that dtype."""
+    if dtype == "bf16":
+        bits = torch.from_numpy(bf16_bits(x).view(np.int16).reshape(x.shape))
+        return bits.to(device).view(torch.bfloat16)
+    return torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(device)
+
+
+def to_host_pinned(x: np.ndarray, dtype: str) -> torch.Tensor:
+    if dtype == "bf16":
+        t = torch.from_numpy(bf16_bits(x).view(np.int16).reshape(x.shape)).view(torch.bfloat16)
+    else:
+        t = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32))
+    return t.pin_memory()
+
+
+class LaneStep:
+    """One workload resident on the GPU + outputs + workspaces; `run()` enqueues the whole step."""
+
+    def __init__(self, handle: B.Handle, wl: LaneStepWorkload, device="cuda:0", want_lse: bool = True,
+                 force_top1: bool = False):
+        self.h = handle
+        self.wl = wl
+        dev = torch.device(device)
+        self.device = dev
+        dt = wl.dtype
+        self.code = B.AL_BF16 if dt == "bf16" else B.AL_F32
+        self.tdtype = torch.bfloat16 if dt == "bf16" else torch.float32
+        self.shape = B.Handle.make_shape(wl.n_q_heads, wl.n_kv_heads, wl.head_dim, self.code, wl.cache_rows)
+        self.q = to_device(wl.q, dt, dev)
+        self.k_new = to_device(wl.k_new, dt, dev)
+        self.v_new = to_device(wl.v_new, dt, dev)
+        self.k_cache = to_device(wl.k_cache, dt, dev)
+        self.v_cache = to_device(wl.v_cache, dt, dev)
+        self.k_src = to_device(wl.k_src, dt, dev)
+        self.v_src = to_device(wl.v_src, dt, dev)
+        self.logits = to_device(wl.logits, dt, dev)
+        self.lanes = torch.from_numpy(np.ascontiguousarray(wl.lanes, dtype=np.int32)).to(dev)
+        self.pos = torch.from_numpy(np.ascontiguousarray(wl.refresh_pos, dtype=np.int32)).to(dev)
+        self.tokens = torch.from_numpy(np.ascontiguousarray(wl.tokens, dtype=np.int32)).to(dev)
+        L, T = wl.n_layers, wl.total_q_rows
+        N, V = wl.logits.shape
+        self.n_layers, self.T, self.N, self.V = L, T, N, V
+        self.out = torch.zeros((L, T, wl.n_q_heads, wl.head_dim), dtype=self.tdtype, device=dev)
+        self.lse = torch.zeros((L, T, wl.n_q_heads), dtype=torch.float32, device=dev) if want_lse else None
+        self.conf = torch.zeros(N, dtype=torch.float32, device=dev)
+        self.argmax = torch.zeros(N, dtype=torch.int32, device=dev)
+        self.commit = torch.zeros(N, dtype=torch.uint8, device=dev)
+        self.tokens_out = torch.zeros(N, dtype=torch.int32, device=dev)
+        self.max_prefix = wl.max_prefix_len
+        ws_a = handle.al_lane_attention_workspace_bytes(self.shape, wl.n_lanes, T, self.max_prefix)
+        ws_c = handle.al_confidence_select_workspace_bytes(N, V)
+        self.ws_attn = torch.empty(max(ws_a, 16), dtype=torch.uint8, device=dev)
+        self.ws_conf = torch.empty(max(ws_c, 16), dtype=torch.uint8, device=dev)
+        self.flags = B.AL_SELECT_FORCE_TOP1 if force_top1 else 0
+        self.gpu_launches_per_step = None   # filled by callers that count (bench)
+
+    # -- the three parts ---------------------------------------------------------------------------
+    def attention(self, stream=None, layers: Optional[range] = None) -> None:
+        wl = self.wl
+        for l in (range(self.n_layers) if layers is None else layers):
+            self.h.al_lane_attention(self.shape, self.q[l], self.k_new[l], self.v_new[l], self.k_cache[l],
+                                     self.v_cache[l], self.lanes, wl.n_lanes, self.T, self.max_prefix,
+                                     self.out[l], None if self.lse is None else self.lse[l], self.ws_attn,
+                                     stream)
+
+    def refresh(self, stream=None) -> None:
+        wl = self.wl
+        R = int(self.pos.numel())
+        per_layer_cache = wl.n_kv_heads * wl.cache_rows * wl.head_dim
+        per_layer_src = R * wl.n_kv_heads * wl.head_dim
+        self.h.al_kv_refresh(self.shape, self.k_cache, self.v_cache, self.k_src, self.v_src, self.pos, R,
+                             wl.refresh_base_row, self.n_layers, per_layer_cache, per_layer_src, stream)
+
+    def confidence(self, stream=None) -> None:
+        wl = self.wl
+        self.h.al_confidence_select(self.logits, self.N, self.V, self.V, self.tokens, wl.mask_id, wl.eos_id,
+                                    float(wl.threshold), self.lanes, wl.n_lanes, self.flags, self.conf,
+                                    self.argmax, self.commit, self.tokens_out, self.ws_conf, stream)
+
+    def run(self, stream=None) -> None:
+        """The whole hot path once.  Attention reads the cache BEFORE this step's refresh writes it
+        (kappa_l is the state the lanes were forked from; refresh is periodic, L176)."""
+        self.attention(stream)
+        self.refresh(stream)
+        self.confidence(stream)

@@ -1,0 +1,381 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star):
+  attention   bf16 in / fp32 accumulate: max over (row, head) of ||out - ref||_inf / ||ref||_inf <= 1e-2
+              (reading C10); LSE abs <= 2e-2... stated per test; fp32 path: 2e-5 normwise
+  refresh     bit-exact
+  confidence  |conf - ref| <= 2e-3; argmax / commit / tokens bit-exact wherever the top-2 probability
+              gap exceeds 1e-3 and |conf - tau| > 4e-3 (reading C7); exempt rows are counted and bounded
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from paper_2606_08411_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def handle():
+    from paper_2606_08411_b200 import binding
+    h = binding.Handle(0)
+    yield h
+    h.close()
+
+
+def make_step(handle, wl, **kw):
+    from paper_2606_08411_b200.step import LaneStep
+    return LaneStep(handle, wl, **kw)
+
+
+def to_np(t):
+    return t.detach().float().cpu().numpy() if t.dtype in (torch.bfloat16, torch.float32) else t.detach().cpu().numpy()
+
+
+# ------------------------------------------------------------------------------------------------
+# attention
+# ------------------------------------------------------------------------------------------------
+def attn_errors(out, ref):
+    """normwise relative error per (row, head) (reading C10) and its max."""
+    num = np.abs(out - ref).max(axis=-1)
+    den = np.abs(ref).max(axis=-1)
+    return (num / np.maximum(den, 1e-30)).max()
+
+
+def check_attention(handle, wl, tol, lse_tol):
+    st = make_step(handle, wl)
+    st.attention()
+    torch.cuda.synchronize()
+    out = to_np(st.out)
+    lse = to_np(st.lse)
+    covered = np.zeros(wl.total_q_rows, bool)
+    for l in wl.lanes:
+        covered[l[W.LANE_Q_START]:l[W.LANE_Q_START] + l[W.LANE_Q_LEN]] = True
+    for layer in range(wl.n_layers):
+        ref, ref_lse = oracle.lane_attention(wl.q[layer], wl.k_new[layer], wl.v_new[layer], wl.k_cache[layer],
+                                             wl.v_cache[layer], wl.lanes)
+        assert np.isfinite(out[layer][covered]).all()
+        err = attn_errors(out[layer][covered], ref[covered])
+        assert err <= tol, f"{wl.name} layer {layer}: normwise rel err {err:.3e} > {tol}"
+        assert np.abs(lse[layer][covered] - ref_lse[covered]).max() <= lse_tol
+    return st
+
+
+def test_attention_cfg1_tiny_fp32(handle):
+    check_attention(handle, W.cfg1_tiny(), tol=2e-5, lse_tol=2e-5)
+
+
+@pytest.mark.parametrize("seed", [101, 102, 103, 104])
+def test_attention_ragged_lanes_bf16(handle, seed):
+    """lane lengths 11..24/32, per-lane prefix lengths inside a group (reading C1),
+    GQA 8/2, several M tiles and ragged tails."""
+    check_attention(handle, W.ragged_case(seed), tol=1e-2, lse_tol=1e-3)
+
+
+def test_attention_ragged_fp32_other_head_dims(handle):
+    for d, seed in ((32, 7), (64, 8), (96, 9)):
+        wl = W.ragged_case(seed, dtype="f32", n_q_heads=4, n_kv_heads=2, head_dim=d, max_prefix=150)
+        check_attention(handle, wl, tol=2e-5, lse_tol=2e-5)
+
+
+def test_attention_cfg2_llada_layer(handle):
+    check_attention(handle, W.cfg2_llada_layer(), tol=1e-2, lse_tol=1e-3)
+
+
+def test_attention_cfg3_dream_layer(handle):
+    check_attention(handle, W.cfg3_dream_layer(), tol=1e-2, lse_tol=1e-3)
+
+
+def test_attention_degenerate_cases(handle):
+    # prefix_len = 0 (pure block self-attention), q_len = 1 lanes, a single lane, MHA and GQA 7
+    cases = [
+        dict(groups=[dict(kv_base_row=0, prefix_len=0, q_lens=[32, 5])], Hq=4, Hkv=4),
+        dict(groups=[dict(kv_base_row=2, prefix_len=130, q_lens=[1, 1, 1])], Hq=14, Hkv=2),
+        dict(groups=[dict(kv_base_row=0, prefix_len=1, q_lens=[32])], Hq=2, Hkv=1),
+        dict(groups=[dict(kv_base_row=0, prefix_len=[257, 129, 1], q_lens=[32, 17, 32]),
+                     dict(kv_base_row=300, prefix_len=128, q_lens=[24])], Hq=7, Hkv=1),
+    ]
+    for i, c in enumerate(cases):
+        wl = W.build_workload(f"degenerate_{i}", 500 + i, "bf16", c["Hq"], c["Hkv"], 128, 1, 512, c["groups"],
+                              n_refresh=1, refresh_base_row=0, refresh_span=8, vocab=64, logit_sigma=1.0,
+                              planted_frac=0.0, mask_id=63, eos_id=-1, threshold=0.9)
+        check_attention(handle, wl, tol=1e-2, lse_tol=1e-3)
+
+
+def test_attention_lane_independence_on_gpu(handle):
+    """Perturbing one lane's Q/K/V must leave every other lane's output unchanged (bit-identical:
+    the other lanes' tiles see identical operands)."""
+    wl = W.ragged_case(105)
+    st = make_step(handle, wl)
+    st.attention(); torch.cuda.synchronize()
+    base = st.out.clone()
+    qs, ql = int(wl.lanes[0, W.LANE_Q_START]), int(wl.lanes[0, W.LANE_Q_LEN])
+    st.q[0, qs:qs + ql] += 1.0
+    st.k_new[0, qs:qs + ql] *= -1.0
+    st.v_new[0, qs:qs + ql] += 2.0
+    st.attention(); torch.cuda.synchronize()
+    rest = torch.ones(wl.total_q_rows, dtype=torch.bool, device=st.out.device); rest[qs:qs + ql] = False
+    assert torch.equal(st.out[0][rest], base[0][rest])
+    assert not torch.equal(st.out[0][~rest], base[0][~rest])
+
+
+def test_attention_full_size_sampled_outputs_cfg4_one_layer(handle):
+    """cfg4 shapes (12 lanes in 4 nested groups, prefixes 512..1280) on 2 layers; sampled rows vs the
+    one-row oracle entry point."""
+    wl = W.cfg4_long_llada(n_layers=2)
+    st = make_step(handle, wl)
+    st.attention(); torch.cuda.synchronize()
+    out = to_np(st.out); lse = to_np(st.lse)
+    rng = np.random.default_rng(0)
+    worst = 0.0
+    for _ in range(96):
+        layer = int(rng.integers(0, wl.n_layers)); li = int(rng.integers(0, wl.n_lanes))
+        lane = wl.lanes[li]; r = int(rng.integers(0, lane[W.LANE_Q_LEN])); h = int(rng.integers(0, wl.n_q_heads))
+        ref, ref_lse = oracle.lane_attention_one(wl.q[layer], wl.k_new[layer], wl.v_new[layer], wl.k_cache[layer],
+                                                 wl.v_cache[layer], lane, r, h)
+        row = int(lane[W.LANE_Q_START]) + r
+        worst = max(worst, np.abs(out[layer, row, h] - ref).max() / np.abs(ref).max())
+        assert abs(lse[layer, row, h] - ref_lse) <= 1e-3
+    assert worst <= 1e-2, worst
+
+
+# ------------------------------------------------------------------------------------------------
+# refresh
+# ------------------------------------------------------------------------------------------------
+def check_refresh(handle, wl):
+    st = make_step(handle, wl)
+    kc = st.k_cache.clone(); vc = st.v_cache.clone()
+    st.refresh(); torch.cuda.synchronize()
+    # oracle on the very same bytes
+    kview = kc.view(torch.int16) if wl.dtype == "bf16" else kc
+    vview = vc.view(torch.int16) if wl.dtype == "bf16" else vc
+    ek, ev = kview.cpu().numpy().copy(), vview.cpu().numpy().copy()
+    ks = (st.k_src.view(torch.int16) if wl.dtype == "bf16" else st.k_src).cpu().numpy()
+    vs = (st.v_src.view(torch.int16) if wl.dtype == "bf16" else st.v_src).cpu().numpy()
+    oracle.kv_refresh(ek, ev, np.ascontiguousarray(ks), np.ascontiguousarray(vs), wl.refresh_pos, wl.refresh_base_row)
+    gk = (st.k_cache.view(torch.int16) if wl.dtype == "bf16" else st.k_cache).cpu().numpy()
+    gv = (st.v_cache.view(torch.int16) if wl.dtype == "bf16" else st.v_cache).cpu().numpy()
+    assert np.array_equal(gk.view(np.uint8), ek.view(np.uint8))
+    assert np.array_equal(gv.view(np.uint8), ev.view(np.uint8))
+    return st
+
+
+def test_refresh_bit_exact_cfg1_cfg2_cfg3(handle):
+    for wl in (W.cfg1_tiny(), W.cfg2_llada_layer(), W.cfg3_dream_layer()):
+        check_refresh(handle, wl)
+
+
+@pytest.mark.parametrize("seed", [201, 202])
+def test_refresh_bit_exact_ragged_and_multilayer(handle, seed):
+    check_refresh(handle, W.ragged_case(seed))
+    wl = W.build_workload("ml", seed, "bf16", 4, 2, 128, 5, 300,
+                          [dict(kv_base_row=0, prefix_len=100, q_lens=[8])], n_refresh=77, refresh_base_row=11,
+                          refresh_span=280, vocab=64, logit_sigma=1.0, planted_frac=0.0, mask_id=63, eos_id=-1,
+                          threshold=0.9)
+    check_refresh(handle, wl)
+
+
+def test_refresh_zero_positions_is_identity_and_all_rows_is_copy(handle):
+    wl = W.cfg1_tiny()
+    st = make_step(handle, wl)
+    before = st.k_cache.clone()
+    empty = torch.zeros(0, dtype=torch.int32, device=st.device)
+    handle.al_kv_refresh(st.shape, st.k_cache, st.v_cache, st.k_src, st.v_src, empty, 0)
+    torch.cuda.synchronize()
+    assert torch.equal(st.k_cache, before)
+    # all rows == memcpy of the transposed source
+    rows = wl.cache_rows
+    src_k = torch.randn(1, rows, wl.n_kv_heads, wl.head_dim, device=st.device)
+    src_v = torch.randn(1, rows, wl.n_kv_heads, wl.head_dim, device=st.device)
+    pos = torch.arange(rows, dtype=torch.int32, device=st.device)
+    handle.al_kv_refresh(st.shape, st.k_cache, st.v_cache, src_k, src_v, pos, rows)
+    torch.cuda.synchronize()
+    assert torch.equal(st.k_cache[0], src_k[0].permute(1, 0, 2))
+    assert torch.equal(st.v_cache[0], src_v[0].permute(1, 0, 2))
+
+
+def test_refresh_then_attention_composition(handle):
+    """Attention after a refresh equals the oracle run on the refreshed cache."""
+    wl = W.ragged_case(203)
+    st = make_step(handle, wl)
+    st.refresh(); st.attention(); torch.cuda.synchronize()
+    kc, vc = wl.k_cache.copy(), wl.v_cache.copy()
+    oracle.kv_refresh(kc, vc, wl.k_src, wl.v_src, wl.refresh_pos, wl.refresh_base_row)
+    ref, _ = oracle.lane_attention(wl.q[0], wl.k_new[0], wl.v_new[0], kc[0], vc[0], wl.lanes)
+    assert attn_errors(to_np(st.out)[0], ref) <= 1e-2
+
+
+# ------------------------------------------------------------------------------------------------
+# confidence / select
+# ------------------------------------------------------------------------------------------------
+def check_confidence(handle, wl, force_top1=False, max_exempt_frac=0.08):
+    st = make_step(handle, wl, force_top1=force_top1)
+    st.confidence(); torch.cuda.synchronize()
+    ref = oracle.confidence_select(wl.logits, wl.tokens, wl.mask_id, wl.eos_id, wl.threshold, wl.lanes, force_top1)
+    conf = to_np(st.conf); am = to_np(st.argmax); commit = to_np(st.commit); tok = to_np(st.tokens_out)
+    assert np.abs(conf - ref["conf"]).max() <= 2e-3
+    gap_ok = (ref["conf"] - ref["p2"]) > 1e-3
+    tau_ok = np.abs(ref["conf"] - wl.threshold) > 4e-3
+    # argmax: exact where the top-2 gap is clear; exact-tie rows must still pick a maximiser... and we
+    # require the FIRST one (reading C6), which the oracle also returns -> compare everywhere.
+    assert np.array_equal(am, ref["argmax"]), f"argmax differs on rows {np.nonzero(am != ref['argmax'])[0][:8]}"
+    sel = gap_ok & tau_ok
+    if not force_top1:
+        assert np.array_equal(commit[sel], ref["commit"][sel])
+        assert np.array_equal(tok[sel], ref["tokens_out"][sel])
+        assert np.array_equal(commit[tau_ok], ref["commit"][tau_ok])      # tie rows never commit at tau=0.9
+    else:
+        assert np.array_equal(commit, ref["commit"]) and np.array_equal(tok, ref["tokens_out"])
+    assert (~tau_ok).mean() <= max_exempt_frac
+    return st, ref
+
+
+def test_confidence_cfg1_tiny_fp32(handle):
+    st, ref = check_confidence(handle, W.cfg1_tiny())
+    assert np.abs(to_np(st.conf) - ref["conf"]).max() <= 1e-5
+    assert ref["commit"].sum() >= 1
+
+
+@pytest.mark.parametrize("seed", [301, 302, 303])
+def test_confidence_ragged_vocab_scalar_path_and_eos_suppression(handle, seed):
+    # vocab 4099 with row_stride 4099: rows are not 16-byte aligned -> element-wise path
+    check_confidence(handle, W.ragged_case(seed))
+
+
+def test_confidence_vector_path_with_tail_and_padded_stride(handle):
+    """row_stride multiple of 8 (aligned rows) but vocab % 8 != 0: vector body + scalar tail."""
+    from paper_2606_08411_b200 import binding as B
+    rng = np.random.default_rng(5)
+    N, V, stride = 37, 5003, 5008
+    x = W.round_to_bf16((rng.standard_normal((N, stride)) * 3).astype(np.float32))
+    x[:, V:] = 100.0                                       # padding must never be read
+    x[3, V - 1] = 30.0; x[4, V - 3] = 30.0; x[5, 0] = 30.0  # maxima inside the tail / at the start
+    tokens = np.full(N, 7, np.int32)
+    from paper_2606_08411_b200.step import to_device
+    dev = torch.device("cuda:0")
+    lg = to_device(x, "bf16", dev)
+    conf = torch.zeros(N, device=dev); am = torch.zeros(N, dtype=torch.int32, device=dev)
+    cm = torch.zeros(N, dtype=torch.uint8, device=dev); to = torch.zeros(N, dtype=torch.int32, device=dev)
+    ws = torch.empty(handle.al_confidence_select_workspace_bytes(N, V), dtype=torch.uint8, device=dev)
+    tk = torch.from_numpy(tokens).to(dev)
+    handle.al_confidence_select(lg, N, V, stride, tk, 7, -1, 0.9, None, 0, 0, conf, am, cm, to, ws)
+    torch.cuda.synchronize()
+    ref = oracle.confidence_select(np.ascontiguousarray(x[:, :V]), tokens, 7, -1, 0.9)
+    assert np.abs(to_np(conf) - ref["conf"]).max() <= 2e-3
+    assert np.array_equal(to_np(am), ref["argmax"])
+    assert np.array_equal(to_np(cm), ref["commit"])
+    assert list(to_np(am)[3:6]) == [V - 1, V - 3, 0]
+
+
+def test_confidence_cfg2_full_size(handle):
+    st, ref = check_confidence(handle, W.cfg2_llada_layer())
+    planted = np.zeros(128, bool); planted[W.cfg2_llada_layer().planted_rows] = True
+    assert (ref["conf"][planted] > 0.9).all() and (ref["conf"][~planted] < 0.5).all()
+
+
+def test_confidence_cfg3_full_size(handle):
+    check_confidence(handle, W.cfg3_dream_layer())
+
+
+def test_confidence_force_top1_and_ties(handle):
+    V = 1024
+    x = np.zeros((6, V), np.float32)
+    x[0, 1] = 1.0; x[1, 2] = 2.0; x[2, 3] = 2.0
+    x[3, 4] = 9.0; x[4, 5] = 1.0; x[5, 6] = 0.5; x[5, 900] = 0.5     # exact tie inside row 5: index 6 wins
+    lanes = np.array([[0, 0, 0, 0, 3, 0], [0, 0, 0, 3, 3, 0]], np.int32)
+    wl = W.cfg1_tiny()
+    wl.logits = x; wl.tokens = np.full(6, 1023, np.int32); wl.mask_id = 1023; wl.eos_id = -1; wl.lanes = lanes
+    wl.threshold = 0.9
+    st, ref = check_confidence(handle, wl, force_top1=True)
+    assert list(to_np(st.commit)) == [0, 1, 0, 1, 0, 0]
+    assert int(to_np(st.argmax)[5]) == 6
+
+
+def test_confidence_closed_forms_on_gpu(handle):
+    """all-equal row -> 1/V and argmax 0; (0,0,-inf...) -> exactly 0.5 and commits at tau 0.5 (>=)."""
+    V = 512
+    x = np.full((3, V), 1.25, np.float32)
+    x[1, :] = -np.inf; x[1, 3] = 0.0; x[1, 9] = 0.0
+    x[2, :] = 0.0; x[2, 137] = 8.0
+    wl = W.cfg1_tiny()
+    wl.logits = x; wl.tokens = np.full(3, 511, np.int32); wl.mask_id = 511; wl.eos_id = -1; wl.threshold = 0.5
+    wl.lanes = np.array([[0, 0, 0, 0, 3, 0]], np.int32)
+    st = make_step(handle, wl)
+    st.confidence(); torch.cuda.synchronize()
+    conf = to_np(st.conf)
+    assert conf[0] == pytest.approx(1.0 / 512, rel=1e-5) and int(to_np(st.argmax)[0]) == 0
+    assert conf[1] == 0.5 and int(to_np(st.argmax)[1]) == 3 and int(to_np(st.commit)[1]) == 1
+    assert conf[2] == pytest.approx(0.853664, abs=2e-5) and int(to_np(st.commit)[2]) == 1
+
+
+# ------------------------------------------------------------------------------------------------
+# whole step, ABI errors, tcgen05 self-test
+# ------------------------------------------------------------------------------------------------
+def test_whole_step_in_a_cuda_graph_matches_eager(handle):
+    wl = W.ragged_case(401)
+    st = make_step(handle, wl)
+    k0, v0 = st.k_cache.clone(), st.v_cache.clone()
+    st.run(); torch.cuda.synchronize()
+    eager = [st.out.clone(), st.conf.clone(), st.tokens_out.clone(), st.k_cache.clone()]
+    st.k_cache.copy_(k0); st.v_cache.copy_(v0); st.out.zero_(); st.conf.zero_()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            st.run(s)
+    st.k_cache.copy_(k0); st.v_cache.copy_(v0); st.out.zero_(); st.conf.zero_()
+    g.replay(); torch.cuda.synchronize()
+    assert torch.equal(st.out, eager[0]) and torch.equal(st.conf, eager[1])
+    assert torch.equal(st.tokens_out, eager[2]) and torch.equal(st.k_cache, eager[3])
+
+
+def test_abi_error_codes(handle):
+    from paper_2606_08411_b200 import binding as B
+    wl = W.cfg1_tiny()
+    st = make_step(handle, wl)
+    bad = B.Handle.make_shape(3, 2, 32, B.AL_F32, 96)            # H_q % H_kv != 0
+    with pytest.raises(B.AlError) as e:
+        handle.al_lane_attention(bad, st.q[0], st.k_new[0], st.v_new[0], st.k_cache[0], st.v_cache[0], st.lanes,
+                                 2, 16, 64, st.out[0])
+    assert e.value.status == B.AL_ERR_INVALID_ARG
+    with pytest.raises(B.AlError) as e:                          # workspace too small
+        handle.al_confidence_select(st.logits, st.N, st.V, st.V, st.tokens, 511, -1, 0.9, None, 0, 0, st.conf,
+                                    st.argmax, st.commit, st.tokens_out, torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == B.AL_ERR_WORKSPACE
+    with pytest.raises(B.AlError) as e:                          # row_stride < vocab
+        handle.al_confidence_select(st.logits, st.N, st.V, st.V - 1, st.tokens, 511, -1, 0.9, None, 0, 0, st.conf,
+                                    st.argmax, st.commit, st.tokens_out, st.ws_conf)
+    assert e.value.status == B.AL_ERR_INVALID_ARG
+    # empty calls are valid no-ops
+    handle.al_lane_attention(st.shape, st.q[0], st.k_new[0], st.v_new[0], st.k_cache[0], st.v_cache[0], st.lanes,
+                             0, 0, 0, st.out[0])
+    handle.al_validate_lanes(st.shape, st.lanes, 2, 16)
+    overl = st.lanes.clone(); overl[1, 3] = 4                    # q_start of lane 1 overlaps lane 0
+    with pytest.raises(B.AlError):
+        handle.al_validate_lanes(st.shape, overl, 2, 16)
+    with pytest.raises(TypeError):                               # host tensors are rejected: no CPU path
+        handle.al_kv_refresh(st.shape, st.k_cache.cpu(), st.v_cache, st.k_src, st.v_src, st.pos, 4)
+
+
+def test_tcgen05_selftest_tile(handle):
+    """S = A.B^T and O = bf16(S*c).V on one 128^3 tile: validates the TMA swizzle, smem/instruction
+    descriptors and the TMEM operand path against a float64 matmul."""
+    rng = np.random.default_rng(11)
+    a = W.round_to_bf16(rng.standard_normal((128, 128)).astype(np.float32))
+    b = W.round_to_bf16(rng.standard_normal((128, 128)).astype(np.float32))
+    v = W.round_to_bf16(rng.standard_normal((128, 128)).astype(np.float32))
+    from paper_2606_08411_b200.step import to_device
+    dev = torch.device("cuda:0")
+    s_out = torch.zeros(128, 128, device=dev); o_out = torch.zeros(128, 128, device=dev)
+    c = 1.0 / 16
+    handle.al_selftest_umma(to_device(a, "bf16", dev), to_device(b, "bf16", dev), to_device(v, "bf16", dev), c,
+                            s_out, o_out)
+    S = a.astype(np.float64) @ b.astype(np.float64).T
+    assert np.abs(to_np(s_out) - S).max() <= 1e-3 * np.abs(S).max()
+    P = W.round_to_bf16((to_np(s_out) * np.float32(c)).astype(np.float32)).astype(np.float64)
+    O = P @ v.astype(np.float64)
+    assert np.abs(to_np(o_out) - O).max() <= 1e-3 * np.abs(O).max()
