@@ -1,0 +1,410 @@
+#!/usr/bin/env python
+"""bench.py -- the lane-batched denoising step of AsyncLane on B200, measured.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is ONE pass of the whole hot path (lane attention for every layer of the
+workload, compact KV refresh, confidence/argmax/threshold select) over one batch of seeded
+synthetic input.  The default workload is BASELINE.json configs[1] (LLaDA-8B-shaped single layer).
+
+What is timed:
+  value     K steps, inputs resident in HBM, each step one CUDA-graph replay; consecutive steps run
+            on DISTINCT copies of every streamed buffer (rotation set > 2x L2) so nothing is served
+            from L2.  Device time from CUDA events on the launching stream, max over ranks.
+  roofline  per-part device time from timing events captured INSIDE those graphs (external event
+            record nodes), read for the last replay of every copy in the timed region.
+  e2e       the same step through the C-ABI host entry al_lane_step_host: every step copies its
+            inputs from pinned host memory, runs the kernels and copies the results back.
+  cpu_baseline / --impl reference   the CPU oracle (oracle/, fp64, as it stands) on the host cores.
+
+Multi-GPU: the path does not shard (BASELINE north_star: one GPU, no collectives) -> "replicas
+only": every rank runs an independent replica, value = all ranks' tokens / max-over-ranks time.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+L2_BYTES = 126e6
+METRIC = "lane-step query tok/s (parts: attention TFLOP/s, refresh+confidence GB/s vs peak)"
+UNIT = "query tok/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm=float(p["hbm_gbs"]), tensor=float(p["bf16_tflops"]),
+                    tensor_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])), source="measured")
+    # fallback stated by /opt/skills/guides/B200_PROFILING.md
+    return dict(hbm=6650.0, tensor=1590.0, tensor_sustained=1400.0, source="fallback")
+
+
+def load_traffic(workload: str):
+    """dram bytes per launch from the committed ncu --set full capture (profiles/), if any."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(path):
+        try:
+            return json.load(open(path)).get(workload, {})
+        except Exception:
+            return {}
+    return {}
+
+
+# --------------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """Samples SM clock and clock-event reasons through NVML while the timed regions run."""
+
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int, period_s: float = 0.002):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period_s
+        self.samples, self.reason_bits, self.power = [], 0, []
+        self.active = threading.Event()
+        self.stop_flag = threading.Event()
+        self.ok = False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag.is_set():
+            if self.active.is_set():
+                try:
+                    self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM)))
+                    try:
+                        r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev))
+                    except Exception:
+                        r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev))
+                    self.reason_bits |= r
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.dev) / 1000.0)
+                except Exception:
+                    pass
+            time.sleep(self.period)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unsampled"], "samples": 0}
+        s = sorted(self.samples)
+        reasons = [n for b, n in self.REASONS.items() if (self.reason_bits & b) and n != "gpu_idle"]
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": reasons,
+                "samples": len(s), "power_w_max": round(max(self.power), 1) if self.power else None}
+
+
+# --------------------------------------------------------------------------------------------------
+def oracle_step(oracle, wl, lanes, rows):
+    """One pass of the hot path on the CPU oracle over whole lanes `lanes` / logits rows `rows`."""
+    for layer in range(wl.n_layers):
+        oracle.lane_attention(wl.q[layer], wl.k_new[layer], wl.v_new[layer], wl.k_cache[layer], wl.v_cache[layer],
+                              lanes)
+    kc, vc = wl.k_cache, wl.v_cache            # in place: the oracle's refresh is idempotent
+    oracle.kv_refresh(kc, vc, wl.k_src, wl.v_src, wl.refresh_pos, wl.refresh_base_row)
+    r0, r1 = (int(rows.min()), int(rows.max()) + 1) if len(rows) else (0, 0)     # dense: a view, no copy
+    oracle.confidence_select(wl.logits[r0:r1], wl.tokens[r0:r1], wl.mask_id, wl.eos_id, wl.threshold, None)
+
+
+def time_oracle(wl, steps: int, warmup: int, budget_s: float):
+    """Times the oracle on a bounded sample: the first n whole lanes (lanes are independent)
+    and the logits rows of those lanes, n chosen so that steps+warmup passes fit in `budget_s`."""
+    import numpy as np
+    import oracle
+    from paper_2606_08411_b200 import workloads as W
+    oracle.build()
+    cores = oracle.num_threads()
+    one = wl.lanes[:1]
+    rows1 = np.arange(int(one[0, W.LANE_Q_START]), int(one[0, W.LANE_Q_START] + one[0, W.LANE_Q_LEN]))
+    rows1 = rows1[rows1 < wl.logits.shape[0]]
+    oracle_step(oracle, wl, one, rows1)                       # page-in, thread pool start
+    t0 = time.perf_counter()
+    oracle_step(oracle, wl, one, rows1)
+    t_lane = max(time.perf_counter() - t0, 1e-4)
+    n = int(max(1, min(wl.n_lanes, (budget_s / max(1, steps + warmup)) / t_lane)))
+    lanes = wl.lanes[:n]
+    rows = np.concatenate([np.arange(int(l[W.LANE_Q_START]), int(l[W.LANE_Q_START] + l[W.LANE_Q_LEN])) for l in lanes])
+    rows = rows[rows < wl.logits.shape[0]]
+    tokens = int(lanes[:, W.LANE_Q_LEN].sum())
+    for _ in range(warmup):
+        oracle_step(oracle, wl, lanes, rows)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(oracle, wl, lanes, rows)
+    dt = time.perf_counter() - t0
+    sample = (f"{n} of {wl.n_lanes} whole lanes ({tokens} of {wl.total_q_rows} query rows; all heads, all "
+              f"{wl.n_layers} layer(s)) + their {rows.size} logits rows + the full refresh, {steps} passes")
+    return dict(value=tokens * steps / dt, unit=UNIT, cores=cores, kind="oracle", sample=sample), dt / steps
+
+
+# --------------------------------------------------------------------------------------------------
+def run_reference(args, rank: int):
+    if rank != 0:
+        return
+    from paper_2606_08411_b200 import workloads as W
+    wl = W.CONFIGS[args.workload]()
+    cpu, s_per_step = time_oracle(wl, args.steps, args.warmup, budget_s=150.0)
+    line = {"impl": "reference", "metric": METRIC, "value": cpu["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": s_per_step * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": wl.name, "note": "CPU oracle (oracle/) on the host cores"},
+            "cpu_baseline": cpu,
+            "e2e": {"value": cpu["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+def run_ours(args, rank: int, local_rank: int, world: int):
+    import numpy as np
+    import torch
+    from paper_2606_08411_b200 import accounting, binding, workloads as W
+    from paper_2606_08411_b200.step import LaneStep, to_host_pinned
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the library has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    peaks = load_peaks()
+    wl = W.CONFIGS[args.workload]()
+    acc = accounting.summary(wl)
+    h = binding.Handle(local_rank)
+
+    # ---- resident copies: rotation set larger than 2x L2 ---------------------------------------
+    first = LaneStep(h, wl, device=dev, want_lse=False)
+    per_copy = first.streamed_bytes()
+    n_copies = max(2, int(math.ceil(2.2 * L2_BYTES / per_copy)))
+    copies = [first] + [first.replicate() for _ in range(n_copies - 1)]
+    stream = torch.cuda.Stream(device=dev)
+
+    # ---- one CUDA graph per copy, timing marks captured as external event-record nodes ---------
+    graphs, marks = [], []
+    launches_per_step = None
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        copies[0].run(stream)                                  # load modules / set attributes before capture
+        stream.synchronize()
+        for st in copies:
+            ev = [torch.cuda.Event(enable_timing=True, external=True) for _ in range(4)] if args.kernel_events else None
+            g = torch.cuda.CUDAGraph()
+            before = h.al_launch_count
+            with torch.cuda.graph(g, stream=stream):
+                st.run(stream, marks=ev)
+            launches_per_step = h.al_launch_count - before
+            graphs.append(g)
+            marks.append(ev)
+    stream.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up, then EXACTLY K timed steps ------------------------------------------------------
+    with torch.cuda.stream(stream):
+        for i in range(args.warmup):
+            graphs[i % n_copies].replay()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.active.set()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for i in range(args.steps):
+            graphs[i % n_copies].replay()
+        e1.record(stream)
+    barrier()
+    sampler.active.clear()
+    step_ms = e0.elapsed_time(e1) / args.steps
+
+    # per-part device times: the marks of every copy hold its LAST replay inside the timed region
+    part_ms = None
+    if args.kernel_events:
+        used = [c for c in range(n_copies) if c < args.steps]
+        a = np.array([[marks[c][j].elapsed_time(marks[c][j + 1]) for j in range(3)] for c in used])
+        part_ms = dict(zip(("attention", "refresh", "confidence"), a.mean(axis=0).tolist()))
+        part_ms["n_samples"] = len(used)
+
+    t = torch.tensor([step_ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    step_ms_max = float(t.item())
+    value = world * acc["query_tokens"] / (step_ms_max * 1e-3)
+
+    # ---- e2e: host buffers through al_lane_step_host ----------------------------------------------
+    hs = binding.al_host_step()
+    host = {}
+
+    def pin(name, arr, dtype=None):
+        tt = to_host_pinned(arr, dtype) if dtype else torch.from_numpy(np.ascontiguousarray(arr)).pin_memory()
+        host[name] = tt
+        return tt.data_ptr()
+
+    layer0 = 0
+    hs.q = pin("q", wl.q[layer0], wl.dtype)
+    hs.k_new = pin("k_new", wl.k_new[layer0], wl.dtype)
+    hs.v_new = pin("v_new", wl.v_new[layer0], wl.dtype)
+    hs.lanes = pin("lanes", wl.lanes.astype(np.int32))
+    hs.n_lanes, hs.total_q_rows, hs.max_prefix_len = wl.n_lanes, wl.total_q_rows, wl.max_prefix_len
+    hs.k_src = pin("k_src", wl.k_src[layer0], wl.dtype)
+    hs.v_src = pin("v_src", wl.v_src[layer0], wl.dtype)
+    hs.pos = pin("pos", wl.refresh_pos.astype(np.int32))
+    hs.n_pos, hs.refresh_base_row = int(wl.refresh_pos.size), wl.refresh_base_row
+    hs.logits = pin("logits", wl.logits, wl.dtype)
+    hs.n_rows, hs.vocab = wl.logits.shape
+    hs.tokens_in = pin("tokens", wl.tokens.astype(np.int32))
+    hs.mask_id, hs.eos_id, hs.threshold, hs.select_flags = wl.mask_id, wl.eos_id, float(wl.threshold), 0
+    tdt = torch.bfloat16 if wl.dtype == "bf16" else torch.float32
+    host["out"] = torch.empty((wl.total_q_rows, wl.n_q_heads, wl.head_dim), dtype=tdt).pin_memory()
+    host["conf"] = torch.empty(hs.n_rows, dtype=torch.float32).pin_memory()
+    host["argmax"] = torch.empty(hs.n_rows, dtype=torch.int32).pin_memory()
+    host["commit"] = torch.empty(hs.n_rows, dtype=torch.uint8).pin_memory()
+    host["tokens_out"] = torch.empty(hs.n_rows, dtype=torch.int32).pin_memory()
+    hs.out, hs.conf, hs.argmax = host["out"].data_ptr(), host["conf"].data_ptr(), host["argmax"].data_ptr()
+    hs.commit, hs.tokens_out = host["commit"].data_ptr(), host["tokens_out"].data_ptr()
+    arena = torch.empty(h.al_lane_step_host_arena_bytes(first.shape, hs) + 256, dtype=torch.uint8, device=dev)
+    h2d, d2h = h.al_lane_step_host_traffic(first.shape, hs)
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    before = h.al_launch_count
+    with torch.cuda.stream(stream):
+        for i in range(min(3, args.warmup) or 1):
+            c = copies[i % n_copies]
+            h.al_lane_step_host(first.shape, hs, c.k_cache[layer0], c.v_cache[layer0], arena, stream)
+    e2e_launches = (h.al_launch_count - before) // (min(3, args.warmup) or 1)
+    barrier()
+    sampler.active.set()
+    t0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for i in range(e2e_steps):
+            c = copies[i % n_copies]
+            h.al_lane_step_host(first.shape, hs, c.k_cache[layer0], c.v_cache[layer0], arena, stream)
+        e1.record(stream)
+    barrier()
+    wall_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    sampler.active.clear()
+    e2e_ms = max(e0.elapsed_time(e1) / e2e_steps, wall_ms)       # host-visible completion time
+    t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item())
+    e2e_tokens = wl.total_q_rows                                  # one layer of the workload per host step
+    sampler.stop_flag.set()
+    sampler.join(timeout=2)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of every part; `roofline` = the part with the largest share of the step ------
+    traffic = load_traffic(wl.name)
+    parts = {}
+    if part_ms:
+        ai = acc["attn_flops"] / acc["attn_bytes"]
+        ridge = peaks["tensor"] * 1e12 / (peaks["hbm"] * 1e9)
+        ta, tr, tc = (part_ms[k] * 1e-3 for k in ("attention", "refresh", "confidence"))
+        n_attn_launch = wl.n_layers
+        if ai < ridge:
+            parts["attention"] = dict(bound="hbm", achieved=acc["attn_bytes"] / ta / 1e9, peak=peaks["hbm"], unit="GB/s")
+        else:
+            parts["attention"] = dict(bound="tensor", achieved=acc["attn_flops"] / ta / 1e12, peak=peaks["tensor"],
+                                      unit="TFLOP/s")
+        parts["attention"].update(ms=ta * 1e3, launches=n_attn_launch, tflops=acc["attn_flops"] / ta / 1e12,
+                                  gbs=acc["attn_bytes"] / ta / 1e9, arithmetic_intensity=ai)
+        parts["refresh"] = dict(bound="hbm", achieved=acc["refresh_bytes"] / tr / 1e9, peak=peaks["hbm"], unit="GB/s",
+                                ms=tr * 1e3, launches=1)
+        parts["confidence"] = dict(bound="hbm", achieved=acc["confidence_bytes"] / tc / 1e9, peak=peaks["hbm"],
+                                   unit="GB/s", ms=tc * 1e3, launches=2)
+        for k, p in parts.items():
+            p["frac"] = p["achieved"] / p["peak"]
+            p["traffic"] = traffic.get(k)
+            p["share_of_step"] = p["ms"] / (step_ms)
+        dom = max(parts, key=lambda k: parts[k]["ms"])
+        roofline = {k: parts[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")}
+        roofline.update(kernel=dom, peak_source=peaks["source"], avg_launch_ms=parts[dom]["ms"] / parts[dom]["launches"],
+                        timed_with="CUDA events captured in the step graphs, last replay of each copy in the timed region")
+    else:
+        roofline = None
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu, _ = time_oracle(wl, steps=args.cpu_steps, warmup=1, budget_s=args.cpu_budget)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": step_ms_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": wl.dtype, "data": "synthetic",
+        "config": {"workload": wl.name, "layers": wl.n_layers, "lanes": wl.n_lanes, "groups": wl.n_groups,
+                   "query_rows": wl.total_q_rows, "heads": f"{wl.n_q_heads}q/{wl.n_kv_heads}kv", "head_dim": wl.head_dim,
+                   "max_prefix": wl.max_prefix_len, "refresh_rows": int(wl.refresh_pos.size),
+                   "logits": list(wl.logits.shape), "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "l2": f"rotating {n_copies} resident copies of every streamed buffer "
+                         f"({n_copies * per_copy / 1e6:.0f} MB > 2x 126 MB L2), one CUDA graph per step"},
+        "clocks": sampler.summary(),
+        "e2e": {"value": world * e2e_tokens / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                "api": "al_lane_step_host (pinned host buffers; H2D + kernels + D2H per step)",
+                "gpu_launches_per_step": e2e_launches},
+        "gpu_launches": launches_per_step * args.steps,
+        "roofline": roofline, "parts": parts, "cpu_baseline": cpu,
+        "algorithmic": acc, "peaks": peaks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--e2e-steps", type=int, default=100)
+    ap.add_argument("--cpu-steps", type=int, default=20)
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-kernel-events", dest="kernel_events", action="store_false")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -156,6 +156,54 @@ al_status al_confidence_select(al_handle* handle, const void* logits, int32_t lo
                                uint8_t* commit_out, int32_t* tokens_out, void* workspace,
                                size_t workspace_bytes, void* cuda_stream);
 
+/* ---- whole step from HOST buffers (end-to-end entry) ------------------------------------------ */
+
+/*
+ * One lane-batched denoising step (one layer) whose per-step inputs and
+ * results live in HOST memory (pinned for true asynchrony): the call enqueues, on `cuda_stream`,
+ * the host->device copies of the inputs into `arena_dev`, then al_lane_attention, al_kv_refresh and
+ * al_confidence_select on the device copies, then the device->host copies of the results.  It does
+ * not synchronise: the caller synchronises the stream before reading the outputs or reusing the
+ * host inputs.  The KV cache is persistent device state (kappa_l is carried between
+ * iterations) and is passed as device pointers; attention reads it before this step's refresh
+ * writes it.  Every pointer inside al_host_step is a HOST pointer owned by the caller.
+ */
+typedef struct {
+  const void* q;            /* [T][H_q][d]                                  */
+  const void* k_new;        /* [T][H_kv][d]                                 */
+  const void* v_new;        /* [T][H_kv][d]                                 */
+  const al_lane_desc* lanes;/* [n_lanes]                                    */
+  int32_t n_lanes, total_q_rows, max_prefix_len;
+  const void* k_src;        /* [n_pos][H_kv][d] recomputed rows (Eq.12)     */
+  const void* v_src;
+  const int32_t* pos;       /* [n_pos] strictly increasing                  */
+  int32_t n_pos, refresh_base_row;
+  const void* logits;       /* [n_rows][vocab], dtype = shape->dtype        */
+  int32_t n_rows, vocab;
+  const int32_t* tokens_in; /* [n_rows]                                     */
+  int32_t mask_id, eos_id;
+  float threshold;
+  int32_t select_flags;     /* AL_SELECT_*                                  */
+  void* out;                /* [T][H_q][d]   result, host                   */
+  float* conf;              /* [n_rows]                                     */
+  int32_t* argmax;          /* [n_rows]                                     */
+  uint8_t* commit;          /* [n_rows]                                     */
+  int32_t* tokens_out;      /* [n_rows]                                     */
+} al_host_step;
+
+/* Bytes of device scratch al_lane_step_host needs for these sizes (0 on invalid arguments). */
+size_t al_lane_step_host_arena_bytes(const al_attn_shape* shape, const al_host_step* step);
+al_status al_lane_step_host(al_handle* handle, const al_attn_shape* shape, const al_host_step* step,
+                            void* k_cache_dev, void* v_cache_dev, void* arena_dev,
+                            size_t arena_bytes, void* cuda_stream);
+/* Bytes copied host->device / device->host by one al_lane_step_host call with these sizes. */
+void al_lane_step_host_traffic(const al_attn_shape* shape, const al_host_step* step,
+                               uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+
+/* Number of kernel launches this handle has enqueued so far (bench accounting; a captured graph
+ * counts its launches once, at capture). */
+uint64_t al_launch_count(const al_handle* handle);
+
 /* ---- debug / self-test (synchronising; never on the hot path) --------------------------------- */
 
 /* Copies the descriptors to the host and checks the preconditions listed above.  Synchronises. */

@@ -22,7 +22,8 @@ EXPORTS = [
     "al_create", "al_destroy", "al_last_error", "al_version", "al_sm_count",
     "al_lane_attention_workspace_bytes", "al_lane_attention", "al_kv_refresh",
     "al_confidence_select_workspace_bytes", "al_confidence_select", "al_validate_lanes",
-    "al_selftest_umma",
+    "al_selftest_umma", "al_lane_step_host", "al_lane_step_host_arena_bytes", "al_lane_step_host_traffic",
+    "al_launch_count",
 ]
 
 
@@ -36,6 +37,20 @@ class al_attn_shape(ctypes.Structure):
     _fields_ = [("n_q_heads", ctypes.c_int32), ("n_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
                 ("dtype", ctypes.c_int32), ("cache_rows", ctypes.c_int64), ("scale", ctypes.c_float),
                 ("reserved", ctypes.c_int32)]
+
+
+class al_host_step(ctypes.Structure):
+    """Mirror of al_host_step (include/asynclane.h): HOST pointers of one step's inputs and results."""
+    _fields_ = [("q", ctypes.c_void_p), ("k_new", ctypes.c_void_p), ("v_new", ctypes.c_void_p),
+                ("lanes", ctypes.c_void_p), ("n_lanes", ctypes.c_int32), ("total_q_rows", ctypes.c_int32),
+                ("max_prefix_len", ctypes.c_int32),
+                ("k_src", ctypes.c_void_p), ("v_src", ctypes.c_void_p), ("pos", ctypes.c_void_p),
+                ("n_pos", ctypes.c_int32), ("refresh_base_row", ctypes.c_int32),
+                ("logits", ctypes.c_void_p), ("n_rows", ctypes.c_int32), ("vocab", ctypes.c_int32),
+                ("tokens_in", ctypes.c_void_p), ("mask_id", ctypes.c_int32), ("eos_id", ctypes.c_int32),
+                ("threshold", ctypes.c_float), ("select_flags", ctypes.c_int32),
+                ("out", ctypes.c_void_p), ("conf", ctypes.c_void_p), ("argmax", ctypes.c_void_p),
+                ("commit", ctypes.c_void_p), ("tokens_out", ctypes.c_void_p)]
 
 
 _lib: Optional[ctypes.CDLL] = None
@@ -70,10 +85,20 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
                                          vp, vp, vp, vp, vp, sz, vp]
     lib.al_validate_lanes.argtypes = [vp, shp, vp, i32, i32]
     lib.al_selftest_umma.argtypes = [vp, vp, vp, vp, f32, vp, vp, vp]
+    hsp = ctypes.POINTER(al_host_step)
+    lib.al_lane_step_host_arena_bytes.argtypes = [shp, hsp]
+    lib.al_lane_step_host_arena_bytes.restype = sz
+    lib.al_lane_step_host.argtypes = [vp, shp, hsp, vp, vp, vp, sz, vp]
+    lib.al_lane_step_host_traffic.argtypes = [shp, hsp, ctypes.POINTER(ctypes.c_uint64),
+                                              ctypes.POINTER(ctypes.c_uint64)]
+    lib.al_lane_step_host_traffic.restype = None
+    lib.al_launch_count.argtypes = [vp]
+    lib.al_launch_count.restype = ctypes.c_uint64
     for name in EXPORTS:
         fn = getattr(lib, name)
         if name not in ("al_last_error", "al_version", "al_sm_count", "al_lane_attention_workspace_bytes",
-                        "al_confidence_select_workspace_bytes"):
+                        "al_confidence_select_workspace_bytes", "al_lane_step_host_arena_bytes",
+                        "al_lane_step_host_traffic", "al_launch_count"):
             fn.restype = ctypes.c_int
     _lib = lib
     return lib
@@ -171,6 +196,24 @@ class Handle:
                                               _ptr(lanes_dev), n_lanes, flags, _ptr(conf_out), _ptr(argmax_out),
                                               _ptr(commit_out), _ptr(tokens_out), _ptr(workspace), ws_bytes,
                                               _stream_ptr(stream)))
+
+    @property
+    def al_launch_count(self) -> int:
+        return int(self._lib.al_launch_count(self._h))
+
+    def al_lane_step_host_arena_bytes(self, shape: al_attn_shape, step: al_host_step) -> int:
+        return int(self._lib.al_lane_step_host_arena_bytes(ctypes.byref(shape), ctypes.byref(step)))
+
+    def al_lane_step_host_traffic(self, shape: al_attn_shape, step: al_host_step):
+        a, b = ctypes.c_uint64(0), ctypes.c_uint64(0)
+        self._lib.al_lane_step_host_traffic(ctypes.byref(shape), ctypes.byref(step), ctypes.byref(a), ctypes.byref(b))
+        return int(a.value), int(b.value)
+
+    def al_lane_step_host(self, shape, step: al_host_step, k_cache, v_cache, arena, stream=None) -> None:
+        """`step` holds HOST pointers (pinned torch tensors' data_ptr()); caches/arena are CUDA tensors."""
+        _check(self._lib.al_lane_step_host(self._h, ctypes.byref(shape), ctypes.byref(step), _ptr(k_cache),
+                                           _ptr(v_cache), _ptr(arena), arena.numel() * arena.element_size(),
+                                           _stream_ptr(stream)))
 
     def al_validate_lanes(self, shape, lanes_dev, n_lanes, total_q_rows) -> None:
         _check(self._lib.al_validate_lanes(self._h, ctypes.byref(shape), _ptr(lanes_dev), n_lanes, total_q_rows))

@@ -59,6 +59,7 @@ extern "C" al_status al_destroy(al_handle* h) {
 }
 
 extern "C" int32_t al_sm_count(const al_handle* h) { return h ? h->sm_count : 0; }
+extern "C" uint64_t al_launch_count(const al_handle* h) { return h ? h->launches.load() : 0; }
 
 static al_status check_shape(const al_attn_shape* s, const char* who) {
   if (!s) AL_FAIL(AL_ERR_INVALID_ARG, "%s: shape is NULL", who);

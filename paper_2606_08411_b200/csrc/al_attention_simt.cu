@@ -116,7 +116,7 @@ al_status al_launch_attention_simt(const al_handle* h, const al_attn_shape* s, f
                                    const void* k_cache, const void* v_cache,
                                    const al_lane_desc* lanes, int n_lanes, int total_q_rows,
                                    void* out, float* lse, cudaStream_t st) {
-  (void)h;
+  h->launches++;
   const size_t smem = (size_t)kWarps * s->head_dim * sizeof(float);
   const float scale_log2 = scale * kLog2e;
   if (s->dtype == AL_F32) {

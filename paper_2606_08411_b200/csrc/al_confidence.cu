@@ -288,6 +288,7 @@ extern "C" al_status al_confidence_select(al_handle* h, const void* logits, int3
   else                  { if (vec) AL_LAUNCH_PARTIAL(float, true);         else AL_LAUNCH_PARTIAL(float, false); }
 #undef AL_LAUNCH_PARTIAL
   AL_CUDA_OK(cudaGetLastError());
+  h->launches += 2;
   const int fin_blocks = (n_rows + warps_per_block - 1) / warps_per_block;
   confidence_finalize_kernel<<<fin_blocks, kThreads, 0, cs>>>(parts, n_rows, ipr, tokens_in, mask_id, threshold,
                                                                conf_out, argmax_out, commit_out, tokens_out);
@@ -297,6 +298,7 @@ extern "C" al_status al_confidence_select(al_handle* h, const void* logits, int3
     force_top1_kernel<<<(nl + warps_per_block - 1) / warps_per_block, kThreads, 0, cs>>>(
         lanes_eff, nl, n_rows, mask_id, conf_out, argmax_out, commit_out, tokens_out);
     AL_CUDA_OK(cudaGetLastError());
+    h->launches++;
   }
   return AL_OK;
 }

@@ -3,6 +3,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
@@ -14,6 +15,7 @@ struct al_handle {
   int sm_count;
   int cc_major, cc_minor;
   size_t smem_optin;
+  mutable std::atomic<uint64_t> launches{0};   // kernels enqueued through this handle
   // cuTensorMapEncodeTiled resolved through the runtime (no -lcuda at link time)
   CUresult (*encode_tiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                            const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,

@@ -89,6 +89,7 @@ extern "C" al_status al_kv_refresh(al_handle* h, const al_attn_shape* s, void* k
   long long blocks = (total + (long long)kThreads * kUnroll - 1) / ((long long)kThreads * kUnroll);
   const long long cap = (long long)h->sm_count * 16;       // grid-stride beyond 16 CTAs per SM
   if (blocks > cap) blocks = cap;
+  h->launches++;
   kv_refresh_kernel<<<(unsigned)blocks, kThreads, 0, static_cast<cudaStream_t>(stream)>>>(
       (int4*)k_cache, (int4*)v_cache, (const int4*)k_src, (const int4*)v_src, pos_dev, n_pos,
       kv_base_row, s->n_kv_heads, (long long)s->cache_rows, vpr, layer_stride_cache * esz / 16,

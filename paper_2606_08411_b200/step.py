@@ -71,6 +71,25 @@ class LaneStep:
         self.flags = B.AL_SELECT_FORCE_TOP1 if force_top1 else 0
         self.gpu_launches_per_step = None   # filled by callers that count (bench)
 
+    def replicate(self) -> "LaneStep":
+        """A second instance on DISTINCT device allocations of every streamed buffer (same values):
+        bench.py rotates over such copies so that consecutive steps never hit in L2."""
+        import copy
+        r = copy.copy(self)
+        for name in ("q", "k_new", "v_new", "k_cache", "v_cache", "k_src", "v_src", "logits", "out", "lse",
+                     "conf", "argmax", "commit", "tokens_out", "ws_attn", "ws_conf"):
+            t = getattr(self, name)
+            setattr(r, name, None if t is None else t.clone())
+        return r
+
+    def streamed_bytes(self) -> int:
+        """Device bytes one step streams (inputs + caches + outputs), for sizing the L2 rotation."""
+        tot = 0
+        for name in ("q", "k_new", "v_new", "k_cache", "v_cache", "k_src", "v_src", "logits", "out"):
+            t = getattr(self, name)
+            tot += t.numel() * t.element_size()
+        return tot
+
     # -- the three parts ---------------------------------------------------------------------------
     def attention(self, stream=None, layers: Optional[range] = None) -> None:
         wl = self.wl
@@ -94,9 +113,19 @@ class LaneStep:
                                     float(wl.threshold), self.lanes, wl.n_lanes, self.flags, self.conf,
                                     self.argmax, self.commit, self.tokens_out, self.ws_conf, stream)
 
-    def run(self, stream=None) -> None:
+    def run(self, stream=None, marks=None) -> None:
         """The whole hot path once.  Attention reads the cache BEFORE this step's refresh writes it
-        (kappa_l is the state the lanes were forked from; refresh is periodic, L176)."""
+        (kappa_l is the state the lanes were forked from; refresh is periodic, L176).
+        `marks`: optional 4 timing events recorded before/between/after the three parts."""
+        s = torch.cuda.current_stream() if stream is None else stream
+        if marks is not None:
+            marks[0].record(s)
         self.attention(stream)
+        if marks is not None:
+            marks[1].record(s)
         self.refresh(stream)
+        if marks is not None:
+            marks[2].record(s)
         self.confidence(stream)
+        if marks is not None:
+            marks[3].record(s)
