@@ -1,30 +1,41 @@
 // al_confidence_select -- per-position vocab softmax confidence / argmax / threshold unmask select
 // (q_i and x^_i of Eq.8).
 //
-// K3  confidence_partial: HBM-bound stream over logits [N][V].  A work item is one CHUNK of one row
-//     (256 16-byte vectors = 4 KB); each WARP owns whole items (grid-stride), issues its 8 128-bit
-//     streaming loads per lane up front, folds them into a per-lane online (max, sum-exp, first
-//     argmax), reduces across the warp with shuffles and writes one 16-byte partial.  No block-level
-//     synchronisation, no shared memory.  Algorithmic bytes: N*V*esz (+ 14 N of outputs).
-// K3b confidence_finalize: one warp per row merges the row's partials with the associative combine
-//     (m, s, i): m' = max, s' = s1 e^{m1-m'} + s2 e^{m2-m'}, i' = index of the larger m (lower index
-//     on ties) and applies the commit rule; K3c force_top1: one warp per lane (optional flag).
+// K3  confidence_select_kernel: ONE launch, HBM-bound stream over logits [N][V].
+//     A thread-block CLUSTER of k CTAs (k in {1,2,4,8}, chosen on the host so that N*k CTAs fill the
+//     148 SMs) owns one row; CTA c streams the c-th contiguous chunk of the row.  A warp folds 4 KB
+//     items (8 x 16-byte streaming loads per lane, the next item's loads issued before the current
+//     item is reduced) in two register passes:
+//       pass A  packed bf16x2 max over the lane's 64 values -> warp max through one REDUX
+//       pass B  sum += ex2(x*log2e - m*log2e): unpack, FFMA, MUFU.EX2, FADD per element
+//     keeping a warp-uniform running max m (rescaling the sum only when an item raises it) and the
+//     first index attaining it.  Warps merge through shared memory, the CTAs of a cluster merge in
+//     the leader's shared memory over DSMEM, and the leader applies the commit rule: no partials in
+//     HBM, no second launch, no atomics.  Algorithmic bytes: N*V*esz (+ 17 N of tokens/outputs).
+//     Merge op on (m, s, i): m' = max, s' = s1 e^{m1-m'} + s2 e^{m2-m'}, i' = index of the larger
+//     m, lower index on ties -- associative, so the argmax is the first maximiser in any order.
+// K3c force_top1: one warp per lane (optional flag, reading C4 of DESIGN.md).
+#include <cooperative_groups.h>
 #include <cuda_bf16.h>
 
 #include "al_internal.h"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
 constexpr int kWarpVecs = 8;                 // 16-byte vectors per lane per item
 constexpr int kItemVecs = 32 * kWarpVecs;    // 256 vectors = 4 KB per item
 constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kMaxCluster = 8;
 constexpr float kLog2e = 1.4426950408889634f;
+constexpr int kNoIdx = 0x7fffffff;
 
-struct __align__(16) Partial {
+struct Triple {
   float m;   // running max (natural units)
   float s;   // sum exp(x - m)
   int idx;   // first index attaining m
-  int pad;
 };
 
 __device__ __forceinline__ int4 ld_stream(const void* p) {
@@ -34,10 +45,42 @@ __device__ __forceinline__ int4 ld_stream(const void* p) {
                : "l"(p));
   return r;
 }
+__device__ __forceinline__ float ex2(float x) {           // x <= 0 here (or -inf): flush-to-zero is exact enough
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// order-preserving float <-> int map, so that one integer REDUX gives the warp max of floats
+__device__ __forceinline__ int f2ord(float f) {
+  const int b = __float_as_int(f);
+  return b ^ ((b >> 31) & 0x7fffffff);
+}
+__device__ __forceinline__ float ord2f(int o) { return __int_as_float(o ^ ((o >> 31) & 0x7fffffff)); }
+__device__ __forceinline__ float warp_max(float v) { return ord2f(__reduce_max_sync(0xffffffffu, f2ord(v))); }
 
-template <typename T> struct VecTraits;
-template <> struct VecTraits<__nv_bfloat16> {
+// (m, s, idx) (+)= (m2, s2, idx2); lower index wins ties so the result is order-independent.
+__device__ __forceinline__ void combine(Triple& a, const Triple& b) {
+  const bool take2 = (b.m > a.m) || (b.m == a.m && b.idx < a.idx);
+  const float mn = fmaxf(a.m, b.m);
+  const float ms = (mn == -INFINITY) ? 0.f : mn;          // all -inf so far: keep sums at 0
+  a.s = a.s * ex2((a.m - ms) * kLog2e) + b.s * ex2((b.m - ms) * kLog2e);
+  a.m = mn;
+  a.idx = take2 ? b.idx : a.idx;
+}
+
+template <typename T> struct Vec;
+template <> struct Vec<__nv_bfloat16> {
   static constexpr int kElems = 8;
+  // max of the 8 values of one vector, folded into a packed bf16x2 running max
+  __device__ static __forceinline__ void max_into(const int4& v, uint32_t& acc) {
+    const uint32_t w[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) asm("max.bf16x2 %0, %0, %1;" : "+r"(acc) : "r"(w[i]));
+  }
+  static constexpr uint32_t kAccInit = 0xff80ff80u;       // (-inf, -inf)
+  __device__ static __forceinline__ float acc_max(uint32_t acc) {
+    return fmaxf(__uint_as_float(acc << 16), __uint_as_float(acc & 0xffff0000u));
+  }
   __device__ static __forceinline__ void unpack(const int4& v, float (&x)[8]) {
     const uint32_t w[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
 #pragma unroll
@@ -46,26 +89,36 @@ template <> struct VecTraits<__nv_bfloat16> {
       x[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
     }
   }
+  __device__ static __forceinline__ void set_neg_inf(int4& v, int e) {
+    const uint32_t sh = (e & 1) * 16, keep = ~(0xffffu << sh), ninf = 0xff80u << sh;   // static selects:
+    const int w = e >> 1;                                    // no dynamic register indexing
+    v.x = w == 0 ? (int)(((uint32_t)v.x & keep) | ninf) : v.x;
+    v.y = w == 1 ? (int)(((uint32_t)v.y & keep) | ninf) : v.y;
+    v.z = w == 2 ? (int)(((uint32_t)v.z & keep) | ninf) : v.z;
+    v.w = w == 3 ? (int)(((uint32_t)v.w & keep) | ninf) : v.w;
+  }
   __device__ static __forceinline__ float load1(const __nv_bfloat16* p) { return __bfloat162float(*p); }
 };
-template <> struct VecTraits<float> {
+template <> struct Vec<float> {
   static constexpr int kElems = 4;
+  __device__ static __forceinline__ void max_into(const int4& v, uint32_t& acc) {
+    float a = __uint_as_float(acc);
+    a = fmaxf(fmaxf(a, __int_as_float(v.x)), fmaxf(__int_as_float(v.y), fmaxf(__int_as_float(v.z), __int_as_float(v.w))));
+    acc = __float_as_uint(a);
+  }
+  static constexpr uint32_t kAccInit = 0xff800000u;       // -inf
+  __device__ static __forceinline__ float acc_max(uint32_t acc) { return __uint_as_float(acc); }
   __device__ static __forceinline__ void unpack(const int4& v, float (&x)[4]) {
     x[0] = __int_as_float(v.x); x[1] = __int_as_float(v.y);
     x[2] = __int_as_float(v.z); x[3] = __int_as_float(v.w);
   }
+  __device__ static __forceinline__ void set_neg_inf(int4& v, int e) {
+    const int ninf = (int)0xff800000u;
+    v.x = e == 0 ? ninf : v.x; v.y = e == 1 ? ninf : v.y;
+    v.z = e == 2 ? ninf : v.z; v.w = e == 3 ? ninf : v.w;
+  }
   __device__ static __forceinline__ float load1(const float* p) { return *p; }
 };
-
-// (m, s, idx) (+)= (m2, s2, idx2); lower index wins ties so the result is order-independent.
-__device__ __forceinline__ void combine(float& m, float& s, int& idx, float m2, float s2, int idx2) {
-  const bool take2 = (m2 > m) || (m2 == m && idx2 < idx);
-  const float mn = fmaxf(m, m2);
-  const float ms = (mn == -INFINITY) ? 0.f : mn;          // all -inf so far: keep sums at 0
-  s = s * exp2f((m - ms) * kLog2e) + s2 * exp2f((m2 - ms) * kLog2e);
-  m = mn;
-  idx = take2 ? idx2 : idx;
-}
 
 // warp-cooperative: does `row` belong to a refine lane (EOS suppressed)?
 __device__ __forceinline__ bool row_suppresses_eos(const al_lane_desc* lanes, int n_lanes, int row, int lane) {
@@ -77,128 +130,173 @@ __device__ __forceinline__ bool row_suppresses_eos(const al_lane_desc* lanes, in
   return __any_sync(0xffffffffu, sup);
 }
 
-// fold n values x[0..n) whose first element has vocabulary index `base` into (m, s, idx)
-template <int N>
-__device__ __forceinline__ void fold(float (&x)[N], int base, float& m, float& s, int& idx) {
-  float vm = x[0];
-  int vi = 0;
-#pragma unroll
-  for (int i = 1; i < N; ++i)
-    if (x[i] > vm) { vm = x[i]; vi = i; }                 // strict >: first maximiser inside the vector
-  if (vm > m) {                                           // strict >: earlier vectors keep ties
-    s *= exp2f((m - vm) * kLog2e);                        // m = -inf: s is 0 and exp2(-inf) = 0
-    m = vm;
-    idx = base + vi;
+// One element per lane (unaligned rows and the < 16-byte row tail): value x at vocabulary index e,
+// or (-inf, kNoIdx) for idle lanes.  m and idx are warp-uniform, s is per lane.
+__device__ __forceinline__ void fold_scalar(float x, int e, float& m, float& s, int& idx) {
+  const float wm = warp_max(x);
+  if (wm > m) {                                            // strict >: earlier items keep ties
+    s *= ex2((m - wm) * kLog2e);                           // m = -inf: s is 0 and stays 0
+    m = wm;
+    idx = __reduce_min_sync(0xffffffffu, x == wm ? e : kNoIdx);
   }
   const float mb = (m == -INFINITY) ? 0.f : m * kLog2e;
-#pragma unroll
-  for (int i = 0; i < N; ++i) s += exp2f(fmaf(x[i], kLog2e, -mb));
+  s += ex2(fmaf(x, kLog2e, -mb));
 }
+
+template <typename T>
+__device__ __forceinline__ void load_item(int4 (&v)[kWarpVecs], const T* __restrict__ row, int vi0, int v_end,
+                                          int sup) {
+  constexpr int E = Vec<T>::kElems;
+  const int pad = (int)Vec<T>::kAccInit;
+#pragma unroll
+  for (int j = 0; j < kWarpVecs; ++j) {
+    const int vi = vi0 + j * 32;
+    v[j] = vi < v_end ? ld_stream(row + (long long)vi * E) : make_int4(pad, pad, pad, pad);
+  }
+  if (sup >= 0) {                                          // EOS suppression (refine rows only)
+    const int sv = sup / E;
+#pragma unroll
+    for (int j = 0; j < kWarpVecs; ++j)
+      if (vi0 + j * 32 == sv) Vec<T>::set_neg_inf(v[j], sup - sv * E);
+  }
+}
+
+// Fold one 4 KB item held in registers into the warp's running (m, idx) and the lane's sum s.
+template <typename T>
+__device__ __forceinline__ void fold_item(const int4 (&v)[kWarpVecs], int vi0, float& m, float& s, int& idx) {
+  constexpr int E = Vec<T>::kElems;
+  uint32_t acc = Vec<T>::kAccInit;
+#pragma unroll
+  for (int j = 0; j < kWarpVecs; ++j) Vec<T>::max_into(v[j], acc);
+  const float lm = Vec<T>::acc_max(acc);
+  const float wm = warp_max(lm);
+  if (wm > m) {                                            // warp-uniform, rare after the first items
+    s *= ex2((m - wm) * kLog2e);
+    m = wm;
+    int cand = kNoIdx;
+    if (lm == wm) {
+#pragma unroll
+      for (int j = kWarpVecs - 1; j >= 0; --j) {           // descending, so the first maximiser wins
+        float x[E];
+        Vec<T>::unpack(v[j], x);
+#pragma unroll
+        for (int e = E - 1; e >= 0; --e)
+          if (x[e] == wm) cand = (vi0 + j * 32) * E + e;
+      }
+    }
+    idx = __reduce_min_sync(0xffffffffu, cand);
+  }
+  const float mb = (m == -INFINITY) ? 0.f : m * kLog2e;
+  float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+  for (int j = 0; j < kWarpVecs; ++j) {
+    float x[E];
+    Vec<T>::unpack(v[j], x);
+#pragma unroll
+    for (int e = 0; e < E; e += 2) {
+      s0 += ex2(fmaf(x[e], kLog2e, -mb));
+      s1 += ex2(fmaf(x[e + 1], kLog2e, -mb));
+    }
+  }
+  s += s0 + s1;
+}
+
+struct SelectArgs {
+  const int32_t* tokens_in;
+  int mask_id;
+  float threshold;
+  float* conf_out;
+  int32_t* argmax_out;
+  uint8_t* commit_out;
+  int32_t* tokens_out;
+};
 
 template <typename T, bool kVector>
-__global__ void __launch_bounds__(kThreads)
-confidence_partial_kernel(const T* __restrict__ logits, int n_rows, int vocab, long long row_stride,
-                          int items_per_row, int eos_id, const al_lane_desc* __restrict__ lanes,
-                          int n_lanes, Partial* __restrict__ partials) {
-  constexpr int E = VecTraits<T>::kElems;
-  const int lane = threadIdx.x & 31;
-  const long long warp = ((long long)blockIdx.x * kThreads + threadIdx.x) >> 5;
-  const long long n_warps = ((long long)gridDim.x * kThreads) >> 5;
-  const long long n_items = (long long)n_rows * items_per_row;
-  const int vec_total = vocab / E;                         // whole vectors per row (vector path)
-
-  for (long long item = warp; item < n_items; item += n_warps) {
-    const int row = (int)(item / items_per_row);
-    const int chunk = (int)(item - (long long)row * items_per_row);
-    const T* base = logits + (long long)row * row_stride;
-    const int sup = (eos_id >= 0 && lanes && row_suppresses_eos(lanes, n_lanes, row, lane)) ? eos_id : -1;
-    float m = -INFINITY, s = 0.f;
-    int idx = 0x7fffffff;
-
-    if (kVector) {
-      const int v0 = chunk * kItemVecs + lane;
-      int4 v[kWarpVecs];
-#pragma unroll
-      for (int j = 0; j < kWarpVecs; ++j) {
-        const int vi = v0 + j * 32;
-        if (vi < vec_total) v[j] = ld_stream(base + (long long)vi * E);
-      }
-#pragma unroll
-      for (int j = 0; j < kWarpVecs; ++j) {
-        const int vi = v0 + j * 32;
-        if (vi < vec_total) {
-          float x[E];
-          VecTraits<T>::unpack(v[j], x);
-          const int sup_local = sup - vi * E;              // sup = -1 => negative
-          if (sup_local >= 0 && sup_local < E) {
-#pragma unroll
-            for (int i = 0; i < E; ++i) x[i] = (i == sup_local) ? -INFINITY : x[i];
-          }
-          fold<E>(x, vi * E, m, s, idx);
-        }
-      }
-      // scalar tail of the row (vocab % E elements) rides with the last item
-      if (chunk == items_per_row - 1) {
-        const int e = vec_total * E + lane;
-        if (e < vocab) {
-          float x[1] = {e == sup ? -INFINITY : VecTraits<T>::load1(base + e)};
-          fold<1>(x, e, m, s, idx);
-        }
-      }
-    } else {                                               // unaligned rows: element-wise, same items
-      const int e0 = chunk * kItemVecs * E;
-      const int e1 = min(vocab, e0 + kItemVecs * E);
-      for (int e = e0 + lane; e < e1; e += 32) {
-        float x[1] = {e == sup ? -INFINITY : VecTraits<T>::load1(base + e)};
-        fold<1>(x, e, m, s, idx);
-      }
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-      const float m2 = __shfl_xor_sync(0xffffffffu, m, off);
-      const float s2 = __shfl_xor_sync(0xffffffffu, s, off);
-      const int i2 = __shfl_xor_sync(0xffffffffu, idx, off);
-      combine(m, s, idx, m2, s2, i2);
-    }
-    if (lane == 0) partials[item] = Partial{m, s, idx, 0};
-  }
-}
-
-__global__ void __launch_bounds__(kThreads)
-confidence_finalize_kernel(const Partial* __restrict__ partials, int n_rows, int items_per_row,
-                           const int32_t* __restrict__ tokens_in, int mask_id, float threshold,
-                           float* __restrict__ conf_out, int32_t* __restrict__ argmax_out,
-                           uint8_t* __restrict__ commit_out, int32_t* __restrict__ tokens_out) {
-  const int lane = threadIdx.x & 31;
-  const int row = (blockIdx.x * kThreads + threadIdx.x) >> 5;
-  if (row >= n_rows) return;
+__global__ void __launch_bounds__(kThreads, 4)
+confidence_select_kernel(const T* __restrict__ logits, int n_rows, int vocab, long long row_stride, int k_cluster,
+                         int eos_id, const al_lane_desc* __restrict__ lanes, int n_lanes, SelectArgs out) {
+  constexpr int E = Vec<T>::kElems;
+  __shared__ Triple s_warp[kWarps];
+  __shared__ Triple s_cta[kMaxCluster];                    // leader CTA: one slot per cluster rank
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int row = blockIdx.x / k_cluster;
+  const int rank = blockIdx.x - row * k_cluster;
+  const T* base = logits + (long long)row * row_stride;
+  const int sup = (eos_id >= 0 && lanes && row_suppresses_eos(lanes, n_lanes, row, lane)) ? eos_id : -1;
   float m = -INFINITY, s = 0.f;
-  int idx = 0x7fffffff;
-  for (int c = lane; c < items_per_row; c += 32) {
-    const Partial p = partials[(long long)row * items_per_row + c];
-    combine(m, s, idx, p.m, p.s, p.idx);
+  int idx = kNoIdx;
+
+  if (kVector) {
+    const int vec_total = vocab / E;
+    const int vpc = (((vec_total + k_cluster - 1) / k_cluster) + 7) & ~7;   // vectors per chunk, 128-B aligned
+    const int c0 = min(vec_total, rank * vpc), c1 = min(vec_total, c0 + vpc);
+    for (int i0 = c0 + warp * kItemVecs; i0 < c1; i0 += kWarps * kItemVecs) {
+      int4 v[kWarpVecs];
+      load_item<T>(v, base, i0 + lane, c1, sup);
+      fold_item<T>(v, i0 + lane, m, s, idx);
+    }
+    if (rank == k_cluster - 1 && warp == 0 && vec_total * E < vocab) {      // < 16-byte row tail
+      const int e = vec_total * E + lane;
+      const bool ok = e < vocab;
+      fold_scalar(ok ? (e == sup ? -INFINITY : Vec<T>::load1(base + e)) : -INFINITY, ok ? e : kNoIdx, m, s, idx);
+    }
+  } else {                                                 // unaligned rows: one element per lane
+    const int epc = (vocab + k_cluster - 1) / k_cluster;
+    const int c0 = min(vocab, rank * epc), c1 = min(vocab, c0 + epc);
+    for (int e0 = c0 + warp * 32; e0 < c1; e0 += kWarps * 32) {
+      const int e = e0 + lane;
+      const bool ok = e < c1;
+      fold_scalar(ok ? (e == sup ? -INFINITY : Vec<T>::load1(base + e)) : -INFINITY, ok ? e : kNoIdx, m, s, idx);
+    }
   }
+  // lanes share m: the warp's sum is a plain add
 #pragma unroll
-  for (int off = 16; off > 0; off >>= 1) {
-    const float m2 = __shfl_xor_sync(0xffffffffu, m, off);
-    const float s2 = __shfl_xor_sync(0xffffffffu, s, off);
-    const int i2 = __shfl_xor_sync(0xffffffffu, idx, off);
-    combine(m, s, idx, m2, s2, i2);
+  for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if (lane == 0) s_warp[warp] = Triple{m, s, idx};
+  __syncthreads();
+  Triple t{-INFINITY, 0.f, kNoIdx};
+  if (warp == 0) {
+    if (lane < kWarps) t = s_warp[lane];
+#pragma unroll
+    for (int off = kWarps / 2; off > 0; off >>= 1) {
+      Triple o;
+      o.m = __shfl_xor_sync(0xffffffffu, t.m, off);
+      o.s = __shfl_xor_sync(0xffffffffu, t.s, off);
+      o.idx = __shfl_xor_sync(0xffffffffu, t.idx, off);
+      combine(t, o);
+    }
   }
-  if (lane == 0) {
-    const float conf = 1.0f / s;                           // = exp(max - logsumexp)
-    const int tok = tokens_in[row];
-    const bool commit = (tok == mask_id) && (conf >= threshold);
-    conf_out[row] = conf;
-    argmax_out[row] = idx;
-    commit_out[row] = commit ? 1 : 0;
-    tokens_out[row] = commit ? idx : tok;
+  if (k_cluster > 1) {
+    cg::cluster_group cluster = cg::this_cluster();
+    if (threadIdx.x == 0) cluster.map_shared_rank(s_cta, 0)[rank] = t;     // DSMEM store into the leader
+    cluster.sync();
+    if (rank != 0) return;
+    if (warp == 0) {
+      t = lane < k_cluster ? s_cta[lane] : Triple{-INFINITY, 0.f, kNoIdx};
+#pragma unroll
+      for (int off = kMaxCluster / 2; off > 0; off >>= 1) {
+        Triple o;
+        o.m = __shfl_xor_sync(0xffffffffu, t.m, off);
+        o.s = __shfl_xor_sync(0xffffffffu, t.s, off);
+        o.idx = __shfl_xor_sync(0xffffffffu, t.idx, off);
+        combine(t, o);
+      }
+    }
+  }
+  if (threadIdx.x == 0) {
+    const float conf = 1.0f / t.s;                         // = exp(max - logsumexp)
+    const int tok = out.tokens_in[row];
+    const bool commit = (tok == out.mask_id) && (conf >= out.threshold);
+    out.conf_out[row] = conf;
+    out.argmax_out[row] = t.idx;
+    out.commit_out[row] = commit ? 1 : 0;
+    out.tokens_out[row] = commit ? t.idx : tok;
   }
 }
 
 // force-top1 (reading C4): one warp per lane; a lane with masked rows and no commit commits its
-// masked row of largest confidence (lowest row on ties).  tokens_mask[] = commit-independent copy
-// of "row is masked", taken from tokens_out/commit state written by finalize.
+// masked row of largest confidence (lowest row on ties).  After the select kernel a still-masked
+// row has tokens_out == mask_id and commit == 0.
 __global__ void __launch_bounds__(kThreads)
 force_top1_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_rows, int mask_id,
                   const float* __restrict__ conf, const int32_t* __restrict__ argmax,
@@ -210,13 +308,12 @@ force_top1_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_row
   if (lanes) { qs = lanes[l].q_start; ql = lanes[l].q_len; }
   bool any_commit = false;
   float best = -1.f;
-  int best_row = 0x7fffffff;
+  int best_row = kNoIdx;
   for (int i = lane; i < ql; i += 32) {
     const int row = qs + i;
     if (row < 0 || row >= n_rows) continue;
     const bool c = commit[row] != 0;
     any_commit |= c;
-    // after finalize a still-masked row has tokens_out == mask_id and commit == 0
     if (!c && tokens_out[row] == mask_id) {
       const float q = conf[row];
       if (q > best || (q == best && row < best_row)) { best = q; best_row = row; }
@@ -229,22 +326,46 @@ force_top1_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_row
     const int r2 = __shfl_xor_sync(0xffffffffu, best_row, off);
     if (b2 > best || (b2 == best && r2 < best_row)) { best = b2; best_row = r2; }
   }
-  if (lane == 0 && !any_commit && best_row != 0x7fffffff) {
+  if (lane == 0 && !any_commit && best_row != kNoIdx) {
     commit[best_row] = 1;
     tokens_out[best_row] = argmax[best_row];
   }
 }
 
-inline int items_per_row_for(int vocab, int esz) {
-  const int elems_per_item = kItemVecs * (16 / esz);
-  return (vocab + elems_per_item - 1) / elems_per_item;
+// cluster size: the largest k in {1,2,4,8} for which N*k CTAs still fit one resident wave
+// (4 CTAs per SM) and every CTA keeps at least one 4 KB item per warp
+int pick_cluster(int n_rows, int vec_total, int sm_count) {
+  int k = 1;
+  while (k < kMaxCluster && (long long)n_rows * (2 * k) <= 4LL * sm_count &&
+         vec_total / (2 * k) >= kWarps * kItemVecs)
+    k *= 2;
+  return k;
+}
+
+template <typename T, bool kVector>
+cudaError_t launch_select(int k, int n_rows, cudaStream_t cs, const T* logits, int vocab, long long row_stride,
+                          int eos_id, const al_lane_desc* lanes, int n_lanes, const SelectArgs& out) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)(n_rows * k));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = cs;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)k;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, confidence_select_kernel<T, kVector>, logits, n_rows, vocab, row_stride, k, eos_id,
+                            lanes, n_lanes, out);
 }
 
 }  // namespace
 
 extern "C" size_t al_confidence_select_workspace_bytes(int32_t n_rows, int32_t vocab) {
   if (n_rows <= 0 || vocab <= 0) return 0;
-  return (size_t)n_rows * items_per_row_for(vocab, 4) * sizeof(Partial);   // f32 has the most items
+  return (size_t)n_rows * 16;   // reserved (cluster/DSMEM merge needs no HBM partials); kept for ABI stability
 }
 
 extern "C" al_status al_confidence_select(al_handle* h, const void* logits, int32_t dtype, int32_t n_rows,
@@ -265,38 +386,33 @@ extern "C" al_status al_confidence_select(al_handle* h, const void* logits, int3
     AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: NULL pointer");
   if (n_lanes > 0 && !lanes) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: n_lanes > 0 but lanes is NULL");
   if (eos_id >= vocab) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: eos_id %d >= vocab %d", eos_id, vocab);
-  const int esz = al_esize(dtype);
-  const int ipr = items_per_row_for(vocab, esz);
-  const size_t need = (size_t)n_rows * ipr * sizeof(Partial);
+  const size_t need = al_confidence_select_workspace_bytes(n_rows, vocab);
   if (!workspace || workspace_bytes < need || !al_aligned16(workspace))
     AL_FAIL(AL_ERR_WORKSPACE, "al_confidence_select: workspace %zu < %zu (or unaligned)", workspace_bytes, need);
+  if ((long long)n_rows * kMaxCluster > 0x7fffffffLL) AL_FAIL(AL_ERR_UNSUPPORTED, "al_confidence_select: too many rows");
+  const int esz = al_esize(dtype);
   const bool vec = al_aligned16(logits) && ((row_stride * esz) % 16 == 0);
   cudaStream_t cs = static_cast<cudaStream_t>(stream);
-  Partial* parts = static_cast<Partial*>(workspace);
   const al_lane_desc* lanes_eff = n_lanes > 0 ? lanes : nullptr;
+  const SelectArgs out{tokens_in, mask_id, threshold, conf_out, argmax_out, commit_out, tokens_out};
+  const int k = vec ? pick_cluster(n_rows, vocab / (16 / esz), h->sm_count) : pick_cluster(n_rows, vocab / 8, h->sm_count);
 
-  const long long n_items = (long long)n_rows * ipr;
-  const int warps_per_block = kThreads / 32;
-  long long blocks = (n_items + warps_per_block - 1) / warps_per_block;
-  const long long cap = (long long)h->sm_count * 8;        // 8 x 256 threads = 64 warps per SM
-  if (blocks > cap) blocks = cap;
-#define AL_LAUNCH_PARTIAL(T, V)                                                                     \
-  confidence_partial_kernel<T, V><<<(unsigned)blocks, kThreads, 0, cs>>>(                           \
-      static_cast<const T*>(logits), n_rows, vocab, (long long)row_stride, ipr, eos_id, lanes_eff,  \
-      n_lanes, parts)
-  if (dtype == AL_BF16) { if (vec) AL_LAUNCH_PARTIAL(__nv_bfloat16, true); else AL_LAUNCH_PARTIAL(__nv_bfloat16, false); }
-  else                  { if (vec) AL_LAUNCH_PARTIAL(float, true);         else AL_LAUNCH_PARTIAL(float, false); }
-#undef AL_LAUNCH_PARTIAL
-  AL_CUDA_OK(cudaGetLastError());
-  h->launches += 2;
-  const int fin_blocks = (n_rows + warps_per_block - 1) / warps_per_block;
-  confidence_finalize_kernel<<<fin_blocks, kThreads, 0, cs>>>(parts, n_rows, ipr, tokens_in, mask_id, threshold,
-                                                               conf_out, argmax_out, commit_out, tokens_out);
-  AL_CUDA_OK(cudaGetLastError());
+  cudaError_t e;
+  if (dtype == AL_BF16) {
+    const __nv_bfloat16* p = static_cast<const __nv_bfloat16*>(logits);
+    e = vec ? launch_select<__nv_bfloat16, true>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out)
+            : launch_select<__nv_bfloat16, false>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out);
+  } else {
+    const float* p = static_cast<const float*>(logits);
+    e = vec ? launch_select<float, true>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out)
+            : launch_select<float, false>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out);
+  }
+  if (e != cudaSuccess) AL_FAIL(AL_ERR_CUDA, "al_confidence_select: launch failed: %s", cudaGetErrorString(e));
+  h->launches++;
   if (flags & AL_SELECT_FORCE_TOP1) {
     const int nl = lanes_eff ? n_lanes : 1;
-    force_top1_kernel<<<(nl + warps_per_block - 1) / warps_per_block, kThreads, 0, cs>>>(
-        lanes_eff, nl, n_rows, mask_id, conf_out, argmax_out, commit_out, tokens_out);
+    force_top1_kernel<<<(nl + kWarps - 1) / kWarps, kThreads, 0, cs>>>(lanes_eff, nl, n_rows, mask_id, conf_out,
+                                                                      argmax_out, commit_out, tokens_out);
     AL_CUDA_OK(cudaGetLastError());
     h->launches++;
   }
