@@ -41,4 +41,5 @@ def test_lane_desc_and_shape_struct_layouts():
 def test_workspace_queries_need_no_gpu():
     lib = binding.load_library()
     assert lib.al_confidence_select_workspace_bytes(0, 100) == 0
-    assert lib.al_confidence_select_workspace_bytes(4, 126464) >= 4 * 62 * 16
+    # the cluster/DSMEM merge keeps no partials in HBM: the workspace is a small reserved slot per row
+    assert 0 < lib.al_confidence_select_workspace_bytes(4, 126464) <= 4 * 64
