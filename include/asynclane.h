@@ -107,6 +107,8 @@ int32_t al_sm_count(const al_handle* handle);
  * Lanes of one group that are adjacent in the array and contiguous in q_start are stacked into
  * common 128-row tensor-core tiles.
  * Rows of Q not covered by any lane are not written in `out`.
+ * Cache rows of a group up to its largest prefix_len rounded up to 16 must hold finite values
+ * (they are multiplied by exact zeros where a lane may not see them).
  */
 size_t al_lane_attention_workspace_bytes(const al_attn_shape* shape, int32_t n_lanes,
                                          int32_t total_q_rows, int32_t max_prefix_len);
@@ -116,6 +118,28 @@ al_status al_lane_attention(al_handle* handle, const al_attn_shape* shape, const
                             int32_t total_q_rows, int32_t max_prefix_len, void* out,
                             float* lse_or_null, void* workspace, size_t workspace_bytes,
                             void* cuda_stream);
+
+/*
+ * The work decomposition of al_lane_attention (tiles, key ranges, per-CTA work lists) depends only
+ * on the lane descriptors, not on the layer: one scheduler iteration (P:L135 UPDATELANES) calls the
+ * model once per group (Eq.11) and every layer of that call sees the same lanes.
+ *   al_lane_plan               builds the decomposition from lanes_dev into `workspace` (one small launch)
+ *   al_lane_attention_planned  runs the attention of one layer from a workspace al_lane_plan filled
+ *                              with the SAME shape, lanes_dev contents, n_lanes and total_q_rows
+ * al_lane_attention == al_lane_plan followed by al_lane_attention_planned.  The planned call leaves
+ * the plan intact, so it may be repeated (other layers, other q/k/v/cache/out pointers) on the same
+ * stream.  For shapes the tensor-core path does not cover (fp32, head_dim != 128) there is no plan:
+ * al_lane_plan is a no-op and al_lane_attention_planned runs the plain-ALU kernel.
+ */
+al_status al_lane_plan(al_handle* handle, const al_attn_shape* shape, const al_lane_desc* lanes_dev,
+                       int32_t n_lanes, int32_t total_q_rows, int32_t max_prefix_len, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream);
+al_status al_lane_attention_planned(al_handle* handle, const al_attn_shape* shape, const void* q,
+                                    const void* k_new, const void* v_new, const void* k_cache,
+                                    const void* v_cache, const al_lane_desc* lanes_dev,
+                                    int32_t n_lanes, int32_t total_q_rows, int32_t max_prefix_len,
+                                    void* out, float* lse_or_null, void* workspace,
+                                    size_t workspace_bytes, void* cuda_stream);
 
 /* ---- (b) compact cache refresh ---------------------------------------------------------------- */
 

@@ -82,37 +82,75 @@ extern "C" size_t al_lane_attention_workspace_bytes(const al_attn_shape* s, int3
   return al_attention_umma_workspace_bytes(nullptr, s, n_lanes, total_q_rows, max_prefix_len);
 }
 
+// mode bit 0: build the plan; bit 1: run the attention
+static al_status lane_attention_impl(int mode, const char* who, al_handle* h, const al_attn_shape* s, const void* q,
+                                     const void* k_new, const void* v_new, const void* k_cache,
+                                     const void* v_cache, const al_lane_desc* lanes, int32_t n_lanes,
+                                     int32_t total_q_rows, int32_t max_prefix_len, void* out, float* lse,
+                                     void* workspace, size_t workspace_bytes, void* stream) {
+  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "%s: handle is NULL", who);
+  al_status st = check_shape(s, who);
+  if (st != AL_OK) return st;
+  if (n_lanes < 0 || total_q_rows < 0 || max_prefix_len < 0) AL_FAIL(AL_ERR_INVALID_ARG, "%s: negative size", who);
+  if (n_lanes == 0 || total_q_rows == 0) return AL_OK;
+  if (!lanes) AL_FAIL(AL_ERR_INVALID_ARG, "%s: lanes is NULL", who);
+  if (max_prefix_len > s->cache_rows) AL_FAIL(AL_ERR_INVALID_ARG, "%s: max_prefix_len > cache_rows", who);
+  if (s->head_dim > 256 || s->head_dim % 8 != 0)
+    AL_FAIL(AL_ERR_UNSUPPORTED, "%s: head_dim %d (need multiple of 8, <= 256)", who, s->head_dim);
+  if (!al_aligned16(workspace)) AL_FAIL(AL_ERR_INVALID_ARG, "%s: workspace must be 16-byte aligned", who);
+  if (mode & 2) {
+    if (!q || !k_new || !v_new || !out) AL_FAIL(AL_ERR_INVALID_ARG, "%s: NULL pointer", who);
+    if (max_prefix_len > 0 && (!k_cache || !v_cache)) AL_FAIL(AL_ERR_INVALID_ARG, "%s: NULL cache", who);
+    if (!al_aligned16(q) || !al_aligned16(k_new) || !al_aligned16(v_new) || !al_aligned16(k_cache) ||
+        !al_aligned16(v_cache) || !al_aligned16(out))
+      AL_FAIL(AL_ERR_INVALID_ARG, "%s: pointers must be 16-byte aligned", who);
+  }
+  const float scale = s->scale > 0.f ? s->scale : 1.0f / sqrtf((float)s->head_dim);
+  cudaStream_t cs = static_cast<cudaStream_t>(stream);
+  if (al_attention_umma_supported(s)) {
+    const size_t need = al_attention_umma_workspace_bytes(h, s, n_lanes, total_q_rows, max_prefix_len);
+    if (workspace_bytes < need || (need && !workspace))
+      AL_FAIL(AL_ERR_WORKSPACE, "%s: workspace %zu < %zu", who, workspace_bytes, need);
+    if (mode & 1) {
+      st = al_launch_plan_umma(h, s, lanes, n_lanes, total_q_rows, workspace, workspace_bytes, cs);
+      if (st != AL_OK) return st;
+    }
+    if (mode & 2)
+      return al_launch_attention_umma(h, s, scale, q, k_new, v_new, k_cache, v_cache, lanes, n_lanes,
+                                      total_q_rows, max_prefix_len, out, lse, workspace, workspace_bytes, cs);
+    return AL_OK;
+  }
+  if (mode & 2)
+    return al_launch_attention_simt(h, s, scale, q, k_new, v_new, k_cache, v_cache, lanes, n_lanes,
+                                    total_q_rows, out, lse, cs);
+  return AL_OK;
+}
+
 extern "C" al_status al_lane_attention(al_handle* h, const al_attn_shape* s, const void* q,
                                        const void* k_new, const void* v_new, const void* k_cache,
                                        const void* v_cache, const al_lane_desc* lanes, int32_t n_lanes,
                                        int32_t total_q_rows, int32_t max_prefix_len, void* out,
                                        float* lse, void* workspace, size_t workspace_bytes,
                                        void* stream) {
-  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "al_lane_attention: handle is NULL");
-  al_status st = check_shape(s, "al_lane_attention");
-  if (st != AL_OK) return st;
-  if (n_lanes < 0 || total_q_rows < 0 || max_prefix_len < 0)
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_lane_attention: negative size");
-  if (n_lanes == 0 || total_q_rows == 0) return AL_OK;
-  if (!q || !k_new || !v_new || !out || !lanes) AL_FAIL(AL_ERR_INVALID_ARG, "al_lane_attention: NULL pointer");
-  if (max_prefix_len > 0 && (!k_cache || !v_cache)) AL_FAIL(AL_ERR_INVALID_ARG, "al_lane_attention: NULL cache");
-  if (max_prefix_len > s->cache_rows) AL_FAIL(AL_ERR_INVALID_ARG, "al_lane_attention: max_prefix_len > cache_rows");
-  if (!al_aligned16(q) || !al_aligned16(k_new) || !al_aligned16(v_new) || !al_aligned16(k_cache) ||
-      !al_aligned16(v_cache) || !al_aligned16(out) || !al_aligned16(workspace))
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_lane_attention: pointers must be 16-byte aligned");
-  if (s->head_dim > 256 || s->head_dim % 8 != 0)
-    AL_FAIL(AL_ERR_UNSUPPORTED, "al_lane_attention: head_dim %d (need multiple of 8, <= 256)", s->head_dim);
-  const float scale = s->scale > 0.f ? s->scale : 1.0f / sqrtf((float)s->head_dim);
-  cudaStream_t cs = static_cast<cudaStream_t>(stream);
-  if (al_attention_umma_supported(s)) {
-    const size_t need = al_attention_umma_workspace_bytes(h, s, n_lanes, total_q_rows, max_prefix_len);
-    if (workspace_bytes < need || (need && !workspace))
-      AL_FAIL(AL_ERR_WORKSPACE, "al_lane_attention: workspace %zu < %zu", workspace_bytes, need);
-    return al_launch_attention_umma(h, s, scale, q, k_new, v_new, k_cache, v_cache, lanes, n_lanes,
-                                    total_q_rows, max_prefix_len, out, lse, workspace, workspace_bytes, cs);
-  }
-  return al_launch_attention_simt(h, s, scale, q, k_new, v_new, k_cache, v_cache, lanes, n_lanes,
-                                  total_q_rows, out, lse, cs);
+  return lane_attention_impl(3, "al_lane_attention", h, s, q, k_new, v_new, k_cache, v_cache, lanes, n_lanes,
+                             total_q_rows, max_prefix_len, out, lse, workspace, workspace_bytes, stream);
+}
+
+extern "C" al_status al_lane_plan(al_handle* h, const al_attn_shape* s, const al_lane_desc* lanes,
+                                  int32_t n_lanes, int32_t total_q_rows, int32_t max_prefix_len,
+                                  void* workspace, size_t workspace_bytes, void* stream) {
+  return lane_attention_impl(1, "al_lane_plan", h, s, nullptr, nullptr, nullptr, nullptr, nullptr, lanes, n_lanes,
+                             total_q_rows, max_prefix_len, nullptr, nullptr, workspace, workspace_bytes, stream);
+}
+
+extern "C" al_status al_lane_attention_planned(al_handle* h, const al_attn_shape* s, const void* q,
+                                               const void* k_new, const void* v_new, const void* k_cache,
+                                               const void* v_cache, const al_lane_desc* lanes,
+                                               int32_t n_lanes, int32_t total_q_rows, int32_t max_prefix_len,
+                                               void* out, float* lse, void* workspace,
+                                               size_t workspace_bytes, void* stream) {
+  return lane_attention_impl(2, "al_lane_attention_planned", h, s, q, k_new, v_new, k_cache, v_cache, lanes,
+                             n_lanes, total_q_rows, max_prefix_len, out, lse, workspace, workspace_bytes, stream);
 }
 
 extern "C" al_status al_validate_lanes(al_handle* h, const al_attn_shape* s, const al_lane_desc* lanes,

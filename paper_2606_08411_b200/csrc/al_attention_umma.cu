@@ -3,25 +3,36 @@
 // own rows; L168-172 Eq.11: lanes of one shared-prefix group are evaluated in one batched call).
 //
 // Work decomposition (built ON DEVICE from the lane descriptors by lane_plan_kernel, so the call is
-// graph-replayable with new lanes):
+// graph-replayable with new lanes; the plan depends only on the descriptors and is reused by every
+// layer of one scheduler iteration, see al_lane_plan):
 //   run    = maximal sequence of lanes adjacent in the array, of one group, contiguous in q_start
 //   tile   = up to tpt = floor(128 / n_rep) consecutive tokens of a run; with the n_rep q-heads of a
 //            kv-head stacked under every token it is a 128-row M tile of the tensor core
 //   keys   = [prefix key tiles of 128 cache rows] ++ [local key tiles of 128 K_new rows covering the
 //            lanes that intersect the tile]; every row masks what its own lane may not see
-//   work   = (tile, kv-head, contiguous range of key tiles); a tile whose key range is split over
-//            several CTAs (to fill the SMs when heads x tiles are few) leaves fp32 partials + LSE in
-//            the workspace and lane_combine_kernel merges them.
+//   item   = (tile, kv-head): n_key_tiles iterations of the main loop
+// The iterations of all items, flattened item-major, form one sequence of K key-tile steps that is
+// cut into n_ctas contiguous, equal ranges ("stream-K"): every CTA gets the same number of steps
+// (+-1) whatever the lane structure is.  A range boundary that falls within one step of an item
+// boundary snaps to it.  An item whose steps are spread over several CTAs leaves one normalised
+// fp32 partial + LSE per CTA in the workspace; the CTA that finishes last (a ticket counter per
+// item) merges them -- no combine launch.
 // All CTAs that share (group, kv-head) read the same K/V tiles: HBM sees them once, L2 serves the
 // rest -- "the prefix is read once per lane group" (BASELINE north_star).
 //
-// Main kernel, persistent, 192 threads, warp-specialised:
-//   warp 0     TMA producer: Q tile once per work item, K and V tiles through a 3-stage ring
-//   warp 1     MMA issuer (one elected lane): S = Q.K^T (SS form) into a double-buffered TMEM tile,
-//              O += P.V with P read from TMEM (TS form) and V MN-major in shared memory
-//   warps 2-5  online softmax, one thread per row: tcgen05.ld S, mask, running max with lazy
-//              rescaling of O (only when the max grows by more than 2^8), exp2, bf16 P back into
-//              the TMEM columns of S, row sums in fp32; then the epilogue (normalise, store)
+// Main kernel, persistent, 384 threads, warp-specialised, one CTA per SM:
+//   warp 0      TMA producer: Q tile once per piece, K and V tiles through a 3-stage ring
+//   warp 1      MMA issuer (one elected lane): S = Q.K^T (SS form) into TMEM buffer S[i&1];
+//               O[i&1] += P.V with P read from TMEM (TS form) and V MN-major in shared memory
+//   warps 4-7   softmax of the EVEN key tiles of the piece, one thread per stacked row
+//   warps 8-11  softmax of the ODD key tiles
+//               each group keeps its own running max / row sum and its own O accumulator in TMEM
+//               (two interleaved split-KV streams sharing Q, K and V), so the exponentials of one
+//               key tile overlap the MMAs of the next; O is rescaled lazily (only when the max
+//               grows by more than 2^8) and only then does a group wait for its previous P.V.
+//               Epilogue: the two streams are merged through 2 KB of shared memory, normalised and
+//               stored (bf16 output, or fp32 partial for a split item).
+// TMEM: S0 | S1 | O_even | O_odd, 128 fp32 columns each (P aliases S as packed bf16).
 #include <cuda_bf16.h>
 
 #include "al_internal.h"
@@ -37,148 +48,191 @@ constexpr int kD = 128;                    // head_dim
 constexpr int kStages = 3;                 // K/V ring depth
 constexpr int kHalfBytes = 128 * 64 * 2;   // [128 rows][64 bf16] = one 128-byte-swizzled half tile
 constexpr int kTileBytes = 2 * kHalfBytes;
-constexpr int kThreads = 192;
+constexpr int kThreads = 384;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: P <= 2^8 between rescales
-constexpr int kMaxPlanLanes = 2048;
+constexpr int kMaxPlanLanes = 1024;
+constexpr int kMaxPlanTiles = 2048;
+constexpr int kPlanThreads = 1024;
+constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
+constexpr int kMinPiece = 2;               // do not cut the work finer than 2 key-tile steps per CTA
 
-struct __align__(16) TileRec {
-  int q_tok0, n_tok;         // first packed token row, tokens in the tile
-  int kv_base_row;           // cache row of prefix key 0
-  int kv_len_max, kv_len_min;// largest / smallest prefix_len among the lanes of the tile
-  int lk0, lk1;              // local keys: packed rows [lk0, lk1) of K_new / V_new
+struct __align__(16) TileRec {             // 64 bytes
+  int q_tok0, n_tok;          // first packed token row, tokens in the tile
+  int kv_base_row;            // cache row of prefix key 0
+  int kv_len_max, kv_len_min; // largest / smallest prefix_len among the lanes of the tile
+  int lk0, lk1;               // local keys: packed rows [lk0, lk1) of K_new / V_new
   int lane_first, lane_count;
   int n_pref_tiles, n_key_tiles;
-  int n_splits, work_base, part_base;   // part_base: first partial slot (-1 when not split)
-  int pad0, pad1;
+  int kt_off;                 // index of step (g = 0, kt = 0) of this tile in the flattened sequence
+  int pad[4];
 };
-struct __align__(16) WorkRec {
-  int tile, g, kt_begin, kt_end;
-  int part_slot, split, pad0, pad1;
+struct __align__(16) CtaRec {
+  int f_begin, f_end;         // this CTA's range of the flattened step sequence
+  int tile0;                  // tile that contains f_begin
+  int pad;
 };
 struct PlanHeader {
-  int n_tiles, n_work, n_part, chunk;
+  int n_tiles, n_items, k_total, n_ctas;
 };
 
 struct Plan {
   PlanHeader* hdr;
   TileRec* tiles;
-  WorkRec* work;
-  float* part_o;     // [n_part][128][128]
-  float* part_lse;   // [n_part][128]
+  CtaRec* ctas;
+  int* bounds;       // [n_ctas + 1]
+  int* counters;     // [n_items] tickets, zero between calls (the merging CTA resets its item's)
+  float* part_o;     // [2 * grid][128][128]  slot 2c: CTA c's first piece, 2c+1: its last piece
+  float* part_lse;   // [2 * grid][128]
 };
 
 struct Bounds {
-  int max_tiles, max_work, max_part;
+  int max_tiles, grid;
 };
 
 __host__ __device__ inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 // ---------------------------------------------------------------------------------------------
-// plan: lanes -> tiles -> work items.  One CTA; sizes are tiny (lanes <= 2048, tiles <= a few 100).
+// plan: lanes -> runs -> tiles -> flattened steps -> per-CTA ranges.  One CTA, every stage parallel.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_heads, int tpt, int n_sms,
-                 Bounds bounds, Plan plan) {
-  __shared__ int s_run_of_lane_start[kMaxPlanLanes];   // 1 if lane i starts a run
-  __shared__ int s_run_tile_base[kMaxPlanLanes + 1];   // per run: first tile
-  __shared__ int s_run_lane0[kMaxPlanLanes + 1];       // per run: first lane (sentinel n_lanes at the end)
-  __shared__ int s_n_runs, s_n_tiles, s_total_kt, s_chunk, s_n_work, s_n_part;
+// In-place exclusive scan of a[0, n) by the whole block; returns the total.
+__device__ int block_exclusive_scan(int* a, int n, int* s_warp) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  int carry = 0;
+  for (int base = 0; base < n; base += blockDim.x) {
+    const int i = base + threadIdx.x;
+    const int v = i < n ? a[i] : 0;
+    int x = v;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, x, off);
+      if (lane >= off) x += y;
+    }
+    if (lane == 31) s_warp[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+      int w = lane < n_warps ? s_warp[lane] : 0;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, w, off);
+        if (lane >= off) w += y;
+      }
+      s_warp[lane] = w;
+    }
+    __syncthreads();
+    const int incl = x + (warp ? s_warp[warp - 1] : 0);
+    const int total = s_warp[n_warps - 1];
+    if (i < n) a[i] = carry + incl - v;
+    __syncthreads();
+    carry += total;
+  }
+  return carry;
+}
+// largest i in [0, n) with a[i] <= x   (a ascending, a[0] <= x)
+__device__ __forceinline__ int last_le(const int* a, int n, int x) {
+  int lo = 0, hi = n - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (a[mid] <= x) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+
+__global__ void __launch_bounds__(kPlanThreads)
+lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_heads, int tpt, Bounds bounds,
+                 Plan plan) {
+  __shared__ int s_qs[kMaxPlanLanes], s_qe[kMaxPlanLanes], s_pl[kMaxPlanLanes];
+  __shared__ int s_run_lane0[kMaxPlanLanes + 1];
+  __shared__ int s_a[kMaxPlanTiles + 1];       // scan scratch: run flags, tiles per run, steps per tile
+  __shared__ int s_run_tile_base[kMaxPlanLanes + 1];
+  __shared__ int s_bounds[kMaxCtas + 1];
+  __shared__ int s_warp[32];
   const int tid = threadIdx.x;
 
+  // runs
   for (int i = tid; i < n_lanes; i += blockDim.x) {
+    const al_lane_desc b = lanes[i];
+    s_qs[i] = b.q_start; s_qe[i] = b.q_start + b.q_len; s_pl[i] = b.prefix_len;
     int start = 1;
     if (i > 0) {
-      const al_lane_desc a = lanes[i - 1], b = lanes[i];
+      const al_lane_desc a = lanes[i - 1];
       start = !(a.group_id == b.group_id && a.kv_base_row == b.kv_base_row && a.q_start + a.q_len == b.q_start);
     }
-    s_run_of_lane_start[i] = start;
+    s_a[i] = start;
   }
   __syncthreads();
-  if (tid == 0) {
-    int n_runs = 0, n_tiles = 0;
-    for (int i = 0; i < n_lanes; ++i)
-      if (s_run_of_lane_start[i]) s_run_lane0[n_runs++] = i;
-    s_run_lane0[n_runs] = n_lanes;
-    for (int r = 0; r < n_runs; ++r) {
-      const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
-      const int tok0 = lanes[l0].q_start, tok1 = lanes[l1 - 1].q_start + lanes[l1 - 1].q_len;
-      s_run_tile_base[r] = n_tiles;
-      n_tiles += ceil_div(tok1 - tok0, tpt);
-    }
-    s_run_tile_base[n_runs] = n_tiles;
-    s_n_runs = n_runs;
-    s_n_tiles = min(n_tiles, bounds.max_tiles);
-    s_total_kt = 0;
+  const int n_runs = block_exclusive_scan(s_a, n_lanes, s_warp);
+  for (int i = tid; i < n_lanes; i += blockDim.x) {
+    const bool start = (i + 1 < n_lanes ? s_a[i + 1] : n_runs) != s_a[i];
+    if (start) s_run_lane0[s_a[i]] = i;
   }
+  if (tid == 0) s_run_lane0[n_runs] = n_lanes;
   __syncthreads();
-  const int n_runs = s_n_runs, n_tiles = s_n_tiles;
-
-  // tiles (one thread each)
-  for (int t = tid; t < n_tiles; t += blockDim.x) {
-    int r = 0;
-    while (s_run_tile_base[r + 1] <= t) ++r;
+  // tiles per run
+  for (int r = tid; r < n_runs; r += blockDim.x) {
     const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
-    const int run_tok0 = lanes[l0].q_start, run_tok1 = lanes[l1 - 1].q_start + lanes[l1 - 1].q_len;
+    s_run_tile_base[r] = ceil_div(max(0, s_qe[l1 - 1] - s_qs[l0]), tpt);
+  }
+  __syncthreads();
+  int n_tiles = block_exclusive_scan(s_run_tile_base, n_runs, s_warp);
+  n_tiles = min(n_tiles, min(bounds.max_tiles, kMaxPlanTiles));   // cannot bind when the lanes are disjoint
+  // tiles
+  for (int t = tid; t < n_tiles; t += blockDim.x) {
+    const int r = last_le(s_run_tile_base, n_runs, t);
+    const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
     TileRec T;
-    T.q_tok0 = run_tok0 + (t - s_run_tile_base[r]) * tpt;
-    T.n_tok = min(tpt, run_tok1 - T.q_tok0);
+    T.q_tok0 = s_qs[l0] + (t - s_run_tile_base[r]) * tpt;
+    T.n_tok = min(tpt, s_qe[l1 - 1] - T.q_tok0);
     T.kv_base_row = lanes[l0].kv_base_row;
-    T.kv_len_max = 0; T.kv_len_min = 0x7fffffff; T.lk0 = 0x7fffffff; T.lk1 = 0; T.lane_first = -1; T.lane_count = 0;
-    for (int l = l0; l < l1; ++l) {
-      const al_lane_desc L = lanes[l];
-      if (L.q_start < T.q_tok0 + T.n_tok && L.q_start + L.q_len > T.q_tok0) {
-        if (T.lane_first < 0) T.lane_first = l;
-        T.lane_count = l - T.lane_first + 1;
-        T.kv_len_max = max(T.kv_len_max, L.prefix_len);
-        T.kv_len_min = min(T.kv_len_min, L.prefix_len);
-        T.lk0 = min(T.lk0, L.q_start);
-        T.lk1 = max(T.lk1, L.q_start + L.q_len);
-      }
+    T.kv_len_max = 0; T.kv_len_min = 0x7fffffff; T.lk0 = 0x7fffffff; T.lk1 = 0;
+    const int lf = l0 + last_le(s_qs + l0, l1 - l0, T.q_tok0);    // lane that holds the tile's first token
+    int l = lf;
+    for (; l < l1 && s_qs[l] < T.q_tok0 + T.n_tok; ++l) {
+      T.kv_len_max = max(T.kv_len_max, s_pl[l]);
+      T.kv_len_min = min(T.kv_len_min, s_pl[l]);
+      T.lk0 = min(T.lk0, s_qs[l]);
+      T.lk1 = max(T.lk1, s_qe[l]);
     }
+    T.lane_first = lf; T.lane_count = l - lf;
     T.n_pref_tiles = ceil_div(T.kv_len_max, kBN);
     T.n_key_tiles = T.n_pref_tiles + ceil_div(T.lk1 - T.lk0, kBN);
-    T.n_splits = 1; T.work_base = 0; T.part_base = -1; T.pad0 = T.pad1 = 0;
+    T.kt_off = 0; T.pad[0] = T.pad[1] = T.pad[2] = T.pad[3] = 0;
     plan.tiles[t] = T;
-    atomicAdd(&s_total_kt, T.n_key_tiles);
+    s_a[t] = T.n_key_tiles * n_kv_heads;
   }
   __syncthreads();
-  // split policy: chunk = key tiles per work item so that the busiest SM gets ceil(total / SMs)
+  const int k_total = block_exclusive_scan(s_a, n_tiles, s_warp);
+  if (tid == 0) s_a[n_tiles] = k_total;
+  for (int t = tid; t < n_tiles; t += blockDim.x) plan.tiles[t].kt_off = s_a[t];
+  // per-CTA ranges of the flattened step sequence
+  const int n_ctas = max(1, min(min(bounds.grid, kMaxCtas), ceil_div(k_total, kMinPiece)));
+  const bool snap = k_total / n_ctas >= 4;
+  __syncthreads();
+  for (int c = tid; c <= n_ctas; c += blockDim.x) {
+    int f = (int)((long long)c * k_total / n_ctas);
+    if (snap && c > 0 && c < n_ctas) {
+      const int t = last_le(s_a, n_tiles, f);
+      const int nk = (s_a[t + 1] - s_a[t]) / n_kv_heads;
+      const int rem = (f - s_a[t]) % nk;           // steps into the item
+      if (rem <= 1) f -= rem; else if (nk - rem <= 1) f += nk - rem;
+    }
+    s_bounds[c] = f;
+  }
+  __syncthreads();
+  for (int c = tid; c <= n_ctas; c += blockDim.x) {
+    plan.bounds[c] = s_bounds[c];
+    if (c < n_ctas) {
+      CtaRec C;
+      C.f_begin = s_bounds[c]; C.f_end = s_bounds[c + 1];
+      C.tile0 = n_tiles ? last_le(s_a, n_tiles, C.f_begin) : 0;
+      C.pad = 0;
+      plan.ctas[c] = C;
+    }
+  }
+  for (int i = tid; i < n_tiles * n_kv_heads; i += blockDim.x) plan.counters[i] = 0;
   if (tid == 0) {
-    const long long total = (long long)s_total_kt * n_kv_heads;
-    int chunk = (int)((total + n_sms - 1) / n_sms);
-    if (chunk < 1) chunk = 1;
-    int n_work = 0, n_part = 0;
-    for (int t = 0; t < n_tiles; ++t) {
-      TileRec& T = plan.tiles[t];
-      int ns = ceil_div(T.n_key_tiles, chunk);
-      if (ns > 1 && n_part + ns * n_kv_heads > bounds.max_part) ns = 1;       // never outgrow the workspace
-      T.n_splits = ns;
-      T.work_base = n_work;
-      T.part_base = ns > 1 ? n_part : -1;
-      n_work += ns * n_kv_heads;
-      if (ns > 1) n_part += ns * n_kv_heads;
-    }
-    s_chunk = chunk; s_n_work = n_work; s_n_part = n_part;
-    plan.hdr->n_tiles = n_tiles; plan.hdr->n_work = n_work; plan.hdr->n_part = n_part; plan.hdr->chunk = chunk;
-  }
-  __syncthreads();
-  __threadfence_block();
-  // work items (one thread each): index = work_base + g * n_splits + split
-  for (int t = 0; t < n_tiles; ++t) {
-    const TileRec T = plan.tiles[t];
-    const int n = T.n_splits * n_kv_heads;
-    for (int j = tid; j < n; j += blockDim.x) {
-      const int g = j / T.n_splits, sp = j - g * T.n_splits;
-      WorkRec W;
-      W.tile = t; W.g = g;
-      // even partition of the key tiles over the splits
-      W.kt_begin = (int)((long long)T.n_key_tiles * sp / T.n_splits);
-      W.kt_end = (int)((long long)T.n_key_tiles * (sp + 1) / T.n_splits);
-      W.part_slot = T.part_base < 0 ? -1 : T.part_base + j;
-      W.split = sp; W.pad0 = W.pad1 = 0;
-      plan.work[T.work_base + j] = W;
-    }
+    plan.hdr->n_tiles = n_tiles; plan.hdr->n_items = n_tiles * n_kv_heads;
+    plan.hdr->k_total = k_total; plan.hdr->n_ctas = k_total > 0 ? n_ctas : 0;
   }
 }
 
@@ -189,11 +243,13 @@ struct AttnSmem {
   alignas(1024) uint8_t q[2][kHalfBytes];
   alignas(1024) uint8_t k[kStages][2][kHalfBytes];
   alignas(1024) uint8_t v[kStages][2][kHalfBytes];
+  float2 ml[2][kBM];                       // (running max, row sum) of the two softmax streams
   uint64_t q_full, q_empty;
   uint64_t k_full[kStages], v_full[kStages], kv_empty[kStages];
-  uint64_t s_full[2], p_full[2];
-  uint64_t pv_done, o_empty;
+  uint64_t s_full[2], p_full[2], pv_done[2];
+  uint64_t o_empty;
   uint32_t tmem_base;
+  int ticket[3];
 };
 
 struct AttnParams {
@@ -206,26 +262,116 @@ struct AttnParams {
   float scale_log2;
 };
 
+// One CTA's walk over its range of the flattened step sequence: pieces (tile, g, [kt_begin, kt_end)).
+struct PieceWalk {
+  const Plan& plan;
+  int n_kv;
+  int f, f_end, t, g, kt;
+  TileRec T;
+  int kt_begin, kt_end;                    // the current piece
+  __device__ PieceWalk(const Plan& p, int n_kv_heads, int cta, bool active) : plan(p), n_kv(n_kv_heads) {
+    f = f_end = t = g = kt = 0;
+    if (active) {                          // records beyond hdr->n_ctas are not written by the plan
+      const CtaRec C = p.ctas[cta];
+      f = C.f_begin; f_end = C.f_end; t = C.tile0;
+    }
+    if (f < f_end) {
+      T = p.tiles[t];
+      const int off = f - T.kt_off;
+      g = off / T.n_key_tiles;
+      kt = off - g * T.n_key_tiles;
+    }
+  }
+  // Advances to the next piece; false when the range is exhausted.  After a true return T, g,
+  // kt_begin, kt_end describe the piece.
+  __device__ bool next() {
+    if (f >= f_end) return false;
+    if (kt == T.n_key_tiles) {             // previous piece ended its item
+      kt = 0;
+      if (++g == n_kv) { g = 0; T = plan.tiles[++t]; }
+    }
+    kt_begin = kt;
+    kt_end = min(T.n_key_tiles, kt + (f_end - f));
+    f += kt_end - kt_begin;
+    kt = kt_end;
+    return true;
+  }
+  __device__ bool whole() const { return kt_begin == 0 && kt_end == T.n_key_tiles; }
+  __device__ int item() const { return t * n_kv + g; }
+};
+
 __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
   uint32_t r[32];
   tmem_ld32(taddr, r);
 #pragma unroll
   for (int i = 0; i < 32; ++i) dst[i] = __uint_as_float(r[i]);
 }
+__device__ __forceinline__ void bar_sync_softmax() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ float ld_cg_f(const float* p) {
+  float v;
+  asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ float4 ld_cg_f4(const float* p) {
+  float4 v;
+  asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
+
+// Merge of the partials of one split item by the 256 softmax threads of the CTA that finished last.
+// Pieces of an item live on consecutive CTAs c0..c1: slot 2*c0+1 (c0's last piece), then 2*c for the rest.
+__device__ void merge_item(const AttnParams& p, const TileRec& T, int g, int c0, int c1, int tid256) {
+  const int warp = tid256 >> 5, lane = tid256 & 31;
+  const int n_rows = T.n_tok * p.n_rep;
+  const int n_pieces = c1 - c0 + 1;
+  for (int r = warp; r < n_rows; r += 8) {
+    // weights of the pieces of this row (LSE merge); lanes hold pieces lane, lane+32, ...
+    float mx = -INFINITY;
+    for (int j = lane; j < n_pieces; j += 32) {
+      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
+      mx = fmaxf(mx, ld_cg_f(p.plan.part_lse + (long long)slot * kBM + r));
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+    float wsum = 0.f;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int j = 0; j < n_pieces; ++j) {
+      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
+      const float ls = ld_cg_f(p.plan.part_lse + (long long)slot * kBM + r);
+      const float wgt = (ls == -INFINITY) ? 0.f : exp2f((ls - mx) * kLog2e);
+      if (wgt > 0.f) {
+        const float4 v = ld_cg_f4(p.plan.part_o + ((long long)slot * kBM + r) * kD + lane * 4);
+        acc.x = fmaf(wgt, v.x, acc.x); acc.y = fmaf(wgt, v.y, acc.y);
+        acc.z = fmaf(wgt, v.z, acc.z); acc.w = fmaf(wgt, v.w, acc.w);
+      }
+      wsum += wgt;
+    }
+    const float inv = wsum > 0.f ? 1.0f / wsum : 0.f;
+    const int tok_local = r / p.n_rep;
+    const int head = g * p.n_rep + (r - tok_local * p.n_rep);
+    const long long row = (long long)(T.q_tok0 + tok_local) * p.n_q_heads + head;
+    uint2 pk;
+    pk.x = pack_bf16x2(acc.x * inv, acc.y * inv);
+    pk.y = pack_bf16x2(acc.z * inv, acc.w * inv);
+    reinterpret_cast<uint2*>(p.out + row * kD)[lane] = pk;
+    if (p.lse && lane == 0) p.lse[row] = mx + logf(wsum);
+  }
+}
 
 __global__ void __launch_bounds__(kThreads, 1)
 lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_knew,
                            const __grid_constant__ CUtensorMap map_vnew, const __grid_constant__ CUtensorMap map_kc,
                            const __grid_constant__ CUtensorMap map_vc, const AttnParams p) {
-  extern __shared__ uint8_t smem_raw[];
-  AttnSmem& sm = *reinterpret_cast<AttnSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  AttnSmem& sm = *reinterpret_cast<AttnSmem*>(smem_raw);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
+    if (smem_u32(smem_raw) & 1023u) __trap();          // the 128-byte swizzle atoms need 1024-byte alignment
     mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 1);
     for (int s = 0; s < kStages; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.v_full[s], 1); mbar_init(&sm.kv_empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); }
-    mbar_init(&sm.pv_done, 1); mbar_init(&sm.o_empty, 128);
+    for (int b = 0; b < 2; ++b) { mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); mbar_init(&sm.pv_done[b], 1); }
+    mbar_init(&sm.o_empty, 256);
     fence_barrier_init();
     prefetch_tensormap(&map_q); prefetch_tensormap(&map_knew); prefetch_tensormap(&map_vnew);
     prefetch_tensormap(&map_kc); prefetch_tensormap(&map_vc);
@@ -236,63 +382,63 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   const uint32_t t_s[2] = {tmem, tmem + 128};
-  const uint32_t t_o = tmem + 256;
-  const int n_work = p.plan.hdr->n_work;
+  const uint32_t t_o[2] = {tmem + 256, tmem + 384};
+  const bool active = (int)blockIdx.x < p.plan.hdr->n_ctas;
 
-  if (warp == 0) {
-    // ===================== TMA producer =====================
-    if (lane == 0) {
-      uint32_t kv_it = 0, item_it = 0;
-      for (int w = blockIdx.x; w < n_work; w += gridDim.x, ++item_it) {
-        const WorkRec W = p.plan.work[w];
-        const TileRec T = p.plan.tiles[W.tile];
-        mbar_wait(&sm.q_empty, (item_it & 1) ^ 1);
+  if (warp < 4) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    if (warp == 0 && lane == 0 && active) {
+      // ===================== TMA producer =====================
+      uint32_t kv_it = 0, piece_it = 0;
+      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+      while (w.next()) {
+        const TileRec& T = w.T;
+        mbar_wait(&sm.q_empty, (piece_it & 1) ^ 1);
         mbar_arrive_expect_tx(&sm.q_full, p.q_box_bytes);   // the box is tpt*n_rep (<= 128) rows per half
-        tma_load_3d(sm.q[0], &map_q, &sm.q_full, 0, W.g * p.n_rep, T.q_tok0);
-        tma_load_3d(sm.q[1], &map_q, &sm.q_full, 64, W.g * p.n_rep, T.q_tok0);
-        for (int kt = W.kt_begin; kt < W.kt_end; ++kt, ++kv_it) {
+        tma_load_3d(sm.q[0], &map_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0);
+        tma_load_3d(sm.q[1], &map_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0);
+        for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
           const int s = kv_it % kStages;
           const uint32_t ph = (kv_it / kStages) & 1;
           mbar_wait(&sm.kv_empty[s], ph ^ 1);
           mbar_arrive_expect_tx(&sm.k_full[s], kTileBytes);
           if (kt < T.n_pref_tiles) {
             const int row = T.kv_base_row + kt * kBN;
-            tma_load_3d(sm.k[s][0], &map_kc, &sm.k_full[s], 0, row, W.g);
-            tma_load_3d(sm.k[s][1], &map_kc, &sm.k_full[s], 64, row, W.g);
+            tma_load_3d(sm.k[s][0], &map_kc, &sm.k_full[s], 0, row, w.g);
+            tma_load_3d(sm.k[s][1], &map_kc, &sm.k_full[s], 64, row, w.g);
             mbar_arrive_expect_tx(&sm.v_full[s], kTileBytes);
-            tma_load_3d(sm.v[s][0], &map_vc, &sm.v_full[s], 0, row, W.g);
-            tma_load_3d(sm.v[s][1], &map_vc, &sm.v_full[s], 64, row, W.g);
+            tma_load_3d(sm.v[s][0], &map_vc, &sm.v_full[s], 0, row, w.g);
+            tma_load_3d(sm.v[s][1], &map_vc, &sm.v_full[s], 64, row, w.g);
           } else {
             const int row = T.lk0 + (kt - T.n_pref_tiles) * kBN;
-            tma_load_3d(sm.k[s][0], &map_knew, &sm.k_full[s], 0, W.g, row);
-            tma_load_3d(sm.k[s][1], &map_knew, &sm.k_full[s], 64, W.g, row);
+            tma_load_3d(sm.k[s][0], &map_knew, &sm.k_full[s], 0, w.g, row);
+            tma_load_3d(sm.k[s][1], &map_knew, &sm.k_full[s], 64, w.g, row);
             mbar_arrive_expect_tx(&sm.v_full[s], kTileBytes);
-            tma_load_3d(sm.v[s][0], &map_vnew, &sm.v_full[s], 0, W.g, row);
-            tma_load_3d(sm.v[s][1], &map_vnew, &sm.v_full[s], 64, W.g, row);
+            tma_load_3d(sm.v[s][0], &map_vnew, &sm.v_full[s], 0, w.g, row);
+            tma_load_3d(sm.v[s][1], &map_vnew, &sm.v_full[s], 64, w.g, row);
           }
         }
+        ++piece_it;
       }
-    }
-  } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    if (lane == 0) {
+    } else if (warp == 1 && lane == 0 && active) {
+      // ===================== MMA issuer =====================
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
       const uint32_t idesc_pv = make_idesc_bf16(kBM, kD, 0, 1);
-      uint32_t kv_it = 0, sp_it = 0, item_it = 0;
-      for (int w = blockIdx.x; w < n_work; w += gridDim.x, ++item_it) {
-        const WorkRec W = p.plan.work[w];
-        const TileRec T = p.plan.tiles[W.tile];
-        const int n = W.kt_end - W.kt_begin;
-        mbar_wait(&sm.q_full, item_it & 1);
+      uint32_t kv_it = 0, piece_it = 0;
+      uint32_t cb[2] = {0, 0};                 // tiles issued so far into S/O buffer b (all pieces)
+      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+      while (w.next()) {
+        const TileRec& T = w.T;
+        const int n = w.kt_end - w.kt_begin;
+        mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
-        const uint32_t kv_base_it = kv_it, sp_base_it = sp_it;
         for (int i = 0; i <= n; ++i) {
-          if (i < n) {
-            const uint32_t it = kv_base_it + i;
+          if (i < n) {                          // S[i&1] = Q . K_i^T
+            const uint32_t it = kv_it + i;
             const int s = it % kStages;
             mbar_wait(&sm.k_full[s], (it / kStages) & 1);
             tc_fence_after();
-            const uint32_t b = (sp_base_it + i) & 1;
+            const uint32_t b = i & 1;
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
@@ -304,45 +450,49 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
             mma_commit(&sm.s_full[b]);
             if (i == n - 1) mma_commit(&sm.q_empty);
           }
-          if (i >= 1) {
+          if (i >= 1) {                         // O[j&1] += P_j . V_j
             const int j = i - 1;
-            const uint32_t it = kv_base_it + j;
+            const uint32_t it = kv_it + j;
             const int s = it % kStages;
-            const uint32_t spj = sp_base_it + j;
-            const uint32_t b = spj & 1;
-            mbar_wait(&sm.p_full[b], (spj >> 1) & 1);
+            const uint32_t b = j & 1;
+            mbar_wait(&sm.p_full[b], (cb[b] + (uint32_t)(j >> 1)) & 1);
             mbar_wait(&sm.v_full[s], (it / kStages) & 1);
-            if (j == 0) mbar_wait(&sm.o_empty, (item_it & 1) ^ 1);
+            if (j == 0 && piece_it > 0) mbar_wait(&sm.o_empty, (piece_it - 1) & 1);
             tc_fence_after();
             // keys of this tile that any row may see, rounded up to the MMA K step
-            const int kt = W.kt_begin + j;
-            int valid = kt < T.n_pref_tiles ? min(kBN, T.kv_len_max - kt * kBN)
-                                            : min(kBN, T.lk1 - T.lk0 - (kt - T.n_pref_tiles) * kBN);
+            const int kt = w.kt_begin + j;
+            const int valid = kt < T.n_pref_tiles ? min(kBN, T.kv_len_max - kt * kBN)
+                                                  : min(kBN, T.lk1 - T.lk0 - (kt - T.n_pref_tiles) * kBN);
             const int ksteps = (valid + 15) >> 4;
             for (int k = 0; k < ksteps; ++k) {
               const uint64_t db = make_desc_sw128(smem_u32(sm.v[s][0]) + k * 2048, kHalfBytes, 1024);
-              mma_ts(t_o, t_s[b] + k * 8, db, idesc_pv, (j | k) ? 1u : 0u);
+              mma_ts(t_o[b], t_s[b] + k * 8, db, idesc_pv, (j >= 2 || k) ? 1u : 0u);
             }
             mma_commit(&sm.kv_empty[s]);
-            mma_commit(&sm.pv_done);
+            mma_commit(&sm.pv_done[b]);
           }
         }
-        kv_it += n; sp_it += n;
+        kv_it += n;
+        cb[0] += (uint32_t)((n + 1) >> 1); cb[1] += (uint32_t)(n >> 1);
+        ++piece_it;
       }
     }
   } else {
-    // ===================== softmax + epilogue: one thread per stacked row =====================
+    // ===================== softmax + epilogue: two streams, one thread per stacked row =====================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
+    const int b = (warp - 4) >> 2;                     // stream: 0 = even key tiles, 1 = odd key tiles
     const int quad = warp & 3;                         // TMEM lane group this warp may access
     const int r = quad * 32 + lane;                    // row of the tile
+    const int tid256 = threadIdx.x - 128;
     const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
-    uint32_t sp_it = 0, pv_it = 0;
-    for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-      const WorkRec W = p.plan.work[w];
-      const TileRec T = p.plan.tiles[W.tile];
-      const int n = W.kt_end - W.kt_begin;
+    uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
+    PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+    while (w.next()) {
+      const TileRec& T = w.T;
+      const int n = w.kt_end - w.kt_begin;
       // ---- this row's token, head and lane ----
       const int tok_local = r / p.n_rep;
-      const int head = W.g * p.n_rep + (r - tok_local * p.n_rep);
+      const int head = w.g * p.n_rep + (r - tok_local * p.n_rep);
       const int tok = T.q_tok0 + tok_local;
       bool valid = tok_local < T.n_tok;
       int prefix_len = 0, ls = 0, le = 0;
@@ -354,11 +504,11 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         }
       }
       float m_used = -INFINITY, l_sum = 0.f;           // m_used in raw score units
+      int n_mine = 0;
 
-      for (int i = 0; i < n; ++i, ++sp_it) {
-        const int kt = W.kt_begin + i;
-        const uint32_t b = sp_it & 1;
-        mbar_wait(&sm.s_full[b], (sp_it >> 1) & 1);
+      for (int i = b; i < n; i += 2, ++cnt, ++n_mine) {
+        const int kt = w.kt_begin + i;
+        mbar_wait(&sm.s_full[b], cnt & 1);
         tc_fence_after();
         float s[kBN];
 #pragma unroll
@@ -380,29 +530,36 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #pragma unroll
           for (int c = 0; c < kBN; ++c) s[c] = (c >= lo && c < hi) ? s[c] : -INFINITY;
         }
-        float mx = s[0];
+        float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
 #pragma unroll
-        for (int c = 1; c < kBN; ++c) mx = fmaxf(mx, s[c]);
-        // PV of the previous key tile must have landed before O may be rescaled
-        if (i > 0) { mbar_wait(&sm.pv_done, pv_it & 1); ++pv_it; tc_fence_after(); }
+        for (int c = 4; c < kBN; c += 4) {
+          mx0 = fmaxf(mx0, s[c]); mx1 = fmaxf(mx1, s[c + 1]); mx2 = fmaxf(mx2, s[c + 2]); mx3 = fmaxf(mx3, s[c + 3]);
+        }
+        const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
         const float m_new = fmaxf(m_used, mx);
         bool grow = false;
         if (m_used == -INFINITY) m_used = m_new;         // nothing accumulated yet (O row is 0 or unwritten)
         else grow = (m_new - m_used) * p.scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, grow)) {             // warp-uniform: tcgen05.ld/st are .sync.aligned
+          // rare: O of this stream must be rescaled, so its previous P.V has to have landed.  At most
+          // cnt completions of pv_done[b] can have happened here, so the parity wait cannot alias.
+          if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
           const float alpha = grow ? exp2f((m_used - m_new) * p.scale_log2) : 1.0f;
           if (grow) { l_sum *= alpha; m_used = m_new; }
+          if (n_mine > 0) {
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            uint32_t o[32];
-            tmem_ld32(t_o + lane_addr + c * 32, o);
-            tmem_wait_ld();
+            for (int c = 0; c < 4; ++c) {
+              uint32_t o[32];
+              tmem_ld32(t_o[b] + lane_addr + c * 32, o);
+              tmem_wait_ld();
 #pragma unroll
-            for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-            tmem_st32(t_o + lane_addr + c * 32, o);
+              for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+              tmem_st32(t_o[b] + lane_addr + c * 32, o);
+            }
           }
         }
         const float mb = (m_used == -INFINITY) ? 0.f : m_used * p.scale_log2;
+        float l0 = 0.f, l1 = 0.f;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t pk[16];
@@ -410,101 +567,94 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           for (int e = 0; e < 16; ++e) {
             const float p0 = exp2f(fmaf(s[c * 32 + 2 * e], p.scale_log2, -mb));
             const float p1 = exp2f(fmaf(s[c * 32 + 2 * e + 1], p.scale_log2, -mb));
-            l_sum += p0 + p1;
+            l0 += p0; l1 += p1;
             pk[e] = pack_bf16x2(p0, p1);
           }
           tmem_st16(t_s[b] + lane_addr + c * 16, pk);
         }
+        l_sum += l0 + l1;
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(&sm.p_full[b]);
       }
-      // ---- epilogue ----
-      mbar_wait(&sm.pv_done, pv_it & 1); ++pv_it;
-      tc_fence_after();
-      const float inv = l_sum > 0.f ? 1.0f / l_sum : 0.f;
-      const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
-      if (W.part_slot < 0) {
-        __nv_bfloat16* orow = p.out + ((long long)tok * p.n_q_heads + head) * kD;
+      // ---- epilogue: merge the two streams, normalise, store ----
+      if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
+      sm.ml[b][r] = make_float2(m_used, l_sum);
+      bar_sync_softmax();
+      const float2 oth = sm.ml[b ^ 1][r];
+      const float m_e = b ? oth.x : m_used, l_e = b ? oth.y : l_sum;
+      const float m_o = b ? m_used : oth.x, l_o = b ? l_sum : oth.y;
+      const float M = fmaxf(m_e, m_o);
+      const float w_e = l_e > 0.f ? exp2f((m_e - M) * p.scale_log2) : 0.f;
+      const float w_o = l_o > 0.f ? exp2f((m_o - M) * p.scale_log2) : 0.f;
+      const float L = w_e * l_e + w_o * l_o;
+      const float inv = L > 0.f ? 1.0f / L : 0.f;
+      const float f_e = w_e * inv, f_o = w_o * inv;
+      const float lse = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
+      const bool whole = w.whole();
+      const int slot = 2 * (int)blockIdx.x + (w.kt_begin == 0 ? 1 : 0);
+      __nv_bfloat16* orow = p.out + ((long long)tok * p.n_q_heads + head) * kD + b * 64;
+      float* prow = p.plan.part_o + ((long long)slot * kBM + r) * kD + b * 64;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          float o[32];
-          tmem_ld32_f(t_o + lane_addr + c * 32, o);
+      for (int c = 0; c < 2; ++c) {                    // this stream's threads store columns [64b, 64b+64)
+        float o[32];
+        tmem_ld32_f(t_o[0] + lane_addr + b * 64 + c * 32, o);
+        tmem_wait_ld();
+#pragma unroll
+        for (int e = 0; e < 32; ++e) o[e] *= f_e;
+        if (n >= 2) {                                  // the odd stream has an accumulator (warp-uniform)
+          float o2[32];
+          tmem_ld32_f(t_o[1] + lane_addr + b * 64 + c * 32, o2);
           tmem_wait_ld();
-          if (valid) {
+#pragma unroll
+          for (int e = 0; e < 32; ++e) o[e] = f_o > 0.f ? fmaf(o2[e], f_o, o[e]) : o[e];
+        }
+        if (valid) {
+          if (whole) {
             uint32_t pk[16];
 #pragma unroll
-            for (int e = 0; e < 16; ++e) pk[e] = pack_bf16x2(o[2 * e] * inv, o[2 * e + 1] * inv);
+            for (int e = 0; e < 16; ++e) pk[e] = pack_bf16x2(o[2 * e], o[2 * e + 1]);
             uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
 #pragma unroll
             for (int e = 0; e < 4; ++e) dst[e] = make_uint4(pk[4 * e], pk[4 * e + 1], pk[4 * e + 2], pk[4 * e + 3]);
-          }
-        }
-        if (valid && p.lse) p.lse[(long long)tok * p.n_q_heads + head] = lse;
-      } else {
-        float* prow = p.plan.part_o + ((long long)W.part_slot * kBM + r) * kD;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          float o[32];
-          tmem_ld32_f(t_o + lane_addr + c * 32, o);
-          tmem_wait_ld();
-          if (valid) {
+          } else {
             float4* dst = reinterpret_cast<float4*>(prow + c * 32);
 #pragma unroll
-            for (int e = 0; e < 8; ++e)
-              dst[e] = make_float4(o[4 * e] * inv, o[4 * e + 1] * inv, o[4 * e + 2] * inv, o[4 * e + 3] * inv);
+            for (int e = 0; e < 8; ++e) dst[e] = make_float4(o[4 * e], o[4 * e + 1], o[4 * e + 2], o[4 * e + 3]);
           }
         }
-        if (valid) p.plan.part_lse[(long long)W.part_slot * kBM + r] = lse;
       }
       tc_fence_before();
       mbar_arrive(&sm.o_empty);
+      if (whole) {
+        if (valid && b == 0 && p.lse) p.lse[(long long)tok * p.n_q_heads + head] = lse;
+      } else {
+        if (b == 0) p.plan.part_lse[(long long)slot * kBM + r] = valid ? lse : -INFINITY;
+        __threadfence();
+        bar_sync_softmax();
+        if (tid256 == 0) {
+          // pieces of this item live on consecutive CTAs c0..c1 (ranges are never empty)
+          const int f0 = T.kt_off + w.g * T.n_key_tiles, f1 = f0 + T.n_key_tiles;
+          int c0 = blockIdx.x, c1 = blockIdx.x;
+          while (p.plan.bounds[c0] > f0) --c0;
+          while (p.plan.bounds[c1 + 1] < f1) ++c1;
+          const int old = atomicAdd(&p.plan.counters[w.item()], 1);
+          const bool last = old == c1 - c0;
+          if (last) p.plan.counters[w.item()] = 0;     // every piece has arrived: leave the counter clean
+          sm.ticket[0] = last ? 1 : 0; sm.ticket[1] = c0; sm.ticket[2] = c1;
+        }
+        bar_sync_softmax();
+        if (sm.ticket[0]) {
+          __threadfence();
+          merge_item(p, T, w.g, sm.ticket[1], sm.ticket[2], tid256);
+        }
+      }
+      bar_sync_softmax();                              // ml / ticket are reused by the next piece
     }
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 1) { __syncwarp(); tmem_dealloc<512>(tmem); }
-}
-
-// ---------------------------------------------------------------------------------------------
-// combine: merge the split-KV partials of every split tile (one warp per stacked row)
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-lane_combine_kernel(Plan plan, int n_q_heads, int n_kv_heads, int n_rep, __nv_bfloat16* __restrict__ out,
-                    float* __restrict__ lse_out) {
-  const int n_tiles = plan.hdr->n_tiles;
-  const int t = blockIdx.x / n_kv_heads, g = blockIdx.x - t * n_kv_heads;
-  if (t >= n_tiles) return;
-  const TileRec T = plan.tiles[t];
-  if (T.n_splits <= 1) return;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_rows = T.n_tok * n_rep;
-  const int slot0 = T.part_base + g * T.n_splits;
-  for (int r = warp; r < n_rows; r += 8) {
-    float mx = -INFINITY;
-    for (int s = 0; s < T.n_splits; ++s) mx = fmaxf(mx, plan.part_lse[(long long)(slot0 + s) * kBM + r]);
-    float wsum = 0.f;
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int s = 0; s < T.n_splits; ++s) {
-      const float ls = plan.part_lse[(long long)(slot0 + s) * kBM + r];
-      const float wgt = (ls == -INFINITY) ? 0.f : exp2f((ls - mx) * kLog2e);
-      if (wgt > 0.f) {
-        const float4 v = reinterpret_cast<const float4*>(plan.part_o + ((long long)(slot0 + s) * kBM + r) * kD)[lane];
-        acc.x = fmaf(wgt, v.x, acc.x); acc.y = fmaf(wgt, v.y, acc.y);
-        acc.z = fmaf(wgt, v.z, acc.z); acc.w = fmaf(wgt, v.w, acc.w);
-      }
-      wsum += wgt;
-    }
-    const float inv = 1.0f / wsum;
-    const int tok_local = r / n_rep;
-    const int head = g * n_rep + (r - tok_local * n_rep);
-    const long long row = (long long)(T.q_tok0 + tok_local) * n_q_heads + head;
-    uint2 pk;
-    pk.x = pack_bf16x2(acc.x * inv, acc.y * inv);
-    pk.y = pack_bf16x2(acc.z * inv, acc.w * inv);
-    reinterpret_cast<uint2*>(out + row * kD)[lane] = pk;
-    if (lse_out && lane == 0) lse_out[row] = mx + logf(wsum);
-  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -515,13 +665,12 @@ Bounds bounds_for(const al_attn_shape* s, int n_lanes, int total_q_rows, int n_s
   const int tpt = kBM / n_rep;
   Bounds b;
   b.max_tiles = ceil_div(total_q_rows, tpt) + n_lanes;
-  b.max_work = b.max_tiles * s->n_kv_heads + n_sms;
-  b.max_part = 2 * n_sms + 2 * s->n_kv_heads;
+  b.grid = n_sms < kMaxCtas ? n_sms : kMaxCtas;
   return b;
 }
 
 struct WsLayout {
-  size_t hdr, tiles, work, part_lse, part_o, total;
+  size_t hdr, tiles, ctas, bounds, counters, part_lse, part_o, total;
 };
 WsLayout ws_layout(const al_attn_shape* s, const Bounds& b) {
   WsLayout L;
@@ -529,14 +678,29 @@ WsLayout ws_layout(const al_attn_shape* s, const Bounds& b) {
   auto take = [&](size_t n) { size_t o = off; off = al_round_up(off + n, 256); return o; };
   L.hdr = take(sizeof(PlanHeader));
   L.tiles = take(sizeof(TileRec) * (size_t)b.max_tiles);
-  L.work = take(sizeof(WorkRec) * (size_t)b.max_work);
-  L.part_lse = take(sizeof(float) * (size_t)b.max_part * kBM);
-  L.part_o = take(sizeof(float) * (size_t)b.max_part * kBM * kD);
+  L.ctas = take(sizeof(CtaRec) * (size_t)b.grid);
+  L.bounds = take(sizeof(int) * (size_t)(b.grid + 1));
+  L.counters = take(sizeof(int) * (size_t)b.max_tiles * s->n_kv_heads);
+  L.part_lse = take(sizeof(float) * (size_t)2 * b.grid * kBM);
+  L.part_o = take(sizeof(float) * (size_t)2 * b.grid * kBM * kD);
   L.total = off;
   return L;
 }
 
-constexpr int kSmsForBounds = 160;   // workspace sizing when no handle is at hand (>= SMs of any B200)
+constexpr int kSmsForBounds = kMaxCtas;   // workspace sizing when no handle is at hand (>= SMs of any B200)
+
+Plan plan_in(void* workspace, const WsLayout& L) {
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+  Plan plan;
+  plan.hdr = reinterpret_cast<PlanHeader*>(ws + L.hdr);
+  plan.tiles = reinterpret_cast<TileRec*>(ws + L.tiles);
+  plan.ctas = reinterpret_cast<CtaRec*>(ws + L.ctas);
+  plan.bounds = reinterpret_cast<int*>(ws + L.bounds);
+  plan.counters = reinterpret_cast<int*>(ws + L.counters);
+  plan.part_lse = reinterpret_cast<float*>(ws + L.part_lse);
+  plan.part_o = reinterpret_cast<float*>(ws + L.part_o);
+  return plan;
+}
 
 al_status make_map_3d(const al_handle* h, CUtensorMap* map, const void* base, uint64_t d0, uint64_t d1, uint64_t d2,
                       uint64_t stride1_bytes, uint64_t stride2_bytes, uint32_t b0, uint32_t b1, uint32_t b2) {
@@ -548,6 +712,14 @@ al_status make_map_3d(const al_handle* h, CUtensorMap* map, const void* base, ui
                                estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) AL_FAIL(AL_ERR_CUDA, "cuTensorMapEncodeTiled(3d) failed: %d", (int)r);
+  return AL_OK;
+}
+
+al_status check_plan_bounds(const al_attn_shape* s, int n_lanes, const Bounds& b) {
+  (void)s;
+  if (n_lanes > kMaxPlanLanes) AL_FAIL(AL_ERR_UNSUPPORTED, "al_lane_attention: more than %d lanes", kMaxPlanLanes);
+  if (b.max_tiles > kMaxPlanTiles)
+    AL_FAIL(AL_ERR_UNSUPPORTED, "al_lane_attention: more than %d query tiles (total_q_rows too large)", kMaxPlanTiles);
   return AL_OK;
 }
 
@@ -566,28 +738,35 @@ size_t al_attention_umma_workspace_bytes(const al_handle* h, const al_attn_shape
   return ws_layout(s, b).total;
 }
 
+al_status al_launch_plan_umma(const al_handle* h, const al_attn_shape* s, const al_lane_desc* lanes, int n_lanes,
+                              int total_q_rows, void* workspace, size_t workspace_bytes, cudaStream_t st) {
+  const int n_rep = s->n_q_heads / s->n_kv_heads;
+  const int tpt = kBM / n_rep;
+  const Bounds b = bounds_for(s, n_lanes, total_q_rows, h->sm_count);
+  al_status rc = check_plan_bounds(s, n_lanes, b);
+  if (rc != AL_OK) return rc;
+  const WsLayout L = ws_layout(s, b);
+  if (workspace_bytes < L.total) AL_FAIL(AL_ERR_WORKSPACE, "al_lane_plan: workspace %zu < %zu", workspace_bytes, L.total);
+  lane_plan_kernel<<<1, kPlanThreads, 0, st>>>(lanes, n_lanes, s->n_kv_heads, tpt, b, plan_in(workspace, L));
+  AL_CUDA_OK(cudaGetLastError());
+  h->launches += 1;
+  return AL_OK;
+}
+
 al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, float scale, const void* q,
                                    const void* k_new, const void* v_new, const void* k_cache, const void* v_cache,
                                    const al_lane_desc* lanes, int n_lanes, int total_q_rows, int max_prefix_len,
                                    void* out, float* lse, void* workspace, size_t workspace_bytes, cudaStream_t st) {
   (void)max_prefix_len;
-  if (n_lanes > kMaxPlanLanes) AL_FAIL(AL_ERR_UNSUPPORTED, "al_lane_attention: more than %d lanes", kMaxPlanLanes);
   const int n_rep = s->n_q_heads / s->n_kv_heads;
   const int tpt = kBM / n_rep;
-  // the workspace may have been sized without a handle (kSmsForBounds): use the bound it was sized for
-  Bounds b = bounds_for(s, n_lanes, total_q_rows, h->sm_count);
-  WsLayout L = ws_layout(s, b);
+  const Bounds b = bounds_for(s, n_lanes, total_q_rows, h->sm_count);
+  al_status rc = check_plan_bounds(s, n_lanes, b);
+  if (rc != AL_OK) return rc;
+  const WsLayout L = ws_layout(s, b);
   if (workspace_bytes < L.total) AL_FAIL(AL_ERR_WORKSPACE, "al_lane_attention: workspace %zu < %zu", workspace_bytes, L.total);
-  uint8_t* ws = static_cast<uint8_t*>(workspace);
-  Plan plan;
-  plan.hdr = reinterpret_cast<PlanHeader*>(ws + L.hdr);
-  plan.tiles = reinterpret_cast<TileRec*>(ws + L.tiles);
-  plan.work = reinterpret_cast<WorkRec*>(ws + L.work);
-  plan.part_lse = reinterpret_cast<float*>(ws + L.part_lse);
-  plan.part_o = reinterpret_cast<float*>(ws + L.part_o);
 
   CUtensorMap mq, mkn, mvn, mkc, mvc;
-  al_status rc;
   const uint64_t T = (uint64_t)total_q_rows, Hq = (uint64_t)s->n_q_heads, Hkv = (uint64_t)s->n_kv_heads;
   const uint64_t rowb = kD * 2;
   if ((rc = make_map_3d(h, &mq, q, kD, Hq, T, rowb, Hq * rowb, 64, (uint32_t)n_rep, (uint32_t)tpt)) != AL_OK) return rc;
@@ -600,22 +779,16 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   if ((rc = make_map_3d(h, &mkc, kc, kD, crows, Hkv, rowb, crows * rowb, 64, kBN, 1)) != AL_OK) return rc;
   if ((rc = make_map_3d(h, &mvc, vc, kD, crows, Hkv, rowb, crows * rowb, 64, kBN, 1)) != AL_OK) return rc;
 
-  lane_plan_kernel<<<1, 256, 0, st>>>(lanes, n_lanes, s->n_kv_heads, tpt, h->sm_count, b, plan);
-  AL_CUDA_OK(cudaGetLastError());
-
   AttnParams p;
-  p.lanes = lanes; p.plan = plan; p.out = static_cast<__nv_bfloat16*>(out); p.lse = lse;
+  p.lanes = lanes; p.plan = plan_in(workspace, L); p.out = static_cast<__nv_bfloat16*>(out); p.lse = lse;
   p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_rep = n_rep;
   p.scale_log2 = scale * kLog2e;
   p.q_box_bytes = (uint32_t)(2 * tpt * n_rep * 64 * 2);
-  const size_t smem = sizeof(AttnSmem) + 1024;
+  const size_t smem = sizeof(AttnSmem);
+  static_assert(sizeof(AttnSmem) <= 232448, "AttnSmem exceeds the 227 KB opt-in shared memory of sm_100");
   AL_CUDA_OK(cudaFuncSetAttribute(lane_attention_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const int grid = b.max_work < h->sm_count ? b.max_work : h->sm_count;
-  lane_attention_umma_kernel<<<grid, kThreads, smem, st>>>(mq, mkn, mvn, mkc, mvc, p);
+  lane_attention_umma_kernel<<<b.grid, kThreads, smem, st>>>(mq, mkn, mvn, mkc, mvc, p);
   AL_CUDA_OK(cudaGetLastError());
-  lane_combine_kernel<<<b.max_tiles * s->n_kv_heads, 256, 0, st>>>(plan, s->n_q_heads, s->n_kv_heads, n_rep,
-                                                                    static_cast<__nv_bfloat16*>(out), lse);
-  AL_CUDA_OK(cudaGetLastError());
-  h->launches += 3;
+  h->launches += 1;
   return AL_OK;
 }

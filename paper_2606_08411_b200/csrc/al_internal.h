@@ -58,4 +58,7 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
                                    const al_lane_desc* lanes, int n_lanes, int total_q_rows,
                                    int max_prefix_len, void* out, float* lse, void* workspace,
                                    size_t workspace_bytes, cudaStream_t st);
+al_status al_launch_plan_umma(const al_handle* h, const al_attn_shape* s, const al_lane_desc* lanes,
+                              int n_lanes, int total_q_rows, void* workspace, size_t workspace_bytes,
+                              cudaStream_t st);
 bool al_attention_umma_supported(const al_attn_shape* s);

@@ -92,12 +92,15 @@ class LaneStep:
 
     # -- the three parts ---------------------------------------------------------------------------
     def attention(self, stream=None, layers: Optional[range] = None) -> None:
+        """al_lane_plan once (the lanes are those of one scheduler iteration), then one
+        al_lane_attention_planned per layer."""
         wl = self.wl
+        self.h.al_lane_plan(self.shape, self.lanes, wl.n_lanes, self.T, self.max_prefix, self.ws_attn, stream)
         for l in (range(self.n_layers) if layers is None else layers):
-            self.h.al_lane_attention(self.shape, self.q[l], self.k_new[l], self.v_new[l], self.k_cache[l],
-                                     self.v_cache[l], self.lanes, wl.n_lanes, self.T, self.max_prefix,
-                                     self.out[l], None if self.lse is None else self.lse[l], self.ws_attn,
-                                     stream)
+            self.h.al_lane_attention_planned(self.shape, self.q[l], self.k_new[l], self.v_new[l], self.k_cache[l],
+                                             self.v_cache[l], self.lanes, wl.n_lanes, self.T, self.max_prefix,
+                                             self.out[l], None if self.lse is None else self.lse[l], self.ws_attn,
+                                             stream)
 
     def refresh(self, stream=None) -> None:
         wl = self.wl
