@@ -24,6 +24,7 @@ FLAGS = [
     "-Xcompiler", "-fPIC",
     "--expt-relaxed-constexpr",
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
+    *os.environ.get("AL_NVCC_EXTRA", "").split(),      # e.g. -DAL_ATTN_TRACE (debug stamps in the attention kernel)
 ]
 
 

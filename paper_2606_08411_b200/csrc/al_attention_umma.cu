@@ -45,7 +45,8 @@ namespace {
 constexpr int kBM = 128;                   // stacked query rows per tile
 constexpr int kBN = 128;                   // keys per key tile
 constexpr int kD = 128;                    // head_dim
-constexpr int kStages = 3;                 // K/V ring depth
+constexpr int kStagesK = 2;                // K ring depth (a K tile lives until its Q.K^T has run)
+constexpr int kStagesV = 3;                // V ring depth (a V tile lives until its P.V has run)
 constexpr int kHalfBytes = 128 * 64 * 2;   // [128 rows][64 bf16] = one 128-byte-swizzled half tile
 constexpr int kTileBytes = 2 * kHalfBytes;
 constexpr int kThreads = 384;
@@ -67,10 +68,13 @@ struct __align__(16) TileRec {             // 64 bytes
   int kt_off;                 // index of step (g = 0, kt = 0) of this tile in the flattened sequence
   int pad[4];
 };
-struct __align__(16) CtaRec {
+struct __align__(16) CtaRec {              // 96 bytes
   int f_begin, f_end;         // this CTA's range of the flattened step sequence
   int tile0;                  // tile that contains f_begin
+  int first_c0, first_c1;     // CTAs that hold pieces of the item this CTA's FIRST step belongs to
+  int last_c0, last_c1;       // same for the item of its LAST step
   int pad;
+  TileRec first;              // copy of tiles[tile0]: one load instead of two dependent ones at kernel start
 };
 struct PlanHeader {
   int n_tiles, n_items, k_total, n_ctas;
@@ -225,7 +229,20 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
       CtaRec C;
       C.f_begin = s_bounds[c]; C.f_end = s_bounds[c + 1];
       C.tile0 = n_tiles ? last_le(s_a, n_tiles, C.f_begin) : 0;
+      C.first_c0 = C.first_c1 = C.last_c0 = C.last_c1 = c;
       C.pad = 0;
+      if (n_tiles) { C.first = plan.tiles[C.tile0]; C.first.kt_off = s_a[C.tile0]; }   // written by this block above
+      if (n_tiles && C.f_begin < C.f_end) {
+        for (int e = 0; e < 2; ++e) {            // e = 0: item of the first step, 1: item of the last step
+          const int f = e ? C.f_end - 1 : C.f_begin;
+          const int t = last_le(s_a, n_tiles, f);
+          const int nk = (s_a[t + 1] - s_a[t]) / n_kv_heads;
+          const int f0 = s_a[t] + (f - s_a[t]) / nk * nk, f1 = f0 + nk;
+          const int c0 = last_le(s_bounds, n_ctas + 1, f0);            // bounds[c0] <= f0 < bounds[c0 + 1]
+          const int c1 = last_le(s_bounds, n_ctas + 1, f1 - 1);        // bounds[c1] <  f1 <= bounds[c1 + 1]
+          if (e) { C.last_c0 = c0; C.last_c1 = c1; } else { C.first_c0 = c0; C.first_c1 = c1; }
+        }
+      }
       plan.ctas[c] = C;
     }
   }
@@ -239,18 +256,23 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
 // ---------------------------------------------------------------------------------------------
 // main kernel
 // ---------------------------------------------------------------------------------------------
+constexpr int kStageRowBytes = 272;        // 256 data bytes + 16 pad: conflict-free row-per-thread writes
+
 struct AttnSmem {
   alignas(1024) uint8_t q[2][kHalfBytes];
-  alignas(1024) uint8_t k[kStages][2][kHalfBytes];
-  alignas(1024) uint8_t v[kStages][2][kHalfBytes];
-  float2 ml[2][kBM];                       // (running max, row sum) of the two softmax streams
+  alignas(1024) uint8_t k[kStagesK][2][kHalfBytes];
+  alignas(1024) uint8_t v[kStagesV][2][kHalfBytes];
+  // epilogue staging: row r holds 256 bytes of output (both streams' halves) + in its pad the
+  // (running max, row sum) pairs the two softmax streams exchange
+  alignas(16) uint8_t stage[kBM * kStageRowBytes];
   uint64_t q_full, q_empty;
-  uint64_t k_full[kStages], v_full[kStages], kv_empty[kStages];
+  uint64_t k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV];
   uint64_t s_full[2], p_full[2], pv_done[2];
   uint64_t o_empty;
   uint32_t tmem_base;
   int ticket[3];
 };
+static_assert(sizeof(AttnSmem) <= 232448, "AttnSmem exceeds the 227 KB opt-in shared memory of sm_100");
 
 struct AttnParams {
   const al_lane_desc* lanes;
@@ -269,17 +291,20 @@ struct PieceWalk {
   int f, f_end, t, g, kt;
   TileRec T;
   int kt_begin, kt_end;                    // the current piece
+  int first_c0, first_c1, last_c0, last_c1;
   __device__ PieceWalk(const Plan& p, int n_kv_heads, int cta, bool active) : plan(p), n_kv(n_kv_heads) {
     f = f_end = t = g = kt = 0;
+    first_c0 = first_c1 = last_c0 = last_c1 = cta;
     if (active) {                          // records beyond hdr->n_ctas are not written by the plan
-      const CtaRec C = p.ctas[cta];
-      f = C.f_begin; f_end = C.f_end; t = C.tile0;
-    }
-    if (f < f_end) {
-      T = p.tiles[t];
-      const int off = f - T.kt_off;
-      g = off / T.n_key_tiles;
-      kt = off - g * T.n_key_tiles;
+      const CtaRec* C = p.ctas + cta;
+      f = C->f_begin; f_end = C->f_end; t = C->tile0;
+      first_c0 = C->first_c0; first_c1 = C->first_c1; last_c0 = C->last_c0; last_c1 = C->last_c1;
+      if (f < f_end) {
+        T = C->first;
+        const int off = f - T.kt_off;
+        g = off / T.n_key_tiles;
+        kt = off - g * T.n_key_tiles;
+      }
     }
   }
   // Advances to the next piece; false when the range is exhausted.  After a true return T, g,
@@ -306,55 +331,116 @@ __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
 #pragma unroll
   for (int i = 0; i < 32; ++i) dst[i] = __uint_as_float(r[i]);
 }
+#ifdef AL_ATTN_TRACE
+// debug build only: per-CTA clock64 stamps of the first piece (slot 15 = globaltimer at entry)
+__device__ unsigned long long g_trace[kMaxCtas * 16];
+#define TRACE(i) do { if (g_trace[blockIdx.x * 16 + (i)] == 0) g_trace[blockIdx.x * 16 + (i)] = clock64(); } while (0)
+#else
+#define TRACE(i) do { } while (0)
+#endif
 __device__ __forceinline__ void bar_sync_softmax() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
-__device__ __forceinline__ float ld_cg_f(const float* p) {
-  float v;
-  asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
-  return v;
+__device__ __forceinline__ float ex2(float x) {             // x <= 8 here (or -inf)
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
-__device__ __forceinline__ float4 ld_cg_f4(const float* p) {
-  float4 v;
-  asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-  return v;
+// packed fp32x2 arithmetic (sm_100): halves the FFMA / FADD issue slots of the softmax
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
 }
 
 // Merge of the partials of one split item by the 256 softmax threads of the CTA that finished last.
-// Pieces of an item live on consecutive CTAs c0..c1: slot 2*c0+1 (c0's last piece), then 2*c for the rest.
+// Pieces of an item live on consecutive CTAs c0..c1: slot 2*c0+1 (c0's last piece), then 2*c for the
+// rest.  Warp w owns rows [16w, 16w+16); lanes 0-15 hold the rows' weights, every lane one float4
+// column group, so each piece costs 16 independent fully coalesced 512-byte row loads per warp.
 __device__ void merge_item(const AttnParams& p, const TileRec& T, int g, int c0, int c1, int tid256) {
   const int warp = tid256 >> 5, lane = tid256 & 31;
   const int n_rows = T.n_tok * p.n_rep;
+  const int row0 = warp * 16;
+  if (row0 >= n_rows) return;
   const int n_pieces = c1 - c0 + 1;
-  for (int r = warp; r < n_rows; r += 8) {
-    // weights of the pieces of this row (LSE merge); lanes hold pieces lane, lane+32, ...
-    float mx = -INFINITY;
-    for (int j = lane; j < n_pieces; j += 32) {
-      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
-      mx = fmaxf(mx, ld_cg_f(p.plan.part_lse + (long long)slot * kBM + r));
-    }
+  const int my_row = row0 + (lane & 15);
+  const bool has_row = my_row < n_rows;
+  float mx = -INFINITY;
+  for (int j = 0; j < n_pieces; ++j) {
+    const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
+    if (has_row) mx = fmaxf(mx, __ldcg(p.plan.part_lse + (long long)slot * kBM + my_row));
+  }
+  float wsum = 0.f;
+  float4 acc[16];
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, off));
-    float wsum = 0.f;
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int j = 0; j < n_pieces; ++j) {
-      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
-      const float ls = ld_cg_f(p.plan.part_lse + (long long)slot * kBM + r);
-      const float wgt = (ls == -INFINITY) ? 0.f : exp2f((ls - mx) * kLog2e);
-      if (wgt > 0.f) {
-        const float4 v = ld_cg_f4(p.plan.part_o + ((long long)slot * kBM + r) * kD + lane * 4);
-        acc.x = fmaf(wgt, v.x, acc.x); acc.y = fmaf(wgt, v.y, acc.y);
-        acc.z = fmaf(wgt, v.z, acc.z); acc.w = fmaf(wgt, v.w, acc.w);
+  for (int k = 0; k < 16; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int j = 0; j < n_pieces; ++j) {
+    const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
+    const float ls = has_row ? __ldcg(p.plan.part_lse + (long long)slot * kBM + my_row) : -INFINITY;
+    const float4* src = reinterpret_cast<const float4*>(p.plan.part_o + ((long long)slot * kBM + row0) * kD) + lane;
+    float4 v[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) v[k] = row0 + k < n_rows ? __ldcg(src + k * (kD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float wgt = (ls == -INFINITY) ? 0.f : exp2f((ls - mx) * kLog2e);   // 0: the row saw no key in this piece
+    wsum += wgt;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const float wk = __shfl_sync(0xffffffffu, wgt, k);
+      if (wk > 0.f) {                                  // rows without data in this piece hold stale memory
+        acc[k].x = fmaf(wk, v[k].x, acc[k].x); acc[k].y = fmaf(wk, v[k].y, acc[k].y);
+        acc[k].z = fmaf(wk, v[k].z, acc[k].z); acc[k].w = fmaf(wk, v[k].w, acc[k].w);
       }
-      wsum += wgt;
     }
-    const float inv = wsum > 0.f ? 1.0f / wsum : 0.f;
-    const int tok_local = r / p.n_rep;
-    const int head = g * p.n_rep + (r - tok_local * p.n_rep);
-    const long long row = (long long)(T.q_tok0 + tok_local) * p.n_q_heads + head;
-    uint2 pk;
-    pk.x = pack_bf16x2(acc.x * inv, acc.y * inv);
-    pk.y = pack_bf16x2(acc.z * inv, acc.w * inv);
-    reinterpret_cast<uint2*>(p.out + row * kD)[lane] = pk;
-    if (p.lse && lane == 0) p.lse[row] = mx + logf(wsum);
+  }
+  const float inv = wsum > 0.f ? 1.0f / wsum : 0.f;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    const float ik = __shfl_sync(0xffffffffu, inv, k);
+    const int r = row0 + k;
+    if (r < n_rows) {
+      const int tok_local = r / p.n_rep;
+      const int head = g * p.n_rep + (r - tok_local * p.n_rep);
+      const long long row = (long long)(T.q_tok0 + tok_local) * p.n_q_heads + head;
+      uint2 pk;
+      pk.x = pack_bf16x2(acc[k].x * ik, acc[k].y * ik);
+      pk.y = pack_bf16x2(acc[k].z * ik, acc[k].w * ik);
+      reinterpret_cast<uint2*>(p.out + row * kD)[lane] = pk;
+    }
+  }
+  if (p.lse && has_row && lane < 16) {
+    const int tok_local = my_row / p.n_rep;
+    const int head = g * p.n_rep + (my_row - tok_local * p.n_rep);
+    p.lse[(long long)(T.q_tok0 + tok_local) * p.n_q_heads + head] = mx + logf(wsum);
+  }
+}
+
+// Copies the staged rows [0, n_rows) of the tile to global memory with fully coalesced 16-byte
+// accesses: 16 lanes per row, two rows per warp instruction.  `dst_of(r)` gives the global address
+// of the first byte of row r's first 128-byte segment; the second segment lies seg1_off bytes on.
+template <typename RowPtr>
+__device__ __forceinline__ void copy_out_rows(const uint8_t* stage, int n_rows, int tid256, int seg1_off,
+                                              RowPtr dst_of) {
+  const int warp = tid256 >> 5, lane = tid256 & 31;
+  const int sub = lane >> 4, chunk = lane & 15;             // row within the pair, 16-byte chunk of the row
+#pragma unroll
+  for (int it = 0; it < 8; ++it) {
+    const int r = warp * 16 + it * 2 + sub;
+    if (r < n_rows) {
+      const uint4 v = *reinterpret_cast<const uint4*>(stage + r * kStageRowBytes + chunk * 16);
+      uint8_t* dst = dst_of(r) + (chunk < 8 ? chunk * 16 : seg1_off + (chunk - 8) * 16);
+      *reinterpret_cast<uint4*>(dst) = v;
+    }
   }
 }
 
@@ -366,10 +452,19 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   AttnSmem& sm = *reinterpret_cast<AttnSmem*>(smem_raw);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
+#ifdef AL_ATTN_TRACE
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 16; ++i) g_trace[blockIdx.x * 16 + i] = 0;
+    unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+    g_trace[blockIdx.x * 16 + 15] = gt;
+    g_trace[blockIdx.x * 16 + 0] = clock64();
+  }
+#endif
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) __trap();          // the 128-byte swizzle atoms need 1024-byte alignment
     mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 1);
-    for (int s = 0; s < kStages; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.v_full[s], 1); mbar_init(&sm.kv_empty[s], 1); }
+    for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 1); }
+    for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); mbar_init(&sm.pv_done[b], 1); }
     mbar_init(&sm.o_empty, 256);
     fence_barrier_init();
@@ -384,6 +479,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   const uint32_t t_s[2] = {tmem, tmem + 128};
   const uint32_t t_o[2] = {tmem + 256, tmem + 384};
   const bool active = (int)blockIdx.x < p.plan.hdr->n_ctas;
+  if (threadIdx.x == 0) TRACE(1);
 
   if (warp < 4) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
@@ -397,26 +493,22 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         mbar_arrive_expect_tx(&sm.q_full, p.q_box_bytes);   // the box is tpt*n_rep (<= 128) rows per half
         tma_load_3d(sm.q[0], &map_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0);
         tma_load_3d(sm.q[1], &map_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0);
+        TRACE(2);
         for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
-          const int s = kv_it % kStages;
-          const uint32_t ph = (kv_it / kStages) & 1;
-          mbar_wait(&sm.kv_empty[s], ph ^ 1);
-          mbar_arrive_expect_tx(&sm.k_full[s], kTileBytes);
-          if (kt < T.n_pref_tiles) {
-            const int row = T.kv_base_row + kt * kBN;
-            tma_load_3d(sm.k[s][0], &map_kc, &sm.k_full[s], 0, row, w.g);
-            tma_load_3d(sm.k[s][1], &map_kc, &sm.k_full[s], 64, row, w.g);
-            mbar_arrive_expect_tx(&sm.v_full[s], kTileBytes);
-            tma_load_3d(sm.v[s][0], &map_vc, &sm.v_full[s], 0, row, w.g);
-            tma_load_3d(sm.v[s][1], &map_vc, &sm.v_full[s], 64, row, w.g);
-          } else {
-            const int row = T.lk0 + (kt - T.n_pref_tiles) * kBN;
-            tma_load_3d(sm.k[s][0], &map_knew, &sm.k_full[s], 0, w.g, row);
-            tma_load_3d(sm.k[s][1], &map_knew, &sm.k_full[s], 64, w.g, row);
-            mbar_arrive_expect_tx(&sm.v_full[s], kTileBytes);
-            tma_load_3d(sm.v[s][0], &map_vnew, &sm.v_full[s], 0, w.g, row);
-            tma_load_3d(sm.v[s][1], &map_vnew, &sm.v_full[s], 64, w.g, row);
-          }
+          const int sk = kv_it % kStagesK, sv = kv_it % kStagesV;
+          const bool pref = kt < T.n_pref_tiles;
+          const int row = pref ? T.kv_base_row + kt * kBN : T.lk0 + (kt - T.n_pref_tiles) * kBN;
+          const CUtensorMap* mk = pref ? &map_kc : &map_knew;
+          const CUtensorMap* mv = pref ? &map_vc : &map_vnew;
+          const int c1 = pref ? row : w.g, c2 = pref ? w.g : row;   // cache [g][row][d]; new rows [row][g][d]
+          mbar_wait(&sm.k_empty[sk], ((kv_it / kStagesK) & 1) ^ 1);
+          mbar_arrive_expect_tx(&sm.k_full[sk], kTileBytes);
+          tma_load_3d(sm.k[sk][0], mk, &sm.k_full[sk], 0, c1, c2);
+          tma_load_3d(sm.k[sk][1], mk, &sm.k_full[sk], 64, c1, c2);
+          mbar_wait(&sm.v_empty[sv], ((kv_it / kStagesV) & 1) ^ 1);
+          mbar_arrive_expect_tx(&sm.v_full[sv], kTileBytes);
+          tma_load_3d(sm.v[sv][0], mv, &sm.v_full[sv], 0, c1, c2);
+          tma_load_3d(sm.v[sv][1], mv, &sm.v_full[sv], 64, c1, c2);
         }
         ++piece_it;
       }
@@ -432,12 +524,14 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         const int n = w.kt_end - w.kt_begin;
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
+        TRACE(3);
         for (int i = 0; i <= n; ++i) {
           if (i < n) {                          // S[i&1] = Q . K_i^T
             const uint32_t it = kv_it + i;
-            const int s = it % kStages;
-            mbar_wait(&sm.k_full[s], (it / kStages) & 1);
+            const int s = it % kStagesK;
+            mbar_wait(&sm.k_full[s], (it / kStagesK) & 1);
             tc_fence_after();
+            TRACE(4);
             const uint32_t b = i & 1;
 #pragma unroll
             for (int h = 0; h < 2; ++h)
@@ -448,15 +542,16 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
                 mma_ss(t_s[b], da, db, idesc_qk, (h | k) ? 1u : 0u);
               }
             mma_commit(&sm.s_full[b]);
+            mma_commit(&sm.k_empty[s]);
             if (i == n - 1) mma_commit(&sm.q_empty);
           }
           if (i >= 1) {                         // O[j&1] += P_j . V_j
             const int j = i - 1;
             const uint32_t it = kv_it + j;
-            const int s = it % kStages;
+            const int s = it % kStagesV;
             const uint32_t b = j & 1;
             mbar_wait(&sm.p_full[b], (cb[b] + (uint32_t)(j >> 1)) & 1);
-            mbar_wait(&sm.v_full[s], (it / kStages) & 1);
+            mbar_wait(&sm.v_full[s], (it / kStagesV) & 1);
             if (j == 0 && piece_it > 0) mbar_wait(&sm.o_empty, (piece_it - 1) & 1);
             tc_fence_after();
             // keys of this tile that any row may see, rounded up to the MMA K step
@@ -468,10 +563,11 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
               const uint64_t db = make_desc_sw128(smem_u32(sm.v[s][0]) + k * 2048, kHalfBytes, 1024);
               mma_ts(t_o[b], t_s[b] + k * 8, db, idesc_pv, (j >= 2 || k) ? 1u : 0u);
             }
-            mma_commit(&sm.kv_empty[s]);
+            mma_commit(&sm.v_empty[s]);
             mma_commit(&sm.pv_done[b]);
           }
         }
+        TRACE(5);
         kv_it += n;
         cb[0] += (uint32_t)((n + 1) >> 1); cb[1] += (uint32_t)(n >> 1);
         ++piece_it;
@@ -485,6 +581,8 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     const int r = quad * 32 + lane;                    // row of the tile
     const int tid256 = threadIdx.x - 128;
     const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
+    const uint64_t scale2 = pack2(p.scale_log2, p.scale_log2);
+    uint8_t* my_stage = sm.stage + r * kStageRowBytes;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
     PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
     while (w.next()) {
@@ -492,7 +590,6 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       const int n = w.kt_end - w.kt_begin;
       // ---- this row's token, head and lane ----
       const int tok_local = r / p.n_rep;
-      const int head = w.g * p.n_rep + (r - tok_local * p.n_rep);
       const int tok = T.q_tok0 + tok_local;
       bool valid = tok_local < T.n_tok;
       int prefix_len = 0, ls = 0, le = 0;
@@ -510,6 +607,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         const int kt = w.kt_begin + i;
         mbar_wait(&sm.s_full[b], cnt & 1);
         tc_fence_after();
+        if (tid256 == 0) TRACE(6);
         float s[kBN];
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32_f(t_s[b] + lane_addr + c * 32, s + c * 32);
@@ -541,10 +639,11 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         if (m_used == -INFINITY) m_used = m_new;         // nothing accumulated yet (O row is 0 or unwritten)
         else grow = (m_new - m_used) * p.scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, grow)) {             // warp-uniform: tcgen05.ld/st are .sync.aligned
-          // rare: O of this stream must be rescaled, so its previous P.V has to have landed.  At most
-          // cnt completions of pv_done[b] can have happened here, so the parity wait cannot alias.
+          // rare: O of this stream must be rescaled, so its previous P.V has to have landed (it has:
+          // the commit behind s_full covers every MMA issued before this tile's Q.K^T; the wait
+          // states the dependency and costs nothing)
           if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
-          const float alpha = grow ? exp2f((m_used - m_new) * p.scale_log2) : 1.0f;
+          const float alpha = grow ? ex2((m_used - m_new) * p.scale_log2) : 1.0f;
           if (grow) { l_sum *= alpha; m_used = m_new; }
           if (n_mine > 0) {
 #pragma unroll
@@ -558,45 +657,51 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
             }
           }
         }
-        const float mb = (m_used == -INFINITY) ? 0.f : m_used * p.scale_log2;
-        float l0 = 0.f, l1 = 0.f;
+        const float negmb = (m_used == -INFINITY) ? 0.f : -m_used * p.scale_log2;
+        const uint64_t negmb2 = pack2(negmb, negmb);
+        uint64_t sum_a = pack2(0.f, 0.f), sum_b = sum_a;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t pk[16];
 #pragma unroll
           for (int e = 0; e < 16; ++e) {
-            const float p0 = exp2f(fmaf(s[c * 32 + 2 * e], p.scale_log2, -mb));
-            const float p1 = exp2f(fmaf(s[c * 32 + 2 * e + 1], p.scale_log2, -mb));
-            l0 += p0; l1 += p1;
+            float t0, t1;
+            unpack2(ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2), t0, t1);
+            const float p0 = ex2(t0), p1 = ex2(t1);
+            if (e & 1) sum_b = fadd2(sum_b, pack2(p0, p1)); else sum_a = fadd2(sum_a, pack2(p0, p1));
             pk[e] = pack_bf16x2(p0, p1);
           }
           tmem_st16(t_s[b] + lane_addr + c * 16, pk);
         }
+        float l0, l1;
+        unpack2(fadd2(sum_a, sum_b), l0, l1);
         l_sum += l0 + l1;
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(&sm.p_full[b]);
       }
-      // ---- epilogue: merge the two streams, normalise, store ----
+      // ---- epilogue: merge the two streams, normalise, stage in shared memory, store coalesced ----
+      if (tid256 == 0) TRACE(7);
       if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
-      sm.ml[b][r] = make_float2(m_used, l_sum);
+      if (tid256 == 0) TRACE(8);
+      *reinterpret_cast<float2*>(my_stage + 256 + 8 * b) = make_float2(m_used, l_sum);
       bar_sync_softmax();
-      const float2 oth = sm.ml[b ^ 1][r];
+      const float2 oth = *reinterpret_cast<const float2*>(my_stage + 256 + 8 * (b ^ 1));
       const float m_e = b ? oth.x : m_used, l_e = b ? oth.y : l_sum;
       const float m_o = b ? m_used : oth.x, l_o = b ? l_sum : oth.y;
       const float M = fmaxf(m_e, m_o);
-      const float w_e = l_e > 0.f ? exp2f((m_e - M) * p.scale_log2) : 0.f;
-      const float w_o = l_o > 0.f ? exp2f((m_o - M) * p.scale_log2) : 0.f;
+      const float w_e = l_e > 0.f ? ex2((m_e - M) * p.scale_log2) : 0.f;
+      const float w_o = l_o > 0.f ? ex2((m_o - M) * p.scale_log2) : 0.f;
       const float L = w_e * l_e + w_o * l_o;
       const float inv = L > 0.f ? 1.0f / L : 0.f;
       const float f_e = w_e * inv, f_o = w_o * inv;
       const float lse = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
       const bool whole = w.whole();
       const int slot = 2 * (int)blockIdx.x + (w.kt_begin == 0 ? 1 : 0);
-      __nv_bfloat16* orow = p.out + ((long long)tok * p.n_q_heads + head) * kD + b * 64;
-      float* prow = p.plan.part_o + ((long long)slot * kBM + r) * kD + b * 64;
+      const int n_rows = T.n_tok * p.n_rep;
+      // this stream's threads own columns [64b, 64b+64): two chunks of 32
 #pragma unroll
-      for (int c = 0; c < 2; ++c) {                    // this stream's threads store columns [64b, 64b+64)
+      for (int c = 0; c < 2; ++c) {
         float o[32];
         tmem_ld32_f(t_o[0] + lane_addr + b * 64 + c * 32, o);
         tmem_wait_ld();
@@ -609,35 +714,46 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #pragma unroll
           for (int e = 0; e < 32; ++e) o[e] = f_o > 0.f ? fmaf(o2[e], f_o, o[e]) : o[e];
         }
-        if (valid) {
-          if (whole) {
-            uint32_t pk[16];
+        if (c == 1) { tc_fence_before(); mbar_arrive(&sm.o_empty); }    // both accumulators are in registers
+        if (whole) {                                   // bf16: 64 bytes per chunk at [128 b + 64 c)
+          uint4* dst = reinterpret_cast<uint4*>(my_stage + b * 128 + c * 64);
 #pragma unroll
-            for (int e = 0; e < 16; ++e) pk[e] = pack_bf16x2(o[2 * e], o[2 * e + 1]);
-            uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
-#pragma unroll
-            for (int e = 0; e < 4; ++e) dst[e] = make_uint4(pk[4 * e], pk[4 * e + 1], pk[4 * e + 2], pk[4 * e + 3]);
-          } else {
-            float4* dst = reinterpret_cast<float4*>(prow + c * 32);
-#pragma unroll
-            for (int e = 0; e < 8; ++e) dst[e] = make_float4(o[4 * e], o[4 * e + 1], o[4 * e + 2], o[4 * e + 3]);
+          for (int e = 0; e < 4; ++e)
+            dst[e] = make_uint4(pack_bf16x2(o[8 * e], o[8 * e + 1]), pack_bf16x2(o[8 * e + 2], o[8 * e + 3]),
+                                pack_bf16x2(o[8 * e + 4], o[8 * e + 5]), pack_bf16x2(o[8 * e + 6], o[8 * e + 7]));
+          if (c == 1) {
+            bar_sync_softmax();
+            copy_out_rows(sm.stage, n_rows, tid256, 128, [&](int rr) {
+              const int tl = rr / p.n_rep;
+              return reinterpret_cast<uint8_t*>(p.out + ((long long)(T.q_tok0 + tl) * p.n_q_heads + w.g * p.n_rep +
+                                                         (rr - tl * p.n_rep)) * kD);
+            });
           }
+        } else {                                       // fp32 partial: 128 bytes per chunk, one round per chunk
+          float4* dst = reinterpret_cast<float4*>(my_stage + b * 128);
+#pragma unroll
+          for (int e = 0; e < 8; ++e) dst[e] = make_float4(o[4 * e], o[4 * e + 1], o[4 * e + 2], o[4 * e + 3]);
+          bar_sync_softmax();
+          copy_out_rows(sm.stage, n_rows, tid256, 256, [&](int rr) {
+            return reinterpret_cast<uint8_t*>(p.plan.part_o + ((long long)slot * kBM + rr) * kD) + c * 128;
+          });
+          if (c == 0) bar_sync_softmax();              // the staging rows are rewritten by the next round
         }
       }
-      tc_fence_before();
-      mbar_arrive(&sm.o_empty);
+      if (tid256 == 0) TRACE(9);
       if (whole) {
-        if (valid && b == 0 && p.lse) p.lse[(long long)tok * p.n_q_heads + head] = lse;
+        if (valid && b == 0 && p.lse)
+          p.lse[(long long)tok * p.n_q_heads + w.g * p.n_rep + (r - tok_local * p.n_rep)] = lse;
       } else {
         if (b == 0) p.plan.part_lse[(long long)slot * kBM + r] = valid ? lse : -INFINITY;
         __threadfence();
         bar_sync_softmax();
+        if (tid256 == 0) TRACE(10);
         if (tid256 == 0) {
-          // pieces of this item live on consecutive CTAs c0..c1 (ranges are never empty)
-          const int f0 = T.kt_off + w.g * T.n_key_tiles, f1 = f0 + T.n_key_tiles;
-          int c0 = blockIdx.x, c1 = blockIdx.x;
-          while (p.plan.bounds[c0] > f0) --c0;
-          while (p.plan.bounds[c1 + 1] < f1) ++c1;
+          // pieces of this item live on consecutive CTAs c0..c1 (from the plan): a piece that does not
+          // start its item is this CTA's first piece, one that does not finish it is its last
+          const int c0 = w.kt_begin > 0 ? w.first_c0 : w.last_c0;
+          const int c1 = w.kt_begin > 0 ? w.first_c1 : w.last_c1;
           const int old = atomicAdd(&p.plan.counters[w.item()], 1);
           const bool last = old == c1 - c0;
           if (last) p.plan.counters[w.item()] = 0;     // every piece has arrived: leave the counter clean
@@ -646,16 +762,23 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         bar_sync_softmax();
         if (sm.ticket[0]) {
           __threadfence();
+          if (tid256 == 0) TRACE(11);
           merge_item(p, T, w.g, sm.ticket[1], sm.ticket[2], tid256);
+          if (tid256 == 0) TRACE(12);
         }
       }
-      bar_sync_softmax();                              // ml / ticket are reused by the next piece
+      bar_sync_softmax();                              // staging rows / pads / ticket are reused by the next piece
     }
   }
   tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) TRACE(13);
   if (warp == 1) { __syncwarp(); tmem_dealloc<512>(tmem); }
+  if (threadIdx.x == 32) TRACE(14);
 }
+#ifdef AL_ATTN_TRACE
+int trace_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace)); }
+#endif
 
 // ---------------------------------------------------------------------------------------------
 // host side
@@ -785,10 +908,13 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   p.scale_log2 = scale * kLog2e;
   p.q_box_bytes = (uint32_t)(2 * tpt * n_rep * 64 * 2);
   const size_t smem = sizeof(AttnSmem);
-  static_assert(sizeof(AttnSmem) <= 232448, "AttnSmem exceeds the 227 KB opt-in shared memory of sm_100");
   AL_CUDA_OK(cudaFuncSetAttribute(lane_attention_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   lane_attention_umma_kernel<<<b.grid, kThreads, smem, st>>>(mq, mkn, mvn, mkc, mvc, p);
   AL_CUDA_OK(cudaGetLastError());
   h->launches += 1;
   return AL_OK;
 }
+
+#ifdef AL_ATTN_TRACE
+extern "C" int al_debug_attn_trace(unsigned long long* host_out) { return trace_read(host_out); }   // [kMaxCtas * 16]
+#endif
