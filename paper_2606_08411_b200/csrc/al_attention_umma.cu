@@ -335,8 +335,12 @@ __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
 // debug build only: per-CTA clock64 stamps of the first piece (slot 15 = globaltimer at entry)
 __device__ unsigned long long g_trace[kMaxCtas * 16];
 #define TRACE(i) do { if (g_trace[blockIdx.x * 16 + (i)] == 0) g_trace[blockIdx.x * 16 + (i)] = clock64(); } while (0)
+// CTA 0 only: per key tile (first 32 of the CTA) stamps of kind k: 0 QK issued, 1 S seen by softmax, 2 P ready, 3 PV issued
+__device__ unsigned long long g_trace_tile[4 * 32];
+#define TRACE_TILE(k, i) do { if (blockIdx.x == 0 && (i) < 32) g_trace_tile[(k) * 32 + (i)] = clock64(); } while (0)
 #else
 #define TRACE(i) do { } while (0)
+#define TRACE_TILE(k, i) do { } while (0)
 #endif
 __device__ __forceinline__ void bar_sync_softmax() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 __device__ __forceinline__ float ex2(float x) {             // x <= 8 here (or -inf)
@@ -543,6 +547,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
               }
             mma_commit(&sm.s_full[b]);
             mma_commit(&sm.k_empty[s]);
+            TRACE_TILE(0, it);
             if (i == n - 1) mma_commit(&sm.q_empty);
           }
           if (i >= 1) {                         // O[j&1] += P_j . V_j
@@ -565,6 +570,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
             }
             mma_commit(&sm.v_empty[s]);
             mma_commit(&sm.pv_done[b]);
+            TRACE_TILE(3, it);
           }
         }
         TRACE(5);
@@ -608,6 +614,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         mbar_wait(&sm.s_full[b], cnt & 1);
         tc_fence_after();
         if (tid256 == 0) TRACE(6);
+        if ((tid256 & 127) == 0) TRACE_TILE(1, 2 * cnt + b);
         float s[kBN];
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32_f(t_s[b] + lane_addr + c * 32, s + c * 32);
@@ -679,6 +686,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(&sm.p_full[b]);
+        if ((tid256 & 127) == 0) TRACE_TILE(2, 2 * cnt + b);
       }
       // ---- epilogue: merge the two streams, normalise, stage in shared memory, store coalesced ----
       if (tid256 == 0) TRACE(7);
@@ -778,6 +786,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 }
 #ifdef AL_ATTN_TRACE
 int trace_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace)); }
+int trace_tile_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_tile, sizeof(g_trace_tile)); }
 #endif
 
 // ---------------------------------------------------------------------------------------------
@@ -917,4 +926,5 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
 
 #ifdef AL_ATTN_TRACE
 extern "C" int al_debug_attn_trace(unsigned long long* host_out) { return trace_read(host_out); }   // [kMaxCtas * 16]
+extern "C" int al_debug_attn_trace_tile(unsigned long long* host_out) { return trace_tile_read(host_out); }   // [4 * 32]
 #endif
