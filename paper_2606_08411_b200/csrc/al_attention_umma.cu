@@ -5,34 +5,35 @@
 // Work decomposition (built ON DEVICE from the lane descriptors by lane_plan_kernel, so the call is
 // graph-replayable with new lanes; the plan depends only on the descriptors and is reused by every
 // layer of one scheduler iteration, see al_lane_plan):
-//   run    = maximal sequence of lanes adjacent in the array, of one group, contiguous in q_start
-//   tile   = up to tpt = floor(128 / n_rep) consecutive tokens of a run; with the n_rep q-heads of a
-//            kv-head stacked under every token it is a 128-row M tile of the tensor core
-//   keys   = [prefix key tiles of 128 cache rows] ++ [local key tiles of 128 K_new rows covering the
-//            lanes that intersect the tile]; every row masks what its own lane may not see
-//   item   = (tile, kv-head): n_key_tiles iterations of the main loop
-// The iterations of all items, flattened item-major, form one sequence of K key-tile steps that is
-// cut into n_ctas contiguous, equal ranges ("stream-K"): every CTA gets the same number of steps
-// (+-1) whatever the lane structure is.  A range boundary that falls within one step of an item
-// boundary snaps to it.  An item whose steps are spread over several CTAs leaves one normalised
-// fp32 partial + LSE per CTA in the workspace; the CTA that finishes last (a ticket counter per
-// item) merges them -- no combine launch.
+//   run      = maximal sequence of lanes adjacent in the array, of one group, contiguous in q_start
+//   sub-tile = up to tpt = floor(128 / n_rep) consecutive tokens of a run; with the n_rep q-heads of
+//              a kv-head stacked under every token it is a 128-row M tile of the tensor core
+//   tile     = two consecutive sub-tiles A, B of a run (B may be empty): they share every prefix
+//              K/V tile, so each K/V tile staged in shared memory feeds 2 x (128x128x128) MMAs
+//   keys     = [prefix key tiles of 128 cache rows] ++ [local key tiles of 128 K_new rows covering the
+//              lanes that intersect the tile]; every row masks what its own lane may not see
+//   item     = (tile, kv-head): n_key_tiles steps of the main loop
+// The steps of all items, flattened item-major, form one sequence of K key-tile steps that is cut
+// into n_ctas contiguous, equal ranges ("stream-K"): every CTA gets the same number of steps (+-1)
+// whatever the lane structure is.  A range boundary that falls within one step of an item boundary
+// snaps to it.  An item whose steps are spread over several CTAs leaves one normalised fp32 partial
+// + LSE per CTA in the workspace; the CTA that finishes last (a ticket counter per item) merges
+// them -- no combine launch.
 // All CTAs that share (group, kv-head) read the same K/V tiles: HBM sees them once, L2 serves the
 // rest -- "the prefix is read once per lane group" (BASELINE north_star).
 //
 // Main kernel, persistent, 384 threads, warp-specialised, one CTA per SM:
-//   warp 0      TMA producer: Q tile once per piece, K and V tiles through a 3-stage ring
-//   warp 1      MMA issuer (one elected lane): S = Q.K^T (SS form) into TMEM buffer S[i&1];
-//               O[i&1] += P.V with P read from TMEM (TS form) and V MN-major in shared memory
-//   warps 4-7   softmax of the EVEN key tiles of the piece, one thread per stacked row
-//   warps 8-11  softmax of the ODD key tiles
-//               each group keeps its own running max / row sum and its own O accumulator in TMEM
-//               (two interleaved split-KV streams sharing Q, K and V), so the exponentials of one
-//               key tile overlap the MMAs of the next; O is rescaled lazily (only when the max
-//               grows by more than 2^8) and only then does a group wait for its previous P.V.
-//               Epilogue: the two streams are merged through 2 KB of shared memory, normalised and
-//               stored (bf16 output, or fp32 partial for a split item).
-// TMEM: S0 | S1 | O_even | O_odd, 128 fp32 columns each (P aliases S as packed bf16).
+//   warp 0      TMA producer: both Q sub-tiles once per piece, K and V tiles through 2-stage rings
+//   warp 1      MMA issuer (one elected lane): S_b = Q_b.K^T (SS form) into TMEM buffer S_b;
+//               O_b += P_b.V with P_b read from TMEM (TS form) and V MN-major in shared memory;
+//               per stream b the order is P.V of its previous key tile, then Q.K^T of the next
+//   warps 4-7   softmax of sub-tile A, one thread per stacked row
+//   warps 8-11  softmax of sub-tile B
+//               the exponentials of one sub-tile overlap the MMAs of the other; O is rescaled lazily
+//               (only when the running max grows by more than 2^8).  Epilogue per stream: normalise,
+//               stage 128-byte half rows in shared memory, store coalesced (bf16 output, or fp32
+//               partial for a split item).
+// TMEM: S_A | S_B | O_A | O_B, 128 fp32 columns each (P aliases S as packed bf16).
 #include <cuda_bf16.h>
 
 #include "al_internal.h"
@@ -46,7 +47,7 @@ constexpr int kBM = 128;                   // stacked query rows per tile
 constexpr int kBN = 128;                   // keys per key tile
 constexpr int kD = 128;                    // head_dim
 constexpr int kStagesK = 2;                // K ring depth (a K tile lives until its Q.K^T has run)
-constexpr int kStagesV = 3;                // V ring depth (a V tile lives until its P.V has run)
+constexpr int kStagesV = 2;                // V ring depth (a V tile lives until its P.V has run)
 constexpr int kHalfBytes = 128 * 64 * 2;   // [128 rows][64 bf16] = one 128-byte-swizzled half tile
 constexpr int kTileBytes = 2 * kHalfBytes;
 constexpr int kThreads = 384;
@@ -59,14 +60,14 @@ constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
 constexpr int kMinPiece = 2;               // do not cut the work finer than 2 key-tile steps per CTA
 
 struct __align__(16) TileRec {             // 64 bytes
-  int q_tok0, n_tok;          // first packed token row, tokens in the tile
+  int q_tok0, n_tok;          // first packed token row, tokens in the tile (<= 2 tpt)
   int kv_base_row;            // cache row of prefix key 0
   int kv_len_max, kv_len_min; // largest / smallest prefix_len among the lanes of the tile
   int lk0, lk1;               // local keys: packed rows [lk0, lk1) of K_new / V_new
   int lane_first, lane_count;
   int n_pref_tiles, n_key_tiles;
   int kt_off;                 // index of step (g = 0, kt = 0) of this tile in the flattened sequence
-  int pad[4];
+  int sub_lk0[2], sub_lk1[2]; // local key rows the lanes of sub-tile A / B can see (lk0 > lk1: none)
 };
 struct __align__(16) CtaRec {              // 96 bytes
   int f_begin, f_end;         // this CTA's range of the flattened step sequence
@@ -85,9 +86,9 @@ struct Plan {
   TileRec* tiles;
   CtaRec* ctas;
   int* bounds;       // [n_ctas + 1]
-  int* counters;     // [n_items] tickets, zero between calls (the merging CTA resets its item's)
-  float* part_o;     // [2 * grid][128][128]  slot 2c: CTA c's first piece, 2c+1: its last piece
-  float* part_lse;   // [2 * grid][128]
+  int* counters;     // [n_items][2] tickets per (item, sub-tile), zero between calls (the merging CTA resets its item's)
+  float* part_o;     // [2 * grid][256][128]  slot 2c: CTA c's first piece, 2c+1: its last piece
+  float* part_lse;   // [2 * grid][256]          (rows 128.. belong to sub-tile B)
 };
 
 struct Bounds {
@@ -175,7 +176,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   // tiles per run
   for (int r = tid; r < n_runs; r += blockDim.x) {
     const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
-    s_run_tile_base[r] = ceil_div(max(0, s_qe[l1 - 1] - s_qs[l0]), tpt);
+    s_run_tile_base[r] = ceil_div(max(0, s_qe[l1 - 1] - s_qs[l0]), 2 * tpt);
   }
   __syncthreads();
   int n_tiles = block_exclusive_scan(s_run_tile_base, n_runs, s_warp);
@@ -185,10 +186,11 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     const int r = last_le(s_run_tile_base, n_runs, t);
     const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
     TileRec T;
-    T.q_tok0 = s_qs[l0] + (t - s_run_tile_base[r]) * tpt;
-    T.n_tok = min(tpt, s_qe[l1 - 1] - T.q_tok0);
+    T.q_tok0 = s_qs[l0] + (t - s_run_tile_base[r]) * 2 * tpt;
+    T.n_tok = min(2 * tpt, s_qe[l1 - 1] - T.q_tok0);
     T.kv_base_row = lanes[l0].kv_base_row;
     T.kv_len_max = 0; T.kv_len_min = 0x7fffffff; T.lk0 = 0x7fffffff; T.lk1 = 0;
+    T.sub_lk0[0] = T.sub_lk0[1] = 0x7fffffff; T.sub_lk1[0] = T.sub_lk1[1] = 0;
     const int lf = l0 + last_le(s_qs + l0, l1 - l0, T.q_tok0);    // lane that holds the tile's first token
     int l = lf;
     for (; l < l1 && s_qs[l] < T.q_tok0 + T.n_tok; ++l) {
@@ -196,11 +198,16 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
       T.kv_len_min = min(T.kv_len_min, s_pl[l]);
       T.lk0 = min(T.lk0, s_qs[l]);
       T.lk1 = max(T.lk1, s_qe[l]);
+#pragma unroll
+      for (int b = 0; b < 2; ++b) {
+        const int t0 = T.q_tok0 + b * tpt, t1 = min(t0 + tpt, T.q_tok0 + T.n_tok);
+        if (s_qs[l] < t1 && s_qe[l] > t0) { T.sub_lk0[b] = min(T.sub_lk0[b], s_qs[l]); T.sub_lk1[b] = max(T.sub_lk1[b], s_qe[l]); }
+      }
     }
     T.lane_first = lf; T.lane_count = l - lf;
     T.n_pref_tiles = ceil_div(T.kv_len_max, kBN);
     T.n_key_tiles = T.n_pref_tiles + ceil_div(T.lk1 - T.lk0, kBN);
-    T.kt_off = 0; T.pad[0] = T.pad[1] = T.pad[2] = T.pad[3] = 0;
+    T.kt_off = 0;
     plan.tiles[t] = T;
     s_a[t] = T.n_key_tiles * n_kv_heads;
   }
@@ -246,7 +253,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
       plan.ctas[c] = C;
     }
   }
-  for (int i = tid; i < n_tiles * n_kv_heads; i += blockDim.x) plan.counters[i] = 0;
+  for (int i = tid; i < 2 * n_tiles * n_kv_heads; i += blockDim.x) plan.counters[i] = 0;   // one per (item, sub-tile)
   if (tid == 0) {
     plan.hdr->n_tiles = n_tiles; plan.hdr->n_items = n_tiles * n_kv_heads;
     plan.hdr->k_total = k_total; plan.hdr->n_ctas = k_total > 0 ? n_ctas : 0;
@@ -256,21 +263,18 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
 // ---------------------------------------------------------------------------------------------
 // main kernel
 // ---------------------------------------------------------------------------------------------
-constexpr int kStageRowBytes = 272;        // 256 data bytes + 16 pad: conflict-free row-per-thread writes
+constexpr int kStagePitch = 136;           // 128 data bytes + 8 pad: conflict-free 8-byte row-per-thread writes
 
 struct AttnSmem {
-  alignas(1024) uint8_t q[2][kHalfBytes];
+  alignas(1024) uint8_t q[2][2][kHalfBytes];           // [sub-tile][64-column half]
   alignas(1024) uint8_t k[kStagesK][2][kHalfBytes];
   alignas(1024) uint8_t v[kStagesV][2][kHalfBytes];
-  // epilogue staging: row r holds 256 bytes of output (both streams' halves) + in its pad the
-  // (running max, row sum) pairs the two softmax streams exchange
-  alignas(16) uint8_t stage[kBM * kStageRowBytes];
+  alignas(16) uint8_t stage[2 * kBM * kStagePitch];    // epilogue staging: half row (stream b, row r) at b*128 + r
   uint64_t q_full, q_empty;
   uint64_t k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV];
-  uint64_t s_full[2], p_full[2], pv_done[2];
-  uint64_t o_empty;
+  uint64_t s_full[2], p_full[2], pv_done[2], o_empty[2];
   uint32_t tmem_base;
-  int ticket[3];
+  int ticket[2][3];
 };
 static_assert(sizeof(AttnSmem) <= 232448, "AttnSmem exceeds the 227 KB opt-in shared memory of sm_100");
 
@@ -279,8 +283,8 @@ struct AttnParams {
   Plan plan;
   __nv_bfloat16* out;
   float* lse;
-  int n_q_heads, n_kv_heads, n_rep;
-  uint32_t q_box_bytes;
+  int n_q_heads, n_kv_heads, n_rep, tpt;
+  uint32_t q_box_bytes;                    // bytes of ONE sub-tile's Q box (both halves)
   float scale_log2;
 };
 
@@ -325,6 +329,15 @@ struct PieceWalk {
   __device__ int item() const { return t * n_kv + g; }
 };
 
+// Does sub-tile b of tile T have work in key tile kt?  (prefix tiles: always; local tiles: only
+// those that hold rows of the lanes the sub-tile's tokens belong to)
+__device__ __forceinline__ bool takes_part(const TileRec& T, int tpt, int b, int kt) {
+  if (b * tpt >= T.n_tok) return false;
+  if (kt < T.n_pref_tiles) return true;
+  const int k0 = T.lk0 + (kt - T.n_pref_tiles) * kBN;
+  return T.sub_lk0[b] < k0 + kBN && T.sub_lk1[b] > k0;
+}
+
 __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
   uint32_t r[32];
   tmem_ld32(taddr, r);
@@ -335,14 +348,17 @@ __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
 // debug build only: per-CTA clock64 stamps of the first piece (slot 15 = globaltimer at entry)
 __device__ unsigned long long g_trace[kMaxCtas * 16];
 #define TRACE(i) do { if (g_trace[blockIdx.x * 16 + (i)] == 0) g_trace[blockIdx.x * 16 + (i)] = clock64(); } while (0)
-// CTA 0 only: per key tile (first 32 of the CTA) stamps of kind k: 0 QK issued, 1 S seen by softmax, 2 P ready, 3 PV issued
+// CTA 0 only: per step (first 32 of the CTA) stamps of kind k: 0 QK_A issued, 1 S seen by stream A, 2 P_A ready, 3 PV_A issued
 __device__ unsigned long long g_trace_tile[4 * 32];
 #define TRACE_TILE(k, i) do { if (blockIdx.x == 0 && (i) < 32) g_trace_tile[(k) * 32 + (i)] = clock64(); } while (0)
 #else
 #define TRACE(i) do { } while (0)
 #define TRACE_TILE(k, i) do { } while (0)
 #endif
-__device__ __forceinline__ void bar_sync_softmax() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ void bar_sync_stream(int b) { asm volatile("bar.sync %0, 128;" ::"r"(1 + b) : "memory"); }
+__device__ __forceinline__ void mbar_arrive_n(uint64_t* bar, uint32_t n) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(n) : "memory");
+}
 __device__ __forceinline__ float ex2(float x) {             // x <= 8 here (or -inf)
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -368,83 +384,86 @@ __device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
   return d;
 }
 
-// Merge of the partials of one split item by the 256 softmax threads of the CTA that finished last.
-// Pieces of an item live on consecutive CTAs c0..c1: slot 2*c0+1 (c0's last piece), then 2*c for the
-// rest.  Warp w owns rows [16w, 16w+16); lanes 0-15 hold the rows' weights, every lane one float4
-// column group, so each piece costs 16 independent fully coalesced 512-byte row loads per warp.
-__device__ void merge_item(const AttnParams& p, const TileRec& T, int g, int c0, int c1, int tid256) {
-  const int warp = tid256 >> 5, lane = tid256 & 31;
-  const int n_rows = T.n_tok * p.n_rep;
-  const int row0 = warp * 16;
-  if (row0 >= n_rows) return;
+// global row (token-major [T][H_q][d]) of stacked row r of sub-tile b
+__device__ __forceinline__ long long out_row(const AttnParams& p, const TileRec& T, int g, int b, int r) {
+  const int tl = r / p.n_rep;
+  return (long long)(T.q_tok0 + b * p.tpt + tl) * p.n_q_heads + g * p.n_rep + (r - tl * p.n_rep);
+}
+__device__ __forceinline__ int sub_rows(const AttnParams& p, const TileRec& T, int b) {
+  return max(0, min(p.tpt, T.n_tok - b * p.tpt)) * p.n_rep;
+}
+
+// Merge of the partials of sub-tile b of one split item by the 128 threads of stream b in the CTA
+// that finished last.  Pieces of an item live on consecutive CTAs c0..c1: slot 2*c0+1 (c0's last
+// piece), then 2*c for the rest.  Warp w owns rows [32w, 32w+32) in two passes of 16: lanes 0-15 hold
+// the rows' weights, every lane one float4 column group, so each piece costs 16 independent fully
+// coalesced 512-byte row loads per warp and pass.
+__device__ void merge_item(const AttnParams& p, const TileRec& T, int g, int b, int c0, int c1, int tid128) {
+  const int warp = tid128 >> 5, lane = tid128 & 31;
+  const int n_rows = sub_rows(p, T, b);
   const int n_pieces = c1 - c0 + 1;
-  const int my_row = row0 + (lane & 15);
-  const bool has_row = my_row < n_rows;
-  float mx = -INFINITY;
-  for (int j = 0; j < n_pieces; ++j) {
-    const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
-    if (has_row) mx = fmaxf(mx, __ldcg(p.plan.part_lse + (long long)slot * kBM + my_row));
-  }
-  float wsum = 0.f;
-  float4 acc[16];
+  for (int pass = 0; pass < 2; ++pass) {
+    const int row0 = warp * 32 + pass * 16;
+    if (row0 >= n_rows) break;
+    const int my_row = row0 + (lane & 15);
+    const bool has_row = my_row < n_rows;
+    float mx = -INFINITY;
+    for (int j = 0; j < n_pieces; ++j) {
+      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
+      if (has_row) mx = fmaxf(mx, __ldcg(p.plan.part_lse + ((long long)slot * 2 + b) * kBM + my_row));
+    }
+    float wsum = 0.f;
+    float4 acc[16];
 #pragma unroll
-  for (int k = 0; k < 16; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-  for (int j = 0; j < n_pieces; ++j) {
-    const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
-    const float ls = has_row ? __ldcg(p.plan.part_lse + (long long)slot * kBM + my_row) : -INFINITY;
-    const float4* src = reinterpret_cast<const float4*>(p.plan.part_o + ((long long)slot * kBM + row0) * kD) + lane;
-    float4 v[16];
+    for (int k = 0; k < 16; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int j = 0; j < n_pieces; ++j) {
+      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
+      const float ls = has_row ? __ldcg(p.plan.part_lse + ((long long)slot * 2 + b) * kBM + my_row) : -INFINITY;
+      const float4* src =
+          reinterpret_cast<const float4*>(p.plan.part_o + (((long long)slot * 2 + b) * kBM + row0) * kD) + lane;
+      float4 v[16];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) v[k] = row0 + k < n_rows ? __ldcg(src + k * (kD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-    const float wgt = (ls == -INFINITY) ? 0.f : exp2f((ls - mx) * kLog2e);   // 0: the row saw no key in this piece
-    wsum += wgt;
+      for (int k = 0; k < 16; ++k)
+        v[k] = row0 + k < n_rows ? __ldcg(src + k * (kD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      const float wgt = (ls == -INFINITY) ? 0.f : exp2f((ls - mx) * kLog2e);   // 0: the row saw no key in this piece
+      wsum += wgt;
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const float wk = __shfl_sync(0xffffffffu, wgt, k);
-      if (wk > 0.f) {                                  // rows without data in this piece hold stale memory
-        acc[k].x = fmaf(wk, v[k].x, acc[k].x); acc[k].y = fmaf(wk, v[k].y, acc[k].y);
-        acc[k].z = fmaf(wk, v[k].z, acc[k].z); acc[k].w = fmaf(wk, v[k].w, acc[k].w);
+      for (int k = 0; k < 16; ++k) {
+        const float wk = __shfl_sync(0xffffffffu, wgt, k);
+        if (wk > 0.f) {                                // rows without data in this piece hold stale memory
+          acc[k].x = fmaf(wk, v[k].x, acc[k].x); acc[k].y = fmaf(wk, v[k].y, acc[k].y);
+          acc[k].z = fmaf(wk, v[k].z, acc[k].z); acc[k].w = fmaf(wk, v[k].w, acc[k].w);
+        }
       }
     }
-  }
-  const float inv = wsum > 0.f ? 1.0f / wsum : 0.f;
+    const float inv = wsum > 0.f ? 1.0f / wsum : 0.f;
 #pragma unroll
-  for (int k = 0; k < 16; ++k) {
-    const float ik = __shfl_sync(0xffffffffu, inv, k);
-    const int r = row0 + k;
-    if (r < n_rows) {
-      const int tok_local = r / p.n_rep;
-      const int head = g * p.n_rep + (r - tok_local * p.n_rep);
-      const long long row = (long long)(T.q_tok0 + tok_local) * p.n_q_heads + head;
-      uint2 pk;
-      pk.x = pack_bf16x2(acc[k].x * ik, acc[k].y * ik);
-      pk.y = pack_bf16x2(acc[k].z * ik, acc[k].w * ik);
-      reinterpret_cast<uint2*>(p.out + row * kD)[lane] = pk;
+    for (int k = 0; k < 16; ++k) {
+      const float ik = __shfl_sync(0xffffffffu, inv, k);
+      if (row0 + k < n_rows) {
+        uint2 pk;
+        pk.x = pack_bf16x2(acc[k].x * ik, acc[k].y * ik);
+        pk.y = pack_bf16x2(acc[k].z * ik, acc[k].w * ik);
+        reinterpret_cast<uint2*>(p.out + out_row(p, T, g, b, row0 + k) * kD)[lane] = pk;
+      }
     }
-  }
-  if (p.lse && has_row && lane < 16) {
-    const int tok_local = my_row / p.n_rep;
-    const int head = g * p.n_rep + (my_row - tok_local * p.n_rep);
-    p.lse[(long long)(T.q_tok0 + tok_local) * p.n_q_heads + head] = mx + logf(wsum);
+    if (p.lse && has_row && lane < 16) p.lse[out_row(p, T, g, b, my_row)] = mx + logf(wsum);
   }
 }
 
-// Copies the staged rows [0, n_rows) of the tile to global memory with fully coalesced 16-byte
-// accesses: 16 lanes per row, two rows per warp instruction.  `dst_of(r)` gives the global address
-// of the first byte of row r's first 128-byte segment; the second segment lies seg1_off bytes on.
+// Copies the staged 128-byte half rows [0, n_rows) of stream b to global memory with coalesced
+// 8-byte accesses: 16 lanes per half row, two half rows per warp instruction.  `dst_of(r)` is the
+// global address of half row r.
 template <typename RowPtr>
-__device__ __forceinline__ void copy_out_rows(const uint8_t* stage, int n_rows, int tid256, int seg1_off,
-                                              RowPtr dst_of) {
-  const int warp = tid256 >> 5, lane = tid256 & 31;
-  const int sub = lane >> 4, chunk = lane & 15;             // row within the pair, 16-byte chunk of the row
-#pragma unroll
-  for (int it = 0; it < 8; ++it) {
-    const int r = warp * 16 + it * 2 + sub;
-    if (r < n_rows) {
-      const uint4 v = *reinterpret_cast<const uint4*>(stage + r * kStageRowBytes + chunk * 16);
-      uint8_t* dst = dst_of(r) + (chunk < 8 ? chunk * 16 : seg1_off + (chunk - 8) * 16);
-      *reinterpret_cast<uint4*>(dst) = v;
-    }
+__device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, int n_rows, int tid128, RowPtr dst_of) {
+  const int warp = tid128 >> 5, lane = tid128 & 31;
+  const int sub = lane >> 4, chunk = lane & 15;
+#pragma unroll 4
+  for (int it = 0; it < 16; ++it) {
+    const int r = warp * 32 + it * 2 + sub;
+    if (r < n_rows)
+      *reinterpret_cast<uint2*>(dst_of(r) + chunk * 8) =
+          *reinterpret_cast<const uint2*>(stage_b + r * kStagePitch + chunk * 8);
   }
 }
 
@@ -469,8 +488,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 1);
     for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 1); }
     for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); mbar_init(&sm.pv_done[b], 1); }
-    mbar_init(&sm.o_empty, 256);
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_empty[b], 128);
+    }
     fence_barrier_init();
     prefetch_tensormap(&map_q); prefetch_tensormap(&map_knew); prefetch_tensormap(&map_vnew);
     prefetch_tensormap(&map_kc); prefetch_tensormap(&map_vc);
@@ -493,10 +513,13 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const TileRec& T = w.T;
+        const bool two = T.n_tok > p.tpt;
         mbar_wait(&sm.q_empty, (piece_it & 1) ^ 1);
-        mbar_arrive_expect_tx(&sm.q_full, p.q_box_bytes);   // the box is tpt*n_rep (<= 128) rows per half
-        tma_load_3d(sm.q[0], &map_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0);
-        tma_load_3d(sm.q[1], &map_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0);
+        mbar_arrive_expect_tx(&sm.q_full, two ? 2 * p.q_box_bytes : p.q_box_bytes);   // a box is tpt*n_rep (<= 128) rows per half
+        for (int b = 0; b < (two ? 2 : 1); ++b) {
+          tma_load_3d(sm.q[b][0], &map_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
+          tma_load_3d(sm.q[b][1], &map_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
+        }
         TRACE(2);
         for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
           const int sk = kv_it % kStagesK, sv = kv_it % kStagesV;
@@ -521,7 +544,8 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
       const uint32_t idesc_pv = make_idesc_bf16(kBM, kD, 0, 1);
       uint32_t kv_it = 0, piece_it = 0;
-      uint32_t cb[2] = {0, 0};                 // tiles issued so far into S/O buffer b (all pieces)
+      uint32_t cb[2] = {0, 0};                 // P.V issued so far for stream b (all pieces): p_full phase
+      uint32_t oe[2] = {0, 0};                 // pieces so far in which stream b had key tiles: o_empty phase
       PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const TileRec& T = w.T;
@@ -529,75 +553,101 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
         TRACE(3);
-        for (int i = 0; i <= n; ++i) {
-          if (i < n) {                          // S[i&1] = Q . K_i^T
-            const uint32_t it = kv_it + i;
-            const int s = it % kStagesK;
-            mbar_wait(&sm.k_full[s], (it / kStagesK) & 1);
-            tc_fence_after();
-            TRACE(4);
-            const uint32_t b = i & 1;
+        int pend[2] = {-1, -1};                // step of the piece whose P.V stream b still owes
+        bool first_pv[2] = {true, true};
+        int pv_left[kStagesV];                 // P.V still to issue per V stage before it is released
+        // issues the owed P.V of stream b (waits for its P), releases the V stage after its last reader
+        auto issue_pv = [&](int b) {
+          const int j = pend[b];
+          const uint32_t it = kv_it + j;
+          const int s = it % kStagesV;
+          mbar_wait(&sm.p_full[b], cb[b] & 1);
+          mbar_wait(&sm.v_full[s], (it / kStagesV) & 1);
+          // O_b of the stream's previous piece has been read out.  Only pieces in which the stream had
+          // key tiles complete a phase of o_empty[b] (oe[b] counts them), so neither side can run ahead.
+          if (first_pv[b] && oe[b] > 0) mbar_wait(&sm.o_empty[b], (oe[b] - 1) & 1);
+          tc_fence_after();
+          // keys of this tile that any row may see, rounded up to the MMA K step
+          const int kt = w.kt_begin + j;
+          const int valid = kt < T.n_pref_tiles ? min(kBN, T.kv_len_max - kt * kBN)
+                                                : min(kBN, T.lk1 - T.lk0 - (kt - T.n_pref_tiles) * kBN);
+          const int ksteps = (valid + 15) >> 4;
+          for (int k = 0; k < ksteps; ++k) {
+            const uint64_t db = make_desc_sw128(smem_u32(sm.v[s][0]) + k * 2048, kHalfBytes, 1024);
+            mma_ts(t_o[b], t_s[b] + k * 8, db, idesc_pv, (!first_pv[b] || k) ? 1u : 0u);
+          }
+          if (--pv_left[s] == 0) mma_commit(&sm.v_empty[s]);
+          mma_commit(&sm.pv_done[b]);
+          if (b == 0) TRACE_TILE(3, it);
+          first_pv[b] = false; pend[b] = -1; ++cb[b];
+        };
+        for (int i = 0; i < n; ++i) {
+          const uint32_t it = kv_it + i;
+          const int sk = it % kStagesK;
+          const int kt = w.kt_begin + i;
+          const bool part[2] = {takes_part(T, p.tpt, 0, kt), takes_part(T, p.tpt, 1, kt)};
+          pv_left[it % kStagesV] = (int)part[0] + (int)part[1];
+          bool k_ready = false;
+#pragma unroll
+          for (int b = 0; b < 2; ++b) {
+            // the owed P.V first: it frees S_b (P aliases it) for the stream's next Q.K^T, and no P.V is
+            // ever owed for more than one step (a V stage is reused two steps later)
+            if (pend[b] >= 0) issue_pv(b);
+            if (!part[b]) continue;
+            if (!k_ready) { mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1); tc_fence_after(); TRACE(4); k_ready = true; }
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
-                const uint64_t da = make_desc_sw128(smem_u32(sm.q[h]) + k * 32, 16, 1024);
-                const uint64_t db = make_desc_sw128(smem_u32(sm.k[s][h]) + k * 32, 16, 1024);
+                const uint64_t da = make_desc_sw128(smem_u32(sm.q[b][h]) + k * 32, 16, 1024);
+                const uint64_t db = make_desc_sw128(smem_u32(sm.k[sk][h]) + k * 32, 16, 1024);
                 mma_ss(t_s[b], da, db, idesc_qk, (h | k) ? 1u : 0u);
               }
             mma_commit(&sm.s_full[b]);
-            mma_commit(&sm.k_empty[s]);
-            TRACE_TILE(0, it);
-            if (i == n - 1) mma_commit(&sm.q_empty);
+            if (b == 0) TRACE_TILE(0, it);
+            pend[b] = i;
           }
-          if (i >= 1) {                         // O[j&1] += P_j . V_j
-            const int j = i - 1;
-            const uint32_t it = kv_it + j;
-            const int s = it % kStagesV;
-            const uint32_t b = j & 1;
-            mbar_wait(&sm.p_full[b], (cb[b] + (uint32_t)(j >> 1)) & 1);
-            mbar_wait(&sm.v_full[s], (it / kStagesV) & 1);
-            if (j == 0 && piece_it > 0) mbar_wait(&sm.o_empty, (piece_it - 1) & 1);
-            tc_fence_after();
-            // keys of this tile that any row may see, rounded up to the MMA K step
-            const int kt = w.kt_begin + j;
-            const int valid = kt < T.n_pref_tiles ? min(kBN, T.kv_len_max - kt * kBN)
-                                                  : min(kBN, T.lk1 - T.lk0 - (kt - T.n_pref_tiles) * kBN);
-            const int ksteps = (valid + 15) >> 4;
-            for (int k = 0; k < ksteps; ++k) {
-              const uint64_t db = make_desc_sw128(smem_u32(sm.v[s][0]) + k * 2048, kHalfBytes, 1024);
-              mma_ts(t_o[b], t_s[b] + k * 8, db, idesc_pv, (j >= 2 || k) ? 1u : 0u);
-            }
-            mma_commit(&sm.v_empty[s]);
-            mma_commit(&sm.pv_done[b]);
-            TRACE_TILE(3, it);
+          if (!k_ready) { mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1); }   // a step no sub-tile takes part in
+          mma_commit(&sm.k_empty[sk]);
+          if (pv_left[it % kStagesV] == 0) {   // nobody reads this V tile: hand the stage back once it has landed
+            mbar_wait(&sm.v_full[it % kStagesV], (it / kStagesV) & 1);
+            mma_commit(&sm.v_empty[it % kStagesV]);
           }
+          if (i == n - 1) mma_commit(&sm.q_empty);
         }
+        // owed P.V of the last steps, older step first
+        if (pend[0] >= 0 && pend[1] >= 0) {
+          if (pend[0] <= pend[1]) { issue_pv(0); issue_pv(1); } else { issue_pv(1); issue_pv(0); }
+        } else if (pend[0] >= 0) issue_pv(0);
+        else if (pend[1] >= 0) issue_pv(1);
         TRACE(5);
         kv_it += n;
-        cb[0] += (uint32_t)((n + 1) >> 1); cb[1] += (uint32_t)(n >> 1);
+        if (!first_pv[0]) ++oe[0];
+        if (!first_pv[1]) ++oe[1];
         ++piece_it;
       }
     }
   } else {
-    // ===================== softmax + epilogue: two streams, one thread per stacked row =====================
+    // ===================== softmax + epilogue: stream b = sub-tile b, one thread per stacked row =====================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
-    const int b = (warp - 4) >> 2;                     // stream: 0 = even key tiles, 1 = odd key tiles
+    const int b = (warp - 4) >> 2;                     // stream / sub-tile
     const int quad = warp & 3;                         // TMEM lane group this warp may access
-    const int r = quad * 32 + lane;                    // row of the tile
-    const int tid256 = threadIdx.x - 128;
+    const int r = quad * 32 + lane;                    // row of the sub-tile
+    const int tid128 = (threadIdx.x - 128) & 127;
     const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
     const uint64_t scale2 = pack2(p.scale_log2, p.scale_log2);
-    uint8_t* my_stage = sm.stage + r * kStageRowBytes;
+    uint8_t* stage_b = sm.stage + b * kBM * kStagePitch;
+    uint8_t* my_stage = stage_b + r * kStagePitch;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
     PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
     while (w.next()) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
-      // ---- this row's token, head and lane ----
+      const int n_rows = sub_rows(p, T, b);
+      // ---- this row's token and lane ----
       const int tok_local = r / p.n_rep;
-      const int tok = T.q_tok0 + tok_local;
-      bool valid = tok_local < T.n_tok;
+      const int tok = T.q_tok0 + b * p.tpt + tok_local;
+      bool valid = r < n_rows;
       int prefix_len = 0, ls = 0, le = 0;
       if (valid) {
         valid = false;
@@ -609,12 +659,12 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       float m_used = -INFINITY, l_sum = 0.f;           // m_used in raw score units
       int n_mine = 0;
 
-      for (int i = b; i < n; i += 2, ++cnt, ++n_mine) {
+      for (int i = 0; i < n; ++i) {
         const int kt = w.kt_begin + i;
+        if (!takes_part(T, p.tpt, b, kt)) continue;
         mbar_wait(&sm.s_full[b], cnt & 1);
         tc_fence_after();
-        if (tid256 == 0) TRACE(6);
-        if ((tid256 & 127) == 0) TRACE_TILE(1, 2 * cnt + b);
+        if (tid128 == 0 && b == 0) { TRACE(6); TRACE_TILE(1, cnt); }
         float s[kBN];
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32_f(t_s[b] + lane_addr + c * 32, s + c * 32);
@@ -686,96 +736,87 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(&sm.p_full[b]);
-        if ((tid256 & 127) == 0) TRACE_TILE(2, 2 * cnt + b);
+        if (tid128 == 0 && b == 0) TRACE_TILE(2, cnt);
+        ++cnt; ++n_mine;
       }
-      // ---- epilogue: merge the two streams, normalise, stage in shared memory, store coalesced ----
-      if (tid256 == 0) TRACE(7);
+      // ---- epilogue: normalise, stage 128-byte half rows in shared memory, store coalesced ----
+      if (tid128 == 0 && b == 0) TRACE(7);
       if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
-      if (tid256 == 0) TRACE(8);
-      *reinterpret_cast<float2*>(my_stage + 256 + 8 * b) = make_float2(m_used, l_sum);
-      bar_sync_softmax();
-      const float2 oth = *reinterpret_cast<const float2*>(my_stage + 256 + 8 * (b ^ 1));
-      const float m_e = b ? oth.x : m_used, l_e = b ? oth.y : l_sum;
-      const float m_o = b ? m_used : oth.x, l_o = b ? l_sum : oth.y;
-      const float M = fmaxf(m_e, m_o);
-      const float w_e = l_e > 0.f ? ex2((m_e - M) * p.scale_log2) : 0.f;
-      const float w_o = l_o > 0.f ? ex2((m_o - M) * p.scale_log2) : 0.f;
-      const float L = w_e * l_e + w_o * l_o;
-      const float inv = L > 0.f ? 1.0f / L : 0.f;
-      const float f_e = w_e * inv, f_o = w_o * inv;
-      const float lse = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
+      if (tid128 == 0 && b == 0) TRACE(8);
+      const float inv = l_sum > 0.f ? 1.0f / l_sum : 0.f;
+      const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
       const bool whole = w.whole();
       const int slot = 2 * (int)blockIdx.x + (w.kt_begin == 0 ? 1 : 0);
-      const int n_rows = T.n_tok * p.n_rep;
-      // this stream's threads own columns [64b, 64b+64): two chunks of 32
+      if (n_mine == 0) {
+        // nothing accumulated: no key tile of this piece concerns the sub-tile (or it is empty)
+      } else if (whole) {
+        // bf16 output: two rounds of 64 columns = 128 bytes per row
 #pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        float o[32];
-        tmem_ld32_f(t_o[0] + lane_addr + b * 64 + c * 32, o);
-        tmem_wait_ld();
+        for (int rd = 0; rd < 2; ++rd) {
 #pragma unroll
-        for (int e = 0; e < 32; ++e) o[e] *= f_e;
-        if (n >= 2) {                                  // the odd stream has an accumulator (warp-uniform)
-          float o2[32];
-          tmem_ld32_f(t_o[1] + lane_addr + b * 64 + c * 32, o2);
-          tmem_wait_ld();
+          for (int c = 0; c < 2; ++c) {
+            float o[32];
+            tmem_ld32_f(t_o[b] + lane_addr + rd * 64 + c * 32, o);
+            tmem_wait_ld();
+            if (rd == 1 && c == 1) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }   // O_b is in registers
+            uint2* dst = reinterpret_cast<uint2*>(my_stage + c * 64);
 #pragma unroll
-          for (int e = 0; e < 32; ++e) o[e] = f_o > 0.f ? fmaf(o2[e], f_o, o[e]) : o[e];
-        }
-        if (c == 1) { tc_fence_before(); mbar_arrive(&sm.o_empty); }    // both accumulators are in registers
-        if (whole) {                                   // bf16: 64 bytes per chunk at [128 b + 64 c)
-          uint4* dst = reinterpret_cast<uint4*>(my_stage + b * 128 + c * 64);
-#pragma unroll
-          for (int e = 0; e < 4; ++e)
-            dst[e] = make_uint4(pack_bf16x2(o[8 * e], o[8 * e + 1]), pack_bf16x2(o[8 * e + 2], o[8 * e + 3]),
-                                pack_bf16x2(o[8 * e + 4], o[8 * e + 5]), pack_bf16x2(o[8 * e + 6], o[8 * e + 7]));
-          if (c == 1) {
-            bar_sync_softmax();
-            copy_out_rows(sm.stage, n_rows, tid256, 128, [&](int rr) {
-              const int tl = rr / p.n_rep;
-              return reinterpret_cast<uint8_t*>(p.out + ((long long)(T.q_tok0 + tl) * p.n_q_heads + w.g * p.n_rep +
-                                                         (rr - tl * p.n_rep)) * kD);
-            });
+            for (int e = 0; e < 8; ++e)
+              dst[e] = make_uint2(pack_bf16x2(o[4 * e] * inv, o[4 * e + 1] * inv),
+                                  pack_bf16x2(o[4 * e + 2] * inv, o[4 * e + 3] * inv));
           }
-        } else {                                       // fp32 partial: 128 bytes per chunk, one round per chunk
-          float4* dst = reinterpret_cast<float4*>(my_stage + b * 128);
-#pragma unroll
-          for (int e = 0; e < 8; ++e) dst[e] = make_float4(o[4 * e], o[4 * e + 1], o[4 * e + 2], o[4 * e + 3]);
-          bar_sync_softmax();
-          copy_out_rows(sm.stage, n_rows, tid256, 256, [&](int rr) {
-            return reinterpret_cast<uint8_t*>(p.plan.part_o + ((long long)slot * kBM + rr) * kD) + c * 128;
+          bar_sync_stream(b);
+          copy_out_rows(stage_b, n_rows, tid128, [&](int rr) {
+            return reinterpret_cast<uint8_t*>(p.out + out_row(p, T, w.g, b, rr) * kD) + rd * 128;
           });
-          if (c == 0) bar_sync_softmax();              // the staging rows are rewritten by the next round
+          bar_sync_stream(b);                          // the staging rows are rewritten by the next round / piece
+        }
+        if (valid && p.lse) p.lse[out_row(p, T, w.g, b, r)] = lse;
+      } else {
+        // fp32 partial: four rounds of 32 columns = 128 bytes per row
+        float* prow0 = p.plan.part_o + ((long long)slot * 2 + b) * kBM * kD;
+#pragma unroll
+        for (int rd = 0; rd < 4; ++rd) {
+          float o[32];
+          tmem_ld32_f(t_o[b] + lane_addr + rd * 32, o);
+          tmem_wait_ld();
+          if (rd == 3) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }
+          uint2* dst = reinterpret_cast<uint2*>(my_stage);
+#pragma unroll
+          for (int e = 0; e < 16; ++e) dst[e] = make_uint2(__float_as_uint(o[2 * e] * inv), __float_as_uint(o[2 * e + 1] * inv));
+          bar_sync_stream(b);
+          copy_out_rows(stage_b, n_rows, tid128, [&](int rr) {
+            return reinterpret_cast<uint8_t*>(prow0 + (long long)rr * kD) + rd * 128;
+          });
+          bar_sync_stream(b);
         }
       }
-      if (tid256 == 0) TRACE(9);
-      if (whole) {
-        if (valid && b == 0 && p.lse)
-          p.lse[(long long)tok * p.n_q_heads + w.g * p.n_rep + (r - tok_local * p.n_rep)] = lse;
-      } else {
-        if (b == 0) p.plan.part_lse[(long long)slot * kBM + r] = valid ? lse : -INFINITY;
+      if (tid128 == 0 && b == 0) TRACE(9);
+      if (!whole && n_rows > 0) {
+        p.plan.part_lse[((long long)slot * 2 + b) * kBM + r] = (valid && n_mine > 0) ? lse : -INFINITY;
         __threadfence();
-        bar_sync_softmax();
-        if (tid256 == 0) TRACE(10);
-        if (tid256 == 0) {
+        bar_sync_stream(b);
+        if (tid128 == 0 && b == 0) TRACE(10);
+        if (tid128 == 0) {
           // pieces of this item live on consecutive CTAs c0..c1 (from the plan): a piece that does not
           // start its item is this CTA's first piece, one that does not finish it is its last
           const int c0 = w.kt_begin > 0 ? w.first_c0 : w.last_c0;
           const int c1 = w.kt_begin > 0 ? w.first_c1 : w.last_c1;
-          const int old = atomicAdd(&p.plan.counters[w.item()], 1);
+          int* counter = p.plan.counters + 2 * w.item() + b;
+          const int old = atomicAdd(counter, 1);
           const bool last = old == c1 - c0;
-          if (last) p.plan.counters[w.item()] = 0;     // every piece has arrived: leave the counter clean
-          sm.ticket[0] = last ? 1 : 0; sm.ticket[1] = c0; sm.ticket[2] = c1;
+          if (last) *counter = 0;                      // every piece has arrived: leave the counter clean
+          sm.ticket[b][0] = last ? 1 : 0; sm.ticket[b][1] = c0; sm.ticket[b][2] = c1;
         }
-        bar_sync_softmax();
-        if (sm.ticket[0]) {
+        bar_sync_stream(b);
+        if (sm.ticket[b][0]) {
           __threadfence();
-          if (tid256 == 0) TRACE(11);
-          merge_item(p, T, w.g, sm.ticket[1], sm.ticket[2], tid256);
-          if (tid256 == 0) TRACE(12);
+          if (tid128 == 0 && b == 0) TRACE(11);
+          merge_item(p, T, w.g, b, sm.ticket[b][1], sm.ticket[b][2], tid128);
+          if (tid128 == 0 && b == 0) TRACE(12);
         }
+        bar_sync_stream(b);                            // ticket is reused by the next piece
       }
-      bar_sync_softmax();                              // staging rows / pads / ticket are reused by the next piece
     }
   }
   tc_fence_before();
@@ -796,7 +837,7 @@ Bounds bounds_for(const al_attn_shape* s, int n_lanes, int total_q_rows, int n_s
   const int n_rep = s->n_q_heads / s->n_kv_heads;
   const int tpt = kBM / n_rep;
   Bounds b;
-  b.max_tiles = ceil_div(total_q_rows, tpt) + n_lanes;
+  b.max_tiles = ceil_div(total_q_rows, 2 * tpt) + n_lanes;
   b.grid = n_sms < kMaxCtas ? n_sms : kMaxCtas;
   return b;
 }
@@ -812,9 +853,9 @@ WsLayout ws_layout(const al_attn_shape* s, const Bounds& b) {
   L.tiles = take(sizeof(TileRec) * (size_t)b.max_tiles);
   L.ctas = take(sizeof(CtaRec) * (size_t)b.grid);
   L.bounds = take(sizeof(int) * (size_t)(b.grid + 1));
-  L.counters = take(sizeof(int) * (size_t)b.max_tiles * s->n_kv_heads);
-  L.part_lse = take(sizeof(float) * (size_t)2 * b.grid * kBM);
-  L.part_o = take(sizeof(float) * (size_t)2 * b.grid * kBM * kD);
+  L.counters = take(sizeof(int) * (size_t)b.max_tiles * s->n_kv_heads * 2);
+  L.part_lse = take(sizeof(float) * (size_t)2 * b.grid * 2 * kBM);
+  L.part_o = take(sizeof(float) * (size_t)2 * b.grid * 2 * kBM * kD);
   L.total = off;
   return L;
 }
@@ -913,7 +954,7 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
 
   AttnParams p;
   p.lanes = lanes; p.plan = plan_in(workspace, L); p.out = static_cast<__nv_bfloat16*>(out); p.lse = lse;
-  p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_rep = n_rep;
+  p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_rep = n_rep; p.tpt = tpt;
   p.scale_log2 = scale * kLog2e;
   p.q_box_bytes = (uint32_t)(2 * tpt * n_rep * 64 * 2);
   const size_t smem = sizeof(AttnSmem);
@@ -927,4 +968,7 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
 #ifdef AL_ATTN_TRACE
 extern "C" int al_debug_attn_trace(unsigned long long* host_out) { return trace_read(host_out); }   // [kMaxCtas * 16]
 extern "C" int al_debug_attn_trace_tile(unsigned long long* host_out) { return trace_tile_read(host_out); }   // [4 * 32]
+extern "C" int al_debug_mbar_timeout(unsigned int* host_out) {   // [4]; [0] != 0 when a wait timed out
+  return (int)cudaMemcpyFromSymbol(host_out, alptx::g_mbar_timeout, 16);
+}
 #endif

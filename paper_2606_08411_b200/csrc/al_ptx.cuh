@@ -45,12 +45,28 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
   return ok != 0;
 }
 // Bounded spin: a wedged pipeline (bad descriptor, lost arrival) traps instead of hanging the GPU.
+#ifdef AL_ATTN_TRACE
+// debug build: the first wait that times out records (block, thread, barrier smem address, parity) and returns
+__device__ unsigned int g_mbar_timeout[4];
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if (++spins > (1u << 20)) {
+      if (atomicCAS(&g_mbar_timeout[0], 0u, 0x80000000u | blockIdx.x) == 0u) {
+        g_mbar_timeout[1] = threadIdx.x; g_mbar_timeout[2] = smem_u32(bar); g_mbar_timeout[3] = parity;
+      }
+      return;
+    }
+  }
+}
+#else
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
     if (++spins > (1u << 24)) __trap();
   }
 }
+#endif
 
 // ---- TMA ----------------------------------------------------------------------------------------
 __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap* m) {
