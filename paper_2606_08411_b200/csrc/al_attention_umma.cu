@@ -290,17 +290,18 @@ struct AttnParams {
 
 // One CTA's walk over its range of the flattened step sequence: pieces (tile, g, [kt_begin, kt_end)).
 struct PieceWalk {
-  const Plan& plan;
+  const TileRec* tiles;
   int n_kv;
   int f, f_end, t, g, kt;
   TileRec T;
   int kt_begin, kt_end;                    // the current piece
   int first_c0, first_c1, last_c0, last_c1;
-  __device__ PieceWalk(const Plan& p, int n_kv_heads, int cta, bool active) : plan(p), n_kv(n_kv_heads) {
+  __device__ __forceinline__ PieceWalk(const CtaRec* ctas, const TileRec* tiles_, int n_kv_heads, int cta, bool active)
+      : tiles(tiles_), n_kv(n_kv_heads) {
     f = f_end = t = g = kt = 0;
     first_c0 = first_c1 = last_c0 = last_c1 = cta;
     if (active) {                          // records beyond hdr->n_ctas are not written by the plan
-      const CtaRec* C = p.ctas + cta;
+      const CtaRec* C = ctas + cta;
       f = C->f_begin; f_end = C->f_end; t = C->tile0;
       first_c0 = C->first_c0; first_c1 = C->first_c1; last_c0 = C->last_c0; last_c1 = C->last_c1;
       if (f < f_end) {
@@ -313,11 +314,11 @@ struct PieceWalk {
   }
   // Advances to the next piece; false when the range is exhausted.  After a true return T, g,
   // kt_begin, kt_end describe the piece.
-  __device__ bool next() {
+  __device__ __forceinline__ bool next() {
     if (f >= f_end) return false;
     if (kt == T.n_key_tiles) {             // previous piece ended its item
       kt = 0;
-      if (++g == n_kv) { g = 0; T = plan.tiles[++t]; }
+      if (++g == n_kv) { g = 0; T = tiles[++t]; }
     }
     kt_begin = kt;
     kt_end = min(T.n_key_tiles, kt + (f_end - f));
@@ -325,8 +326,8 @@ struct PieceWalk {
     kt = kt_end;
     return true;
   }
-  __device__ bool whole() const { return kt_begin == 0 && kt_end == T.n_key_tiles; }
-  __device__ int item() const { return t * n_kv + g; }
+  __device__ __forceinline__ bool whole() const { return kt_begin == 0 && kt_end == T.n_key_tiles; }
+  __device__ __forceinline__ int item() const { return t * n_kv + g; }
 };
 
 // Does sub-tile b of tile T have work in key tile kt?  (prefix tiles: always; local tiles: only
@@ -349,7 +350,7 @@ __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
 __device__ unsigned long long g_trace[kMaxCtas * 16];
 #define TRACE(i) do { if (g_trace[blockIdx.x * 16 + (i)] == 0) g_trace[blockIdx.x * 16 + (i)] = clock64(); } while (0)
 // CTA 0 only: per step (first 32 of the CTA) stamps of kind k: 0 QK_A issued, 1 S seen by stream A, 2 P_A ready, 3 PV_A issued
-__device__ unsigned long long g_trace_tile[4 * 32];
+__device__ unsigned long long g_trace_tile[12 * 32];
 #define TRACE_TILE(k, i) do { if (blockIdx.x == 0 && (i) < 32) g_trace_tile[(k) * 32 + (i)] = clock64(); } while (0)
 #else
 #define TRACE(i) do { } while (0)
@@ -398,7 +399,7 @@ __device__ __forceinline__ int sub_rows(const AttnParams& p, const TileRec& T, i
 // piece), then 2*c for the rest.  Warp w owns rows [32w, 32w+32) in two passes of 16: lanes 0-15 hold
 // the rows' weights, every lane one float4 column group, so each piece costs 16 independent fully
 // coalesced 512-byte row loads per warp and pass.
-__device__ void merge_item(const AttnParams& p, const TileRec& T, int g, int b, int c0, int c1, int tid128) {
+__device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T, int g, int b, int c0, int c1, int tid128) {
   const int warp = tid128 >> 5, lane = tid128 & 31;
   const int n_rows = sub_rows(p, T, b);
   const int n_pieces = c1 - c0 + 1;
@@ -506,11 +507,11 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   if (threadIdx.x == 0) TRACE(1);
 
   if (warp < 4) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
     if (warp == 0 && lane == 0 && active) {
       // ===================== TMA producer =====================
       uint32_t kv_it = 0, piece_it = 0;
-      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+      PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const TileRec& T = w.T;
         const bool two = T.n_tok > p.tpt;
@@ -541,89 +542,109 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       }
     } else if (warp == 1 && lane == 0 && active) {
       // ===================== MMA issuer =====================
+      // every descriptor is a constant plus a small address offset: build the bases once
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
       const uint32_t idesc_pv = make_idesc_bf16(kBM, kD, 0, 1);
+      uint64_t dq[2][2], dk[kStagesK][2], dv[kStagesV];
+#pragma unroll
+      for (int b = 0; b < 2; ++b)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) dq[b][h] = make_desc_sw128(smem_u32(sm.q[b][h]), 16, 1024);
+#pragma unroll
+      for (int s = 0; s < kStagesK; ++s)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) dk[s][h] = make_desc_sw128(smem_u32(sm.k[s][h]), 16, 1024);
+#pragma unroll
+      for (int s = 0; s < kStagesV; ++s) dv[s] = make_desc_sw128(smem_u32(sm.v[s][0]), kHalfBytes, 1024);
       uint32_t kv_it = 0, piece_it = 0;
-      uint32_t cb[2] = {0, 0};                 // P.V issued so far for stream b (all pieces): p_full phase
-      uint32_t oe[2] = {0, 0};                 // pieces so far in which stream b had key tiles: o_empty phase
-      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+      uint32_t cb0 = 0, cb1 = 0;               // P.V issued so far per stream (all pieces): p_full phase
+      uint32_t oe0 = 0, oe1 = 0;               // pieces so far in which the stream had key tiles: o_empty phase
+      PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
-        const TileRec& T = w.T;
         const int n = w.kt_end - w.kt_begin;
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
         TRACE(3);
-        int pend[2] = {-1, -1};                // step of the piece whose P.V stream b still owes
-        bool first_pv[2] = {true, true};
-        int pv_left[kStagesV];                 // P.V still to issue per V stage before it is released
-        // issues the owed P.V of stream b (waits for its P), releases the V stage after its last reader
-        auto issue_pv = [&](int b) {
-          const int j = pend[b];
-          const uint32_t it = kv_it + j;
-          const int s = it % kStagesV;
-          mbar_wait(&sm.p_full[b], cb[b] & 1);
-          mbar_wait(&sm.v_full[s], (it / kStagesV) & 1);
-          // O_b of the stream's previous piece has been read out.  Only pieces in which the stream had
-          // key tiles complete a phase of o_empty[b] (oe[b] counts them), so neither side can run ahead.
-          if (first_pv[b] && oe[b] > 0) mbar_wait(&sm.o_empty[b], (oe[b] - 1) & 1);
-          tc_fence_after();
-          // keys of this tile that any row may see, rounded up to the MMA K step
-          const int kt = w.kt_begin + j;
-          const int valid = kt < T.n_pref_tiles ? min(kBN, T.kv_len_max - kt * kBN)
-                                                : min(kBN, T.lk1 - T.lk0 - (kt - T.n_pref_tiles) * kBN);
-          const int ksteps = (valid + 15) >> 4;
-          for (int k = 0; k < ksteps; ++k) {
-            const uint64_t db = make_desc_sw128(smem_u32(sm.v[s][0]) + k * 2048, kHalfBytes, 1024);
-            mma_ts(t_o[b], t_s[b] + k * 8, db, idesc_pv, (!first_pv[b] || k) ? 1u : 0u);
-          }
-          if (--pv_left[s] == 0) mma_commit(&sm.v_empty[s]);
-          mma_commit(&sm.pv_done[b]);
-          if (b == 0) TRACE_TILE(3, it);
-          first_pv[b] = false; pend[b] = -1; ++cb[b];
-        };
+        int pend0 = -1, pend1 = -1;            // step of the piece whose P.V the stream still owes
+        bool first0 = true, first1 = true;
+        int pvl0 = 0, pvl1 = 0;                // P.V still to issue per V stage before it is released
+        // issues the owed P.V of stream B (waits for its P), releases the V stage after its last reader
+#define AL_ISSUE_PV(B, pend, first, cb, oe)                                                                  \
+        do {                                                                                                 \
+          const int j_ = pend;                                                                               \
+          const uint32_t it_ = kv_it + j_;                                                                   \
+          const int s_ = it_ % kStagesV;                                                                     \
+          TRACE_TILE(8 + B, it_);                                                                            \
+          mbar_wait(&sm.p_full[B], cb & 1);                                                                  \
+          TRACE_TILE(10 + B, it_);                                                                           \
+          mbar_wait(&sm.v_full[s_], (it_ / kStagesV) & 1);                                                   \
+          /* O_b of the stream's previous piece has been read out.  Only pieces in which the stream had   */ \
+          /* key tiles complete a phase of o_empty[b] (oe counts them), so neither side can run ahead.    */ \
+          if (first && oe > 0) mbar_wait(&sm.o_empty[B], (oe - 1) & 1);                                      \
+          tc_fence_after();                                                                                  \
+          /* keys of this tile that any row may see, rounded up to the MMA K step */                         \
+          const int kt_ = w.kt_begin + j_;                                                                   \
+          const int valid_ = kt_ < w.T.n_pref_tiles ? min(kBN, w.T.kv_len_max - kt_ * kBN)                   \
+                                                    : min(kBN, w.T.lk1 - w.T.lk0 - (kt_ - w.T.n_pref_tiles) * kBN); \
+          const int ksteps_ = (valid_ + 15) >> 4;                                                            \
+          const uint64_t dv_ = s_ ? dv[1] : dv[0];                                                           \
+          _Pragma("unroll")                                                                                  \
+          for (int k = 0; k < 8; ++k)                                                                        \
+            if (k < ksteps_) mma_ts(t_o[B], t_s[B] + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+          if (s_) { if (--pvl1 == 0) mma_commit(&sm.v_empty[1]); }                                           \
+          else { if (--pvl0 == 0) mma_commit(&sm.v_empty[0]); }                                              \
+          mma_commit(&sm.pv_done[B]);                                                                        \
+          TRACE_TILE(3 + 4 * B, it_);                                                                        \
+          first = false; pend = -1; ++cb;                                                                    \
+        } while (0)
         for (int i = 0; i < n; ++i) {
           const uint32_t it = kv_it + i;
-          const int sk = it % kStagesK;
+          const int sk = it % kStagesK, sv = it % kStagesV;
           const int kt = w.kt_begin + i;
-          const bool part[2] = {takes_part(T, p.tpt, 0, kt), takes_part(T, p.tpt, 1, kt)};
-          pv_left[it % kStagesV] = (int)part[0] + (int)part[1];
-          bool k_ready = false;
+          const bool part0 = takes_part(w.T, p.tpt, 0, kt), part1 = takes_part(w.T, p.tpt, 1, kt);
+          if (sv) pvl1 = (int)part0 + (int)part1; else pvl0 = (int)part0 + (int)part1;
+          const uint64_t dk0 = sk ? dk[1][0] : dk[0][0], dk1 = sk ? dk[1][1] : dk[0][1];
+          // per stream: the owed P.V first (it frees S_b, which P aliases, for the stream's next
+          // Q.K^T; no P.V is ever owed for more than one step, a V stage being reused two steps later)
+          if (pend0 >= 0) AL_ISSUE_PV(0, pend0, first0, cb0, oe0);
+          mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
+          tc_fence_after();
+          TRACE(4);
+          if (part0) {
 #pragma unroll
-          for (int b = 0; b < 2; ++b) {
-            // the owed P.V first: it frees S_b (P aliases it) for the stream's next Q.K^T, and no P.V is
-            // ever owed for more than one step (a V stage is reused two steps later)
-            if (pend[b] >= 0) issue_pv(b);
-            if (!part[b]) continue;
-            if (!k_ready) { mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1); tc_fence_after(); TRACE(4); k_ready = true; }
+            for (int k = 0; k < 4; ++k) mma_ss(t_s[0], dq[0][0] + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const uint64_t da = make_desc_sw128(smem_u32(sm.q[b][h]) + k * 32, 16, 1024);
-                const uint64_t db = make_desc_sw128(smem_u32(sm.k[sk][h]) + k * 32, 16, 1024);
-                mma_ss(t_s[b], da, db, idesc_qk, (h | k) ? 1u : 0u);
-              }
-            mma_commit(&sm.s_full[b]);
-            if (b == 0) TRACE_TILE(0, it);
-            pend[b] = i;
+            for (int k = 0; k < 4; ++k) mma_ss(t_s[0], dq[0][1] + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+            mma_commit(&sm.s_full[0]);
+            TRACE_TILE(0, it);
+            pend0 = i;
           }
-          if (!k_ready) { mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1); }   // a step no sub-tile takes part in
+          if (pend1 >= 0) AL_ISSUE_PV(1, pend1, first1, cb1, oe1);
+          if (part1) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) mma_ss(t_s[1], dq[1][0] + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) mma_ss(t_s[1], dq[1][1] + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+            mma_commit(&sm.s_full[1]);
+            TRACE_TILE(4, it);
+            pend1 = i;
+          }
           mma_commit(&sm.k_empty[sk]);
-          if (pv_left[it % kStagesV] == 0) {   // nobody reads this V tile: hand the stage back once it has landed
-            mbar_wait(&sm.v_full[it % kStagesV], (it / kStagesV) & 1);
-            mma_commit(&sm.v_empty[it % kStagesV]);
+          if (!part0 && !part1) {              // nobody reads this V tile: hand the stage back once it has landed
+            mbar_wait(&sm.v_full[sv], (it / kStagesV) & 1);
+            mma_commit(&sm.v_empty[sv]);
           }
           if (i == n - 1) mma_commit(&sm.q_empty);
         }
         // owed P.V of the last steps, older step first
-        if (pend[0] >= 0 && pend[1] >= 0) {
-          if (pend[0] <= pend[1]) { issue_pv(0); issue_pv(1); } else { issue_pv(1); issue_pv(0); }
-        } else if (pend[0] >= 0) issue_pv(0);
-        else if (pend[1] >= 0) issue_pv(1);
+        if (pend0 >= 0 && (pend1 < 0 || pend0 <= pend1)) AL_ISSUE_PV(0, pend0, first0, cb0, oe0);
+        if (pend1 >= 0) AL_ISSUE_PV(1, pend1, first1, cb1, oe1);
+        if (pend0 >= 0) AL_ISSUE_PV(0, pend0, first0, cb0, oe0);
+#undef AL_ISSUE_PV
         TRACE(5);
         kv_it += n;
-        if (!first_pv[0]) ++oe[0];
-        if (!first_pv[1]) ++oe[1];
+        if (!first0) ++oe0;
+        if (!first1) ++oe1;
         ++piece_it;
       }
     }
@@ -639,7 +660,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     uint8_t* stage_b = sm.stage + b * kBM * kStagePitch;
     uint8_t* my_stage = stage_b + r * kStagePitch;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
-    PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+    PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
     while (w.next()) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
@@ -664,7 +685,8 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         if (!takes_part(T, p.tpt, b, kt)) continue;
         mbar_wait(&sm.s_full[b], cnt & 1);
         tc_fence_after();
-        if (tid128 == 0 && b == 0) { TRACE(6); TRACE_TILE(1, cnt); }
+        if (tid128 == 0 && b == 0) TRACE(6);
+        if (tid128 == 0) TRACE_TILE(1 + 4 * b, cnt);
         float s[kBN];
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32_f(t_s[b] + lane_addr + c * 32, s + c * 32);
@@ -736,7 +758,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(&sm.p_full[b]);
-        if (tid128 == 0 && b == 0) TRACE_TILE(2, cnt);
+        if (tid128 == 0) TRACE_TILE(2 + 4 * b, cnt);
         ++cnt; ++n_mine;
       }
       // ---- epilogue: normalise, stage 128-byte half rows in shared memory, store coalesced ----
