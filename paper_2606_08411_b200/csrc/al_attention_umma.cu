@@ -352,7 +352,11 @@ __device__ unsigned long long g_trace[kMaxCtas * 16];
 // CTA 0 only: per step (first 32 of the CTA) stamps of kind k: 0 QK_A issued, 1 S seen by stream A, 2 P_A ready, 3 PV_A issued
 __device__ unsigned long long g_trace_tile[12 * 32];
 #define TRACE_TILE(k, i) do { if (blockIdx.x == 0 && (i) < 32) g_trace_tile[(k) * 32 + (i)] = clock64(); } while (0)
+// CTA 0, step 4 of each stream: per warp (8 softmax warps) stamps 0 S seen, 1 S in registers, 2 max done, 3 P stored, 4 arrived
+__device__ unsigned long long g_trace_warp[8 * 8];
+#define TRACE_W(k) do { if (blockIdx.x == 0 && cnt == 4 && lane == 0) g_trace_warp[(warp - 4) * 8 + (k)] = clock64(); } while (0)
 #else
+#define TRACE_W(k) do { } while (0)
 #define TRACE(i) do { } while (0)
 #define TRACE_TILE(k, i) do { } while (0)
 #endif
@@ -687,25 +691,37 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         tc_fence_after();
         if (tid128 == 0 && b == 0) TRACE(6);
         if (tid128 == 0) TRACE_TILE(1 + 4 * b, cnt);
+        TRACE_W(0);
         float s[kBN];
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32_f(t_s[b] + lane_addr + c * 32, s + c * 32);
         tmem_wait_ld();
-        // visible columns of this tile for this row: [lo, hi)
-        int lo = 0, hi = 0;
-        bool need_mask;
+        TRACE_W(1);
+        // visible columns of this tile for this row: [lo, hi).  Rows beyond the sub-tile's last token are
+        // never stored: they run unmasked on whatever their Q row holds.
+        int lo = 0, hi = kBN;
         if (kt < T.n_pref_tiles) {
           hi = min(kBN, prefix_len - kt * kBN);
-          need_mask = (kt + 1) * kBN > T.kv_len_min || !valid;
         } else {
           const int base = T.lk0 + (kt - T.n_pref_tiles) * kBN;
           lo = max(0, ls - base); hi = min(kBN, le - base);
-          need_mask = true;
         }
-        if (!valid) { lo = 0; hi = 0; }
+        const bool need_mask = valid && (lo > 0 || hi < kBN);
+        uint32_t hidden = 0;                             // bit c: 32-column chunk c is entirely hidden from this row
         if (need_mask) {
 #pragma unroll
-          for (int c = 0; c < kBN; ++c) s[c] = (c >= lo && c < hi) ? s[c] : -INFINITY;
+          for (int c4 = 0; c4 < 4; ++c4) {
+            const int c0 = c4 * 32;
+            if (lo <= c0 && hi >= c0 + 32) continue;     // entirely visible
+            if (hi <= c0 || lo >= c0 + 32) {
+              hidden |= 1u << c4;
+#pragma unroll
+              for (int e = 0; e < 32; ++e) s[c0 + e] = -INFINITY;
+            } else {
+#pragma unroll
+              for (int e = 0; e < 32; ++e) s[c0 + e] = (c0 + e >= lo && c0 + e < hi) ? s[c0 + e] : -INFINITY;
+            }
+          }
         }
         float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
 #pragma unroll
@@ -714,9 +730,10 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         }
         const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
         const float m_new = fmaxf(m_used, mx);
+        TRACE_W(2);
         bool grow = false;
         if (m_used == -INFINITY) m_used = m_new;         // nothing accumulated yet (O row is 0 or unwritten)
-        else grow = (m_new - m_used) * p.scale_log2 > kRescaleThreshold;
+        else grow = valid && (m_new - m_used) * p.scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, grow)) {             // warp-uniform: tcgen05.ld/st are .sync.aligned
           // rare: O of this stream must be rescaled, so its previous P.V has to have landed (it has:
           // the commit behind s_full covers every MMA issued before this tile's Q.K^T; the wait
@@ -742,22 +759,29 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t pk[16];
+          if (hidden & (1u << c)) {                      // P = 0 without touching the MUFU
 #pragma unroll
-          for (int e = 0; e < 16; ++e) {
-            float t0, t1;
-            unpack2(ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2), t0, t1);
-            const float p0 = ex2(t0), p1 = ex2(t1);
-            if (e & 1) sum_b = fadd2(sum_b, pack2(p0, p1)); else sum_a = fadd2(sum_a, pack2(p0, p1));
-            pk[e] = pack_bf16x2(p0, p1);
+            for (int e = 0; e < 16; ++e) pk[e] = 0u;
+          } else {
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+              float t0, t1;
+              unpack2(ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2), t0, t1);
+              const float p0 = ex2(t0), p1 = ex2(t1);
+              if (e & 1) sum_b = fadd2(sum_b, pack2(p0, p1)); else sum_a = fadd2(sum_a, pack2(p0, p1));
+              pk[e] = pack_bf16x2(p0, p1);
+            }
           }
           tmem_st16(t_s[b] + lane_addr + c * 16, pk);
         }
         float l0, l1;
         unpack2(fadd2(sum_a, sum_b), l0, l1);
         l_sum += l0 + l1;
+        TRACE_W(3);
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(&sm.p_full[b]);
+        TRACE_W(4);
         if (tid128 == 0) TRACE_TILE(2 + 4 * b, cnt);
         ++cnt; ++n_mine;
       }
@@ -849,6 +873,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 }
 #ifdef AL_ATTN_TRACE
 int trace_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace)); }
+int trace_warp_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_warp, sizeof(g_trace_warp)); }
 int trace_tile_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_tile, sizeof(g_trace_tile)); }
 #endif
 
@@ -989,6 +1014,7 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
 
 #ifdef AL_ATTN_TRACE
 extern "C" int al_debug_attn_trace(unsigned long long* host_out) { return trace_read(host_out); }   // [kMaxCtas * 16]
+extern "C" int al_debug_attn_trace_warp(unsigned long long* host_out) { return trace_warp_read(host_out); }   // [8 * 8]
 extern "C" int al_debug_attn_trace_tile(unsigned long long* host_out) { return trace_tile_read(host_out); }   // [4 * 32]
 extern "C" int al_debug_mbar_timeout(unsigned int* host_out) {   // [4]; [0] != 0 when a wait timed out
   return (int)cudaMemcpyFromSymbol(host_out, alptx::g_mbar_timeout, 16);
