@@ -389,6 +389,26 @@ __device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
   return d;
 }
 
+// 2^x for a pair on the FMA pipes (the MUFU does 16 ex2 per clock and SM -- exactly the rate at which
+// the tensor core produces scores, so half of the exponentials are taken off it): x = n + f with
+// n = rint(x), f in [-0.5, 0.5]; 2^f by a degree-3 polynomial (relative error 7.5e-5, far below the bf16
+// rounding of P); 2^n by adding n to the exponent field.  x is clamped at -126 (masked scores are -inf).
+__device__ __forceinline__ void exp2_poly_pair(uint64_t x2, float& p0, float& p1) {
+  float x0, x1;
+  unpack2(x2, x0, x1);
+  x2 = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+  const uint64_t t2 = fadd2(x2, pack2(12582912.f, 12582912.f));            // 1.5 * 2^23: n lands in the low mantissa bits
+  const uint64_t f2 = ffma2(fadd2(t2, pack2(-12582912.f, -12582912.f)), pack2(-1.f, -1.f), x2);
+  uint64_t q2 = ffma2(pack2(0.055171460f, 0.055171460f), f2, pack2(0.24261086f, 0.24261086f));
+  q2 = ffma2(q2, f2, pack2(0.69326097f, 0.69326097f));
+  q2 = ffma2(q2, f2, pack2(0.99992812f, 0.99992812f));
+  float q0, q1, t0, t1;
+  unpack2(q2, q0, q1);
+  unpack2(t2, t0, t1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
+}
+
 // global row (token-major [T][H_q][d]) of stacked row r of sub-tile b
 __device__ __forceinline__ long long out_row(const AttnParams& p, const TileRec& T, int g, int b, int r) {
   const int tl = r / p.n_rep;
@@ -765,9 +785,15 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           } else {
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
-              float t0, t1;
-              unpack2(ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2), t0, t1);
-              const float p0 = ex2(t0), p1 = ex2(t1);
+              const uint64_t x2 = ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2);
+              float p0, p1;
+              if (e & 1) {
+                exp2_poly_pair(x2, p0, p1);
+              } else {
+                float t0, t1;
+                unpack2(x2, t0, t1);
+                p0 = ex2(t0); p1 = ex2(t1);
+              }
               if (e & 1) sum_b = fadd2(sum_b, pack2(p0, p1)); else sum_a = fadd2(sum_a, pack2(p0, p1));
               pk[e] = pack_bf16x2(p0, p1);
             }
