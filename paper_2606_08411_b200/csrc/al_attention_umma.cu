@@ -477,18 +477,22 @@ __device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T
 }
 
 // Copies the staged 128-byte half rows [0, n_rows) of stream b to global memory with coalesced
-// 8-byte accesses: 16 lanes per half row, two half rows per warp instruction.  `dst_of(r)` is the
-// global address of half row r.
-template <typename RowPtr>
-__device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, int n_rows, int tid128, RowPtr dst_of) {
+// 8-byte accesses: 16 lanes per half row, two half rows per warp instruction.  Half row r goes to
+// base + (r / rows_per_tok) * tok_stride + (r % rows_per_tok) * row_stride  (bytes); the quotient and
+// remainder are carried along instead of being recomputed for each of a thread's 16 rows.
+__device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, int n_rows, int tid128, uint8_t* base,
+                                              int rows_per_tok, long long tok_stride, int row_stride) {
   const int warp = tid128 >> 5, lane = tid128 & 31;
   const int sub = lane >> 4, chunk = lane & 15;
+  int r = warp * 32 + sub;
+  int q = r / rows_per_tok, m = r - q * rows_per_tok;
 #pragma unroll 4
   for (int it = 0; it < 16; ++it) {
-    const int r = warp * 32 + it * 2 + sub;
     if (r < n_rows)
-      *reinterpret_cast<uint2*>(dst_of(r) + chunk * 8) =
+      *reinterpret_cast<uint2*>(base + q * tok_stride + m * row_stride + chunk * 8) =
           *reinterpret_cast<const uint2*>(stage_b + r * kStagePitch + chunk * 8);
+    r += 2; m += 2;
+    while (m >= rows_per_tok) { m -= rows_per_tok; ++q; }
   }
 }
 
@@ -510,9 +514,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #endif
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) __trap();          // the 128-byte swizzle atoms need 1024-byte alignment
-    mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 1);
-    for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 1); }
-    for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 1); }
+    mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 2);       // the *_empty barriers collect both MMA issuers
+    for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 2); }
+    for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 2); }
     for (int b = 0; b < 2; ++b) {
       mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_empty[b], 128);
     }
@@ -564,111 +568,88 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         }
         ++piece_it;
       }
-    } else if (warp == 1 && lane == 0 && active) {
-      // ===================== MMA issuer =====================
-      // every descriptor is a constant plus a small address offset: build the bases once
+    } else if ((warp == 1 || warp == 2) && lane == 0 && active) {
+      // ===================== MMA issuers: warp 1 for stream A, warp 2 for stream B =====================
+      // Per stream the order is: the owed P.V of the previous key tile (it frees S_b, which P aliases),
+      // then Q.K^T of the next.  Two issuing threads keep one stream's wait for its softmax from
+      // holding up the other stream's MMAs; both arrive on the K/V/Q stage barriers (count 2).
+      const int b = warp - 1;
+      const uint32_t ts = tmem + b * 128, to = tmem + 256 + b * 128;
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
       const uint32_t idesc_pv = make_idesc_bf16(kBM, kD, 0, 1);
-      uint64_t dq[2][2], dk[kStagesK][2], dv[kStagesV];
-#pragma unroll
-      for (int b = 0; b < 2; ++b)
-#pragma unroll
-        for (int h = 0; h < 2; ++h) dq[b][h] = make_desc_sw128(smem_u32(sm.q[b][h]), 16, 1024);
-#pragma unroll
-      for (int s = 0; s < kStagesK; ++s)
-#pragma unroll
-        for (int h = 0; h < 2; ++h) dk[s][h] = make_desc_sw128(smem_u32(sm.k[s][h]), 16, 1024);
-#pragma unroll
-      for (int s = 0; s < kStagesV; ++s) dv[s] = make_desc_sw128(smem_u32(sm.v[s][0]), kHalfBytes, 1024);
+      // every descriptor is a constant plus a small address offset: build the bases once
+      const uint64_t dq0 = make_desc_sw128(smem_u32(sm.q[b][0]), 16, 1024);
+      const uint64_t dq1 = make_desc_sw128(smem_u32(sm.q[b][1]), 16, 1024);
+      const uint64_t dk00 = make_desc_sw128(smem_u32(sm.k[0][0]), 16, 1024), dk01 = make_desc_sw128(smem_u32(sm.k[0][1]), 16, 1024);
+      const uint64_t dk10 = make_desc_sw128(smem_u32(sm.k[1][0]), 16, 1024), dk11 = make_desc_sw128(smem_u32(sm.k[1][1]), 16, 1024);
+      const uint64_t dv0 = make_desc_sw128(smem_u32(sm.v[0][0]), kHalfBytes, 1024);
+      const uint64_t dv1 = make_desc_sw128(smem_u32(sm.v[1][0]), kHalfBytes, 1024);
+      static_assert(kStagesK == 2 && kStagesV == 2, "the issuers select stage descriptors with a two-way choice");
       uint32_t kv_it = 0, piece_it = 0;
-      uint32_t cb0 = 0, cb1 = 0;               // P.V issued so far per stream (all pieces): p_full phase
-      uint32_t oe0 = 0, oe1 = 0;               // pieces so far in which the stream had key tiles: o_empty phase
+      uint32_t cb = 0;                         // P.V issued so far (all pieces): p_full phase
+      uint32_t oe = 0;                         // pieces so far in which the stream had key tiles: o_empty phase
       PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
-        TRACE(3);
-        int pend0 = -1, pend1 = -1;            // step of the piece whose P.V the stream still owes
-        bool first0 = true, first1 = true;
-        int pvl0 = 0, pvl1 = 0;                // P.V still to issue per V stage before it is released
-        // issues the owed P.V of stream B (waits for its P), releases the V stage after its last reader
-#define AL_ISSUE_PV(B, pend, first, cb, oe)                                                                  \
-        do {                                                                                                 \
-          const int j_ = pend;                                                                               \
-          const uint32_t it_ = kv_it + j_;                                                                   \
-          const int s_ = it_ % kStagesV;                                                                     \
-          TRACE_TILE(8 + B, it_);                                                                            \
-          mbar_wait(&sm.p_full[B], cb & 1);                                                                  \
-          TRACE_TILE(10 + B, it_);                                                                           \
-          mbar_wait(&sm.v_full[s_], (it_ / kStagesV) & 1);                                                   \
-          /* O_b of the stream's previous piece has been read out.  Only pieces in which the stream had   */ \
-          /* key tiles complete a phase of o_empty[b] (oe counts them), so neither side can run ahead.    */ \
-          if (first && oe > 0) mbar_wait(&sm.o_empty[B], (oe - 1) & 1);                                      \
-          tc_fence_after();                                                                                  \
-          /* keys of this tile that any row may see, rounded up to the MMA K step */                         \
-          const int kt_ = w.kt_begin + j_;                                                                   \
-          const int valid_ = kt_ < w.T.n_pref_tiles ? min(kBN, w.T.kv_len_max - kt_ * kBN)                   \
-                                                    : min(kBN, w.T.lk1 - w.T.lk0 - (kt_ - w.T.n_pref_tiles) * kBN); \
-          const int ksteps_ = (valid_ + 15) >> 4;                                                            \
-          const uint64_t dv_ = s_ ? dv[1] : dv[0];                                                           \
-          _Pragma("unroll")                                                                                  \
-          for (int k = 0; k < 8; ++k)                                                                        \
-            if (k < ksteps_) mma_ts(t_o[B], t_s[B] + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
-          if (s_) { if (--pvl1 == 0) mma_commit(&sm.v_empty[1]); }                                           \
-          else { if (--pvl0 == 0) mma_commit(&sm.v_empty[0]); }                                              \
-          mma_commit(&sm.pv_done[B]);                                                                        \
-          TRACE_TILE(3 + 4 * B, it_);                                                                        \
-          first = false; pend = -1; ++cb;                                                                    \
-        } while (0)
-        for (int i = 0; i < n; ++i) {
+        if (b == 0) TRACE(3);
+        int pend = -1;                         // step of the piece whose P.V is still owed
+        bool first = true;
+        for (int i = 0; i <= n; ++i) {
+          if (pend >= 0) {                     // ---- O_b (+)= P_b . V of step `pend`
+            const uint32_t it = kv_it + pend;
+            const int sv = it % kStagesV;
+            TRACE_TILE(8 + b, it);
+            mbar_wait(&sm.p_full[b], cb & 1);
+            TRACE_TILE(10 + b, it);
+            mbar_wait(&sm.v_full[sv], (it / kStagesV) & 1);
+            // O_b of the stream's previous piece has been read out.  Only pieces in which the stream had
+            // key tiles complete a phase of o_empty[b] (oe counts them), so neither side can run ahead.
+            if (first && oe > 0) mbar_wait(&sm.o_empty[b], (oe - 1) & 1);
+            tc_fence_after();
+            // keys of this tile that any row may see, rounded up to the MMA K step
+            const int kt = w.kt_begin + pend;
+            const int valid = kt < w.T.n_pref_tiles ? min(kBN, w.T.kv_len_max - kt * kBN)
+                                                    : min(kBN, w.T.lk1 - w.T.lk0 - (kt - w.T.n_pref_tiles) * kBN);
+            const int ksteps = (valid + 15) >> 4;
+            const uint64_t dv = sv ? dv1 : dv0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+              if (k < ksteps) mma_ts(to, ts + k * 8, dv + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u);
+            mma_commit(&sm.v_empty[sv]);
+            TRACE_TILE(3 + 4 * b, it);
+            first = false; pend = -1; ++cb;
+          }
+          if (i == n) break;
           const uint32_t it = kv_it + i;
           const int sk = it % kStagesK, sv = it % kStagesV;
-          const int kt = w.kt_begin + i;
-          const bool part0 = takes_part(w.T, p.tpt, 0, kt), part1 = takes_part(w.T, p.tpt, 1, kt);
-          if (sv) pvl1 = (int)part0 + (int)part1; else pvl0 = (int)part0 + (int)part1;
-          const uint64_t dk0 = sk ? dk[1][0] : dk[0][0], dk1 = sk ? dk[1][1] : dk[0][1];
-          // per stream: the owed P.V first (it frees S_b, which P aliases, for the stream's next
-          // Q.K^T; no P.V is ever owed for more than one step, a V stage being reused two steps later)
-          if (pend0 >= 0) AL_ISSUE_PV(0, pend0, first0, cb0, oe0);
           mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
-          tc_fence_after();
-          TRACE(4);
-          if (part0) {
+          if (takes_part(w.T, p.tpt, b, w.kt_begin + i)) {   // ---- S_b = Q_b . K^T of step i
+            tc_fence_after();
+            if (b == 0) TRACE(4);
+            const uint64_t dk0 = sk ? dk10 : dk00, dk1 = sk ? dk11 : dk01;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(t_s[0], dq[0][0] + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+            for (int k = 0; k < 4; ++k) mma_ss(ts, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(t_s[0], dq[0][1] + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
-            mma_commit(&sm.s_full[0]);
-            TRACE_TILE(0, it);
-            pend0 = i;
-          }
-          if (pend1 >= 0) AL_ISSUE_PV(1, pend1, first1, cb1, oe1);
-          if (part1) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(t_s[1], dq[1][0] + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(t_s[1], dq[1][1] + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
-            mma_commit(&sm.s_full[1]);
-            TRACE_TILE(4, it);
-            pend1 = i;
-          }
-          mma_commit(&sm.k_empty[sk]);
-          if (!part0 && !part1) {              // nobody reads this V tile: hand the stage back once it has landed
+            for (int k = 0; k < 4; ++k) mma_ss(ts, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+            mma_commit(&sm.s_full[b]);
+            TRACE_TILE(4 * b, it);
+            pend = i;
+            mma_commit(&sm.k_empty[sk]);
+          } else {
+            // not this stream's step: hand both stages back, but only once they have landed, so that
+            // this thread can never be two stage phases ahead of the other issuer
+            mma_commit(&sm.k_empty[sk]);
             mbar_wait(&sm.v_full[sv], (it / kStagesV) & 1);
             mma_commit(&sm.v_empty[sv]);
           }
           if (i == n - 1) mma_commit(&sm.q_empty);
         }
-        // owed P.V of the last steps, older step first
-        if (pend0 >= 0 && (pend1 < 0 || pend0 <= pend1)) AL_ISSUE_PV(0, pend0, first0, cb0, oe0);
-        if (pend1 >= 0) AL_ISSUE_PV(1, pend1, first1, cb1, oe1);
-        if (pend0 >= 0) AL_ISSUE_PV(0, pend0, first0, cb0, oe0);
-#undef AL_ISSUE_PV
-        TRACE(5);
+        if (!first) mma_commit(&sm.pv_done[b]);              // only the epilogue waits for the accumulator
+        if (b == 0) TRACE(5);
         kv_it += n;
-        if (!first0) ++oe0;
-        if (!first1) ++oe1;
+        if (!first) ++oe;
         ++piece_it;
       }
     }
@@ -684,6 +665,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     uint8_t* stage_b = sm.stage + b * kBM * kStagePitch;
     uint8_t* my_stage = stage_b + r * kStagePitch;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
+    uint32_t pieces_done = 0;                          // pieces in which it had key tiles: pv_done phase
     PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
     while (w.next()) {
       const TileRec& T = w.T;
@@ -728,20 +710,18 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         }
         const bool need_mask = valid && (lo > 0 || hi < kBN);
         uint32_t hidden = 0;                             // bit c: 32-column chunk c is entirely hidden from this row
-        if (need_mask) {
+        if (__any_sync(0xffffffffu, need_mask)) {        // warp-uniform: only ragged prefix tails and local tiles
+          uint32_t vis[4];                               // bit e of vis[c]: column 32 c + e is visible
 #pragma unroll
           for (int c4 = 0; c4 < 4; ++c4) {
-            const int c0 = c4 * 32;
-            if (lo <= c0 && hi >= c0 + 32) continue;     // entirely visible
-            if (hi <= c0 || lo >= c0 + 32) {
-              hidden |= 1u << c4;
-#pragma unroll
-              for (int e = 0; e < 32; ++e) s[c0 + e] = -INFINITY;
-            } else {
-#pragma unroll
-              for (int e = 0; e < 32; ++e) s[c0 + e] = (c0 + e >= lo && c0 + e < hi) ? s[c0 + e] : -INFINITY;
-            }
+            const int a = min(32, max(0, lo - c4 * 32)), z = min(32, max(0, hi - c4 * 32));   // visible [a, z) of the chunk
+            const uint32_t below_z = z >= 32 ? 0xffffffffu : ((1u << z) - 1u);
+            const uint32_t below_a = a >= 32 ? 0xffffffffu : ((1u << a) - 1u);
+            vis[c4] = need_mask ? (below_z & ~below_a) : 0xffffffffu;
+            if (vis[c4] == 0u) hidden |= 1u << c4;
           }
+#pragma unroll
+          for (int c = 0; c < kBN; ++c) s[c] = (vis[c >> 5] >> (c & 31)) & 1u ? s[c] : -INFINITY;
         }
         float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
 #pragma unroll
@@ -755,10 +735,8 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         if (m_used == -INFINITY) m_used = m_new;         // nothing accumulated yet (O row is 0 or unwritten)
         else grow = valid && (m_new - m_used) * p.scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, grow)) {             // warp-uniform: tcgen05.ld/st are .sync.aligned
-          // rare: O of this stream must be rescaled, so its previous P.V has to have landed (it has:
-          // the commit behind s_full covers every MMA issued before this tile's Q.K^T; the wait
-          // states the dependency and costs nothing)
-          if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
+          // rare: O of this stream must be rescaled.  Its previous P.V has landed: the commit behind
+          // s_full covers every MMA the issuer sent before this tile's Q.K^T.
           const float alpha = grow ? ex2((m_used - m_new) * p.scale_log2) : 1.0f;
           if (grow) { l_sum *= alpha; m_used = m_new; }
           if (n_mine > 0) {
@@ -787,7 +765,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
             for (int e = 0; e < 16; ++e) {
               const uint64_t x2 = ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2);
               float p0, p1;
-              if (e & 1) {
+              if ((e & 3) == 1) {                         // every fourth pair: FMA pipes instead of the MUFU
                 exp2_poly_pair(x2, p0, p1);
               } else {
                 float t0, t1;
@@ -813,7 +791,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       }
       // ---- epilogue: normalise, stage 128-byte half rows in shared memory, store coalesced ----
       if (tid128 == 0 && b == 0) TRACE(7);
-      if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
+      if (n_mine > 0) { mbar_wait(&sm.pv_done[b], pieces_done & 1); tc_fence_after(); ++pieces_done; }
       if (tid128 == 0 && b == 0) TRACE(8);
       const float inv = l_sum > 0.f ? 1.0f / l_sum : 0.f;
       const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
@@ -838,9 +816,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
                                   pack_bf16x2(o[4 * e + 2] * inv, o[4 * e + 3] * inv));
           }
           bar_sync_stream(b);
-          copy_out_rows(stage_b, n_rows, tid128, [&](int rr) {
-            return reinterpret_cast<uint8_t*>(p.out + out_row(p, T, w.g, b, rr) * kD) + rd * 128;
-          });
+          copy_out_rows(stage_b, n_rows, tid128,
+                        reinterpret_cast<uint8_t*>(p.out + out_row(p, T, w.g, b, 0) * kD) + rd * 128, p.n_rep,
+                        (long long)p.n_q_heads * kD * 2, kD * 2);
           bar_sync_stream(b);                          // the staging rows are rewritten by the next round / piece
         }
         if (valid && p.lse) p.lse[out_row(p, T, w.g, b, r)] = lse;
@@ -857,9 +835,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #pragma unroll
           for (int e = 0; e < 16; ++e) dst[e] = make_uint2(__float_as_uint(o[2 * e] * inv), __float_as_uint(o[2 * e + 1] * inv));
           bar_sync_stream(b);
-          copy_out_rows(stage_b, n_rows, tid128, [&](int rr) {
-            return reinterpret_cast<uint8_t*>(prow0 + (long long)rr * kD) + rd * 128;
-          });
+          copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + rd * 128, kBM, 0, kD * 4);
           bar_sync_stream(b);
         }
       }
