@@ -142,6 +142,84 @@ def test_attention_full_size_sampled_outputs_cfg4_one_layer(handle):
     assert worst <= 1e-2, worst
 
 
+def sampled_rows_check(wl, out, lse, n_samples, seed, layers=None):
+    """Compares sampled (layer, lane, row, head) outputs with the oracle's one-row entry point."""
+    rng = np.random.default_rng(seed)
+    worst = 0.0
+    for _ in range(n_samples):
+        layer = int(rng.integers(0, wl.n_layers)) if layers is None else int(rng.choice(layers))
+        li = int(rng.integers(0, wl.n_lanes))
+        lane = wl.lanes[li]; r = int(rng.integers(0, lane[W.LANE_Q_LEN])); h = int(rng.integers(0, wl.n_q_heads))
+        ref, ref_lse = oracle.lane_attention_one(wl.q[layer], wl.k_new[layer], wl.v_new[layer], wl.k_cache[layer],
+                                                 wl.v_cache[layer], lane, r, h)
+        row = int(lane[W.LANE_Q_START]) + r
+        worst = max(worst, np.abs(out[layer, row, h] - ref).max() / np.abs(ref).max())
+        if lse is not None:
+            assert abs(lse[layer, row, h] - ref_lse) <= 1e-3
+    return worst
+
+
+def test_attention_full_size_sampled_outputs_cfg5_bench_configuration(handle):
+    """BASELINE configs[4] at full size (16 sequences, seeded lane trees, GQA 28/4), launched exactly as
+    bench.py launches it (al_lane_plan once, then al_lane_attention_planned); sampled rows vs the oracle."""
+    wl = W.cfg5_throughput_batch()
+    st = make_step(handle, wl)
+    st.attention(); torch.cuda.synchronize()
+    out = to_np(st.out); lse = to_np(st.lse)
+    assert np.isfinite(out).all()
+    assert sampled_rows_check(wl, out, lse, 128, seed=5) <= 1e-2
+
+
+def test_attention_plan_is_reused_across_layers_and_calls(handle):
+    """al_lane_plan + al_lane_attention_planned == al_lane_attention, and a plan survives being used:
+    the second planned call on the same workspace (tickets reset by the merging CTAs) is bit-identical."""
+    wl = W.cfg4_long_llada(n_layers=2)
+    st = make_step(handle, wl)
+    for l in range(wl.n_layers):                               # fused entry point, layer by layer
+        handle.al_lane_attention(st.shape, st.q[l], st.k_new[l], st.v_new[l], st.k_cache[l], st.v_cache[l], st.lanes,
+                                 wl.n_lanes, st.T, st.max_prefix, st.out[l], st.lse[l], st.ws_attn)
+    torch.cuda.synchronize()
+    fused = st.out.clone()
+    st.out.zero_()
+    st.attention(); torch.cuda.synchronize()                   # one plan, two planned layers
+    assert torch.equal(st.out, fused)
+    st.out.zero_()
+    for l in range(wl.n_layers):                               # the plan is still valid: no al_lane_plan here
+        handle.al_lane_attention_planned(st.shape, st.q[l], st.k_new[l], st.v_new[l], st.k_cache[l], st.v_cache[l],
+                                         st.lanes, wl.n_lanes, st.T, st.max_prefix, st.out[l], st.lse[l], st.ws_attn)
+    torch.cuda.synchronize()
+    assert torch.equal(st.out, fused)
+
+
+def test_attention_one_item_split_over_many_ctas_long_prefix(handle):
+    """A single lane group with a 6000-row prefix and one kv-head: every CTA of the grid gets a piece of
+    the same two items, so the in-kernel merge combines dozens of partials (also: prefix not a multiple
+    of 128, lanes with different prefix lengths inside the tile)."""
+    groups = [dict(kv_base_row=5, prefix_len=[6000, 5990, 6000], q_lens=[32, 20, 32])]
+    wl = W.build_workload("long_prefix", 777, "bf16", 2, 1, 128, 1, 6100, groups, n_refresh=1, refresh_base_row=0,
+                          refresh_span=8, vocab=64, logit_sigma=1.0, planted_frac=0.0, mask_id=63, eos_id=-1,
+                          threshold=0.9)
+    check_attention(handle, wl, tol=1e-2, lse_tol=1e-3)
+
+
+def test_attention_many_lanes_limits(handle):
+    """300 single-token lanes in 100 groups run; more than the plan's 1024 lanes is AL_ERR_UNSUPPORTED."""
+    from paper_2606_08411_b200 import binding as B
+    groups = [dict(kv_base_row=3 * i, prefix_len=3 + (i % 5), q_lens=[1, 1, 1]) for i in range(100)]
+    wl = W.build_workload("many_lanes", 778, "bf16", 4, 2, 128, 1, 400, groups, n_refresh=1, refresh_base_row=0,
+                          refresh_span=8, vocab=64, logit_sigma=1.0, planted_frac=0.0, mask_id=63, eos_id=-1,
+                          threshold=0.9)
+    st = check_attention(handle, wl, tol=1e-2, lse_tol=1e-3)
+    n = 1025
+    lanes = torch.zeros((n, 6), dtype=torch.int32, device=st.lanes.device)
+    q = torch.zeros((n, 4, 128), dtype=torch.bfloat16, device=st.lanes.device)
+    kv = torch.zeros((n, 2, 128), dtype=torch.bfloat16, device=st.lanes.device)
+    ws = torch.empty(handle.al_lane_attention_workspace_bytes(st.shape, n, n, 8), dtype=torch.uint8, device=st.lanes.device)
+    with pytest.raises(B.AlError) as e:
+        handle.al_lane_attention(st.shape, q, kv, kv, st.k_cache[0], st.v_cache[0], lanes, n, n, 8, q.clone(), None, ws)
+    assert e.value.status == B.AL_ERR_UNSUPPORTED
+
+
 # ------------------------------------------------------------------------------------------------
 # refresh
 # ------------------------------------------------------------------------------------------------
