@@ -44,12 +44,13 @@ using namespace alptx;
 namespace {
 
 constexpr int kBM = 128;                   // stacked query rows per tile
-constexpr int kBN = 128;                   // keys per key tile
+constexpr int kBN = 64;                    // keys per key tile (step): S_b is 64 fp32 TMEM columns, double-buffered
 constexpr int kD = 128;                    // head_dim
-constexpr int kStagesK = 2;                // K ring depth (a K tile lives until its Q.K^T has run)
-constexpr int kStagesV = 2;                // V ring depth (a V tile lives until its P.V has run)
-constexpr int kHalfBytes = 128 * 64 * 2;   // [128 rows][64 bf16] = one 128-byte-swizzled half tile
-constexpr int kTileBytes = 2 * kHalfBytes;
+constexpr int kStagesK = 4;                // K ring depth (a K tile lives until its Q.K^T has run)
+constexpr int kStagesV = 4;                // V ring depth (a V tile lives until its P.V has run)
+constexpr int kHalfBytes = kBM * 64 * 2;   // Q: [128 rows][64 bf16] = one 128-byte-swizzled half tile
+constexpr int kKvHalfBytes = kBN * 64 * 2; // K, V: [64 keys][64 bf16]
+constexpr int kTileBytes = 2 * kKvHalfBytes;
 constexpr int kThreads = 384;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: P <= 2^8 between rescales
@@ -57,7 +58,7 @@ constexpr int kMaxPlanLanes = 1024;
 constexpr int kMaxPlanTiles = 2048;
 constexpr int kPlanThreads = 1024;
 constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
-constexpr int kMinPiece = 2;               // do not cut the work finer than 2 key-tile steps per CTA
+constexpr int kMinPiece = 4;               // do not cut the work finer than 4 key-tile steps (256 keys) per CTA
 
 struct __align__(16) TileRec {             // 64 bytes
   int q_tok0, n_tok;          // first packed token row, tokens in the tile (<= 2 tpt)
@@ -267,12 +268,14 @@ constexpr int kStagePitch = 136;           // 128 data bytes + 8 pad: conflict-f
 
 struct AttnSmem {
   alignas(1024) uint8_t q[2][2][kHalfBytes];           // [sub-tile][64-column half]
-  alignas(1024) uint8_t k[kStagesK][2][kHalfBytes];
-  alignas(1024) uint8_t v[kStagesV][2][kHalfBytes];
+  alignas(1024) uint8_t k[kStagesK][2][kKvHalfBytes];
+  alignas(1024) uint8_t v[kStagesV][2][kKvHalfBytes];
   alignas(16) uint8_t stage[2 * kBM * kStagePitch];    // epilogue staging: half row (stream b, row r) at b*128 + r
   uint64_t q_full, q_empty;
   uint64_t k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV];
-  uint64_t s_full[2], p_full[2], pv_done[2], o_empty[2];
+  uint64_t s_full[2][2], p_full[2][2];     // [stream][S buffer]
+  uint64_t pv_done[2];                     // per P.V: the lazy rescale of O waits for the stream's previous P.V
+  uint64_t o_full[2], o_empty[2];          // per piece: accumulator complete / read out
   uint32_t tmem_base;
   int ticket[2][3];
 };
@@ -361,9 +364,6 @@ __device__ unsigned long long g_trace_warp[8 * 8];
 #define TRACE_TILE(k, i) do { } while (0)
 #endif
 __device__ __forceinline__ void bar_sync_stream(int b) { asm volatile("bar.sync %0, 128;" ::"r"(1 + b) : "memory"); }
-__device__ __forceinline__ void mbar_arrive_n(uint64_t* bar, uint32_t n) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(n) : "memory");
-}
 __device__ __forceinline__ float ex2(float x) {             // x <= 8 here (or -inf)
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -518,7 +518,8 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 2); }
     for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 2); }
     for (int b = 0; b < 2; ++b) {
-      mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_empty[b], 128);
+      for (int u = 0; u < 2; ++u) { mbar_init(&sm.s_full[b][u], 1); mbar_init(&sm.p_full[b][u], 128); }
+      mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_full[b], 1); mbar_init(&sm.o_empty[b], 128);
     }
     fence_barrier_init();
     prefetch_tensormap(&map_q); prefetch_tensormap(&map_knew); prefetch_tensormap(&map_vnew);
@@ -529,8 +530,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
-  const uint32_t t_s[2] = {tmem, tmem + 128};
-  const uint32_t t_o[2] = {tmem + 256, tmem + 384};
+  // TMEM columns: S of stream b, buffer u at (2 b + u) * 64; O of stream b at 256 + 128 b
   const bool active = (int)blockIdx.x < p.plan.hdr->n_ctas;
   if (threadIdx.x == 0) TRACE(1);
 
@@ -570,9 +570,10 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       }
     } else if ((warp == 1 || warp == 2) && lane == 0 && active) {
       // ===================== MMA issuers: warp 1 for stream A, warp 2 for stream B =====================
-      // Per stream the order is: the owed P.V of the previous key tile (it frees S_b, which P aliases),
-      // then Q.K^T of the next.  Two issuing threads keep one stream's wait for its softmax from
-      // holding up the other stream's MMAs; both arrive on the K/V/Q stage barriers (count 2).
+      // Per stream S is double-buffered (2 x 64 TMEM columns; P aliases S), so Q.K^T runs two key tiles
+      // ahead of P.V: the order is QK(0) QK(1) PV(0) QK(2) PV(1) QK(3) ... and the softmax of tile i+1
+      // never waits for the MMAs of tile i.  Two issuing threads keep one stream's wait for its softmax
+      // from holding up the other stream's MMAs; both arrive on the K/V/Q stage barriers (count 2).
       const int b = warp - 1;
       const uint32_t ts = tmem + b * 128, to = tmem + 256 + b * 128;
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
@@ -580,13 +581,10 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       // every descriptor is a constant plus a small address offset: build the bases once
       const uint64_t dq0 = make_desc_sw128(smem_u32(sm.q[b][0]), 16, 1024);
       const uint64_t dq1 = make_desc_sw128(smem_u32(sm.q[b][1]), 16, 1024);
-      const uint64_t dk00 = make_desc_sw128(smem_u32(sm.k[0][0]), 16, 1024), dk01 = make_desc_sw128(smem_u32(sm.k[0][1]), 16, 1024);
-      const uint64_t dk10 = make_desc_sw128(smem_u32(sm.k[1][0]), 16, 1024), dk11 = make_desc_sw128(smem_u32(sm.k[1][1]), 16, 1024);
-      const uint64_t dv0 = make_desc_sw128(smem_u32(sm.v[0][0]), kHalfBytes, 1024);
-      const uint64_t dv1 = make_desc_sw128(smem_u32(sm.v[1][0]), kHalfBytes, 1024);
-      static_assert(kStagesK == 2 && kStagesV == 2, "the issuers select stage descriptors with a two-way choice");
+      const uint64_t dk = make_desc_sw128(smem_u32(sm.k[0][0]), 16, 1024);               // + stage * (16 KB >> 4) + half * (8 KB >> 4)
+      const uint64_t dv = make_desc_sw128(smem_u32(sm.v[0][0]), kKvHalfBytes, 1024);     // + stage * (16 KB >> 4)
       uint32_t kv_it = 0, piece_it = 0;
-      uint32_t cb = 0;                         // P.V issued so far (all pieces): p_full phase
+      uint32_t c_qk = 0, c_pv = 0;             // key tiles of this stream whose Q.K^T / P.V has been issued (all pieces)
       uint32_t oe = 0;                         // pieces so far in which the stream had key tiles: o_empty phase
       PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
@@ -594,59 +592,69 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
         if (b == 0) TRACE(3);
-        int pend = -1;                         // step of the piece whose P.V is still owed
+        int owed0 = 0, owed1 = 0;              // steps (of the piece) of the up to two key tiles whose P.V is owed, oldest first
         bool first = true;
-        for (int i = 0; i <= n; ++i) {
-          if (pend >= 0) {                     // ---- O_b (+)= P_b . V of step `pend`
-            const uint32_t it = kv_it + pend;
-            const int sv = it % kStagesV;
-            TRACE_TILE(8 + b, it);
-            mbar_wait(&sm.p_full[b], cb & 1);
-            TRACE_TILE(10 + b, it);
-            mbar_wait(&sm.v_full[sv], (it / kStagesV) & 1);
-            // O_b of the stream's previous piece has been read out.  Only pieces in which the stream had
-            // key tiles complete a phase of o_empty[b] (oe counts them), so neither side can run ahead.
-            if (first && oe > 0) mbar_wait(&sm.o_empty[b], (oe - 1) & 1);
-            tc_fence_after();
-            // keys of this tile that any row may see, rounded up to the MMA K step
-            const int kt = w.kt_begin + pend;
-            const int valid = kt < w.T.n_pref_tiles ? min(kBN, w.T.kv_len_max - kt * kBN)
-                                                    : min(kBN, w.T.lk1 - w.T.lk0 - (kt - w.T.n_pref_tiles) * kBN);
-            const int ksteps = (valid + 15) >> 4;
-            const uint64_t dv = sv ? dv1 : dv0;
-#pragma unroll
-            for (int k = 0; k < 8; ++k)
-              if (k < ksteps) mma_ts(to, ts + k * 8, dv + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u);
-            mma_commit(&sm.v_empty[sv]);
-            TRACE_TILE(3 + 4 * b, it);
-            first = false; pend = -1; ++cb;
-          }
-          if (i == n) break;
+        // O_b (+)= P . V of the oldest owed key tile
+#define AL_ISSUE_PV()                                                                                          \
+        do {                                                                                                   \
+          const uint32_t it_ = kv_it + owed0;                                                                  \
+          const int sv_ = it_ % kStagesV;                                                                      \
+          const uint32_t u_ = c_pv & 1;                                                                        \
+          TRACE_TILE(8 + b, it_);                                                                              \
+          mbar_wait(&sm.p_full[b][u_], (c_pv >> 1) & 1);                                                       \
+          TRACE_TILE(10 + b, it_);                                                                             \
+          mbar_wait(&sm.v_full[sv_], (it_ / kStagesV) & 1);                                                    \
+          /* O_b of the stream's previous piece has been read out.  Only pieces in which the stream had     */ \
+          /* key tiles complete a phase of o_empty[b] (oe counts them), so neither side can run ahead.      */ \
+          if (first && oe > 0) mbar_wait(&sm.o_empty[b], (oe - 1) & 1);                                        \
+          tc_fence_after();                                                                                    \
+          /* keys of this tile that any row may see, rounded up to the MMA K step */                           \
+          const int kt_ = w.kt_begin + owed0;                                                                  \
+          const int valid_ = kt_ < w.T.n_pref_tiles ? min(kBN, w.T.kv_len_max - kt_ * kBN)                     \
+                                                    : min(kBN, w.T.lk1 - w.T.lk0 - (kt_ - w.T.n_pref_tiles) * kBN); \
+          const int ksteps_ = (valid_ + 15) >> 4;                                                              \
+          const uint64_t dv_ = dv + (uint64_t)(sv_ * (kTileBytes >> 4));                                       \
+          _Pragma("unroll")                                                                                    \
+          for (int k = 0; k < kBN / 16; ++k)                                                                   \
+            if (k < ksteps_) mma_ts(to, ts + u_ * 64 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+          mma_commit(&sm.v_empty[sv_]);                                                                        \
+          mma_commit(&sm.pv_done[b]);                                                                          \
+          TRACE_TILE(3 + 4 * b, it_);                                                                          \
+          first = false; ++c_pv; owed0 = owed1;                                                                \
+        } while (0)
+        for (int i = 0; i < n; ++i) {
           const uint32_t it = kv_it + i;
           const int sk = it % kStagesK, sv = it % kStagesV;
           mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
-          if (takes_part(w.T, p.tpt, b, w.kt_begin + i)) {   // ---- S_b = Q_b . K^T of step i
+          if (takes_part(w.T, p.tpt, b, w.kt_begin + i)) {   // ---- S_b[u] = Q_b . K^T of step i
+            if (c_qk - c_pv == 2) AL_ISSUE_PV();             // frees the S buffer this Q.K^T writes (P aliases S)
             tc_fence_after();
             if (b == 0) TRACE(4);
-            const uint64_t dk0 = sk ? dk10 : dk00, dk1 = sk ? dk11 : dk01;
+            const uint32_t u = c_qk & 1;
+            const uint64_t dk0 = dk + (uint64_t)(sk * (kTileBytes >> 4)), dk1 = dk0 + (uint64_t)(kKvHalfBytes >> 4);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(ts, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+            for (int k = 0; k < 4; ++k) mma_ss(ts + u * 64, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(ts, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
-            mma_commit(&sm.s_full[b]);
-            TRACE_TILE(4 * b, it);
-            pend = i;
+            for (int k = 0; k < 4; ++k) mma_ss(ts + u * 64, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+            mma_commit(&sm.s_full[b][u]);
             mma_commit(&sm.k_empty[sk]);
+            TRACE_TILE(4 * b, it);
+            if (c_qk == c_pv) owed0 = i; else owed1 = i;
+            ++c_qk;
           } else {
-            // not this stream's step: hand both stages back, but only once they have landed, so that
-            // this thread can never be two stage phases ahead of the other issuer
+            // not this stream's step: pay what is owed (a V stage is reused four steps later), then hand
+            // both stages back -- but only once they have landed, so that this thread can never be two
+            // stage phases ahead of the other issuer
+            while (c_qk != c_pv) AL_ISSUE_PV();
             mma_commit(&sm.k_empty[sk]);
             mbar_wait(&sm.v_full[sv], (it / kStagesV) & 1);
             mma_commit(&sm.v_empty[sv]);
           }
           if (i == n - 1) mma_commit(&sm.q_empty);
         }
-        if (!first) mma_commit(&sm.pv_done[b]);              // only the epilogue waits for the accumulator
+        while (c_qk != c_pv) AL_ISSUE_PV();
+        if (!first) mma_commit(&sm.o_full[b]);               // the piece's accumulator is complete
+#undef AL_ISSUE_PV
         if (b == 0) TRACE(5);
         kv_it += n;
         if (!first) ++oe;
@@ -661,11 +669,12 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     const int r = quad * 32 + lane;                    // row of the sub-tile
     const int tid128 = (threadIdx.x - 128) & 127;
     const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
+    const uint32_t t_o = tmem + 256 + b * 128;
     const uint64_t scale2 = pack2(p.scale_log2, p.scale_log2);
     uint8_t* stage_b = sm.stage + b * kBM * kStagePitch;
     uint8_t* my_stage = stage_b + r * kStagePitch;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
-    uint32_t pieces_done = 0;                          // pieces in which it had key tiles: pv_done phase
+    uint32_t pieces_done = 0;                          // pieces in which it had key tiles: o_full phase
     PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
     while (w.next()) {
       const TileRec& T = w.T;
@@ -689,14 +698,16 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       for (int i = 0; i < n; ++i) {
         const int kt = w.kt_begin + i;
         if (!takes_part(T, p.tpt, b, kt)) continue;
-        mbar_wait(&sm.s_full[b], cnt & 1);
+        const uint32_t u = cnt & 1;                      // S buffer of this key tile
+        const uint32_t t_s = tmem + b * 128 + u * 64;
+        mbar_wait(&sm.s_full[b][u], (cnt >> 1) & 1);
         tc_fence_after();
         if (tid128 == 0 && b == 0) TRACE(6);
         if (tid128 == 0) TRACE_TILE(1 + 4 * b, cnt);
         TRACE_W(0);
         float s[kBN];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) tmem_ld32_f(t_s[b] + lane_addr + c * 32, s + c * 32);
+        for (int c = 0; c < kBN / 32; ++c) tmem_ld32_f(t_s + lane_addr + c * 32, s + c * 32);
         tmem_wait_ld();
         TRACE_W(1);
         // visible columns of this tile for this row: [lo, hi).  Rows beyond the sub-tile's last token are
@@ -711,9 +722,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         const bool need_mask = valid && (lo > 0 || hi < kBN);
         uint32_t hidden = 0;                             // bit c: 32-column chunk c is entirely hidden from this row
         if (__any_sync(0xffffffffu, need_mask)) {        // warp-uniform: only ragged prefix tails and local tiles
-          uint32_t vis[4];                               // bit e of vis[c]: column 32 c + e is visible
+          uint32_t vis[kBN / 32];                        // bit e of vis[c]: column 32 c + e is visible
 #pragma unroll
-          for (int c4 = 0; c4 < 4; ++c4) {
+          for (int c4 = 0; c4 < kBN / 32; ++c4) {
             const int a = min(32, max(0, lo - c4 * 32)), z = min(32, max(0, hi - c4 * 32));   // visible [a, z) of the chunk
             const uint32_t below_z = z >= 32 ? 0xffffffffu : ((1u << z) - 1u);
             const uint32_t below_a = a >= 32 ? 0xffffffffu : ((1u << a) - 1u);
@@ -735,19 +746,21 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         if (m_used == -INFINITY) m_used = m_new;         // nothing accumulated yet (O row is 0 or unwritten)
         else grow = valid && (m_new - m_used) * p.scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, grow)) {             // warp-uniform: tcgen05.ld/st are .sync.aligned
-          // rare: O of this stream must be rescaled.  Its previous P.V has landed: the commit behind
-          // s_full covers every MMA the issuer sent before this tile's Q.K^T.
+          // rare: O of this stream must be rescaled, so its previous P.V has to have landed.  pv_done[b]
+          // completes once per P.V; at most cnt of them can have completed here and all before cnt - 1
+          // have (the commit behind s_full covers them), so the parity wait cannot alias.
+          if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
           const float alpha = grow ? ex2((m_used - m_new) * p.scale_log2) : 1.0f;
           if (grow) { l_sum *= alpha; m_used = m_new; }
           if (n_mine > 0) {
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
               uint32_t o[32];
-              tmem_ld32(t_o[b] + lane_addr + c * 32, o);
+              tmem_ld32(t_o + lane_addr + c * 32, o);
               tmem_wait_ld();
 #pragma unroll
               for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-              tmem_st32(t_o[b] + lane_addr + c * 32, o);
+              tmem_st32(t_o + lane_addr + c * 32, o);
             }
           }
         }
@@ -755,7 +768,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         const uint64_t negmb2 = pack2(negmb, negmb);
         uint64_t sum_a = pack2(0.f, 0.f), sum_b = sum_a;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < kBN / 32; ++c) {
           uint32_t pk[16];
           if (hidden & (1u << c)) {                      // P = 0 without touching the MUFU
 #pragma unroll
@@ -776,7 +789,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
               pk[e] = pack_bf16x2(p0, p1);
             }
           }
-          tmem_st16(t_s[b] + lane_addr + c * 16, pk);
+          tmem_st16(t_s + lane_addr + c * 16, pk);
         }
         float l0, l1;
         unpack2(fadd2(sum_a, sum_b), l0, l1);
@@ -784,14 +797,16 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         TRACE_W(3);
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(&sm.p_full[b]);
+        mbar_arrive(&sm.p_full[b][u]);
         TRACE_W(4);
         if (tid128 == 0) TRACE_TILE(2 + 4 * b, cnt);
         ++cnt; ++n_mine;
       }
       // ---- epilogue: normalise, stage 128-byte half rows in shared memory, store coalesced ----
       if (tid128 == 0 && b == 0) TRACE(7);
-      if (n_mine > 0) { mbar_wait(&sm.pv_done[b], pieces_done & 1); tc_fence_after(); ++pieces_done; }
+      // o_full[b] completes once per piece in which the stream had key tiles (a per-P.V parity wait
+      // could alias here: with Q.K^T two tiles ahead, two P.V may still be in flight)
+      if (n_mine > 0) { mbar_wait(&sm.o_full[b], pieces_done & 1); tc_fence_after(); ++pieces_done; }
       if (tid128 == 0 && b == 0) TRACE(8);
       const float inv = l_sum > 0.f ? 1.0f / l_sum : 0.f;
       const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
@@ -806,7 +821,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #pragma unroll
           for (int c = 0; c < 2; ++c) {
             float o[32];
-            tmem_ld32_f(t_o[b] + lane_addr + rd * 64 + c * 32, o);
+            tmem_ld32_f(t_o + lane_addr + rd * 64 + c * 32, o);
             tmem_wait_ld();
             if (rd == 1 && c == 1) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }   // O_b is in registers
             uint2* dst = reinterpret_cast<uint2*>(my_stage + c * 64);
@@ -828,7 +843,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #pragma unroll
         for (int rd = 0; rd < 4; ++rd) {
           float o[32];
-          tmem_ld32_f(t_o[b] + lane_addr + rd * 32, o);
+          tmem_ld32_f(t_o + lane_addr + rd * 32, o);
           tmem_wait_ld();
           if (rd == 3) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }
           uint2* dst = reinterpret_cast<uint2*>(my_stage);
