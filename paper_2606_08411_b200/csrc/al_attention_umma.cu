@@ -358,7 +358,10 @@ __device__ unsigned long long g_trace_tile[12 * 32];
 // CTA 0, step 4 of each stream: per warp (8 softmax warps) stamps 0 S seen, 1 S in registers, 2 max done, 3 P stored, 4 arrived
 __device__ unsigned long long g_trace_warp[8 * 8];
 #define TRACE_W(k) do { if (blockIdx.x == 0 && cnt == 4 && lane == 0) g_trace_warp[(warp - 4) * 8 + (k)] = clock64(); } while (0)
+__device__ unsigned long long g_trace_epi[16];
+#define TRACE_E(k) do { if (blockIdx.x == 0 && warp == 4 && lane == 0 && g_trace_epi[k] == 0) g_trace_epi[k] = clock64(); } while (0)
 #else
+#define TRACE_E(k) do { } while (0)
 #define TRACE_W(k) do { } while (0)
 #define TRACE(i) do { } while (0)
 #define TRACE_TILE(k, i) do { } while (0)
@@ -477,23 +480,23 @@ __device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T
 }
 
 // Copies the staged 128-byte half rows [0, n_rows) of stream b to global memory with coalesced
-// 8-byte accesses: 16 lanes per half row, two half rows per warp instruction.  Half row r goes to
-// base + (r / rows_per_tok) * tok_stride + (r % rows_per_tok) * row_stride  (bytes); the quotient and
-// remainder are carried along instead of being recomputed for each of a thread's 16 rows.
-__device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, int n_rows, int tid128, uint8_t* base,
-                                              int rows_per_tok, long long tok_stride, int row_stride) {
+// 8-byte accesses: 16 lanes per half row, two half rows per warp instruction.  The 8-byte pad of a
+// staging row holds the row's global offset in units of 128 bytes (written by the row's own thread,
+// which knows its token and head), so the copy loop is address arithmetic free.
+__device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, int n_rows, int tid128, uint8_t* base) {
   const int warp = tid128 >> 5, lane = tid128 & 31;
-  const int sub = lane >> 4, chunk = lane & 15;
-  int r = warp * 32 + sub;
-  int q = r / rows_per_tok, m = r - q * rows_per_tok;
-#pragma unroll 4
+  const uint8_t* src = stage_b + (warp * 32 + (lane >> 4)) * kStagePitch + (lane & 15) * 8;
+  const int r0 = warp * 32 + (lane >> 4);
+  uint2 v[16];
+  uint32_t off[16];
+#pragma unroll
   for (int it = 0; it < 16; ++it) {
-    if (r < n_rows)
-      *reinterpret_cast<uint2*>(base + q * tok_stride + m * row_stride + chunk * 8) =
-          *reinterpret_cast<const uint2*>(stage_b + r * kStagePitch + chunk * 8);
-    r += 2; m += 2;
-    while (m >= rows_per_tok) { m -= rows_per_tok; ++q; }
+    v[it] = *reinterpret_cast<const uint2*>(src + it * 2 * kStagePitch);
+    off[it] = *reinterpret_cast<const uint32_t*>(src + it * 2 * kStagePitch - (lane & 15) * 8 + 128);
   }
+#pragma unroll
+  for (int it = 0; it < 16; ++it)
+    if (r0 + it * 2 < n_rows) *reinterpret_cast<uint2*>(base + (size_t)off[it] * 128 + (lane & 15) * 8) = v[it];
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -506,6 +509,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 
 #ifdef AL_ATTN_TRACE
   if (threadIdx.x == 0) {
+    if (blockIdx.x == 0) for (int i = 0; i < 16; ++i) g_trace_epi[i] = 0;
     for (int i = 0; i < 16; ++i) g_trace[blockIdx.x * 16 + i] = 0;
     unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
     g_trace[blockIdx.x * 16 + 15] = gt;
@@ -808,16 +812,21 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       // could alias here: with Q.K^T two tiles ahead, two P.V may still be in flight)
       if (n_mine > 0) { mbar_wait(&sm.o_full[b], pieces_done & 1); tc_fence_after(); ++pieces_done; }
       if (tid128 == 0 && b == 0) TRACE(8);
+      TRACE_E(0);
       const float inv = l_sum > 0.f ? 1.0f / l_sum : 0.f;
       const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
       const bool whole = w.whole();
       const int slot = 2 * (int)blockIdx.x + (w.kt_begin == 0 ? 1 : 0);
+      // global offset of this row's output in units of 128 bytes, for the copy loop (pad of the staging row)
+      *reinterpret_cast<uint32_t*>(my_stage + 128) =
+          whole ? (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
       if (n_mine == 0) {
         // nothing accumulated: no key tile of this piece concerns the sub-tile (or it is empty)
       } else if (whole) {
         // bf16 output: two rounds of 64 columns = 128 bytes per row
 #pragma unroll
         for (int rd = 0; rd < 2; ++rd) {
+          TRACE_E(1 + 5 * rd);
 #pragma unroll
           for (int c = 0; c < 2; ++c) {
             float o[32];
@@ -830,11 +839,13 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
               dst[e] = make_uint2(pack_bf16x2(o[4 * e] * inv, o[4 * e + 1] * inv),
                                   pack_bf16x2(o[4 * e + 2] * inv, o[4 * e + 3] * inv));
           }
+          TRACE_E(2 + 5 * rd);
           bar_sync_stream(b);
-          copy_out_rows(stage_b, n_rows, tid128,
-                        reinterpret_cast<uint8_t*>(p.out + out_row(p, T, w.g, b, 0) * kD) + rd * 128, p.n_rep,
-                        (long long)p.n_q_heads * kD * 2, kD * 2);
+          TRACE_E(3 + 5 * rd);
+          copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + rd * 128);
+          TRACE_E(4 + 5 * rd);
           bar_sync_stream(b);                          // the staging rows are rewritten by the next round / piece
+          TRACE_E(5 + 5 * rd);
         }
         if (valid && p.lse) p.lse[out_row(p, T, w.g, b, r)] = lse;
       } else {
@@ -850,7 +861,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 #pragma unroll
           for (int e = 0; e < 16; ++e) dst[e] = make_uint2(__float_as_uint(o[2 * e] * inv), __float_as_uint(o[2 * e + 1] * inv));
           bar_sync_stream(b);
-          copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + rd * 128, kBM, 0, kD * 4);
+          copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + rd * 128);
           bar_sync_stream(b);
         }
       }
@@ -890,6 +901,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 }
 #ifdef AL_ATTN_TRACE
 int trace_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace)); }
+int trace_epi_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_epi, sizeof(g_trace_epi)); }
 int trace_warp_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_warp, sizeof(g_trace_warp)); }
 int trace_tile_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_tile, sizeof(g_trace_tile)); }
 #endif
@@ -1031,6 +1043,7 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
 
 #ifdef AL_ATTN_TRACE
 extern "C" int al_debug_attn_trace(unsigned long long* host_out) { return trace_read(host_out); }   // [kMaxCtas * 16]
+extern "C" int al_debug_attn_trace_epi(unsigned long long* host_out) { return trace_epi_read(host_out); }   // [16]
 extern "C" int al_debug_attn_trace_warp(unsigned long long* host_out) { return trace_warp_read(host_out); }   // [8 * 8]
 extern "C" int al_debug_attn_trace_tile(unsigned long long* host_out) { return trace_tile_read(host_out); }   // [4 * 32]
 extern "C" int al_debug_mbar_timeout(unsigned int* host_out) {   // [4]; [0] != 0 when a wait timed out
