@@ -572,12 +572,15 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         }
         ++piece_it;
       }
-    } else if ((warp == 1 || warp == 2) && lane == 0 && active) {
+    } else if ((warp == 1 || warp == 2) && active) {
       // ===================== MMA issuers: warp 1 for stream A, warp 2 for stream B =====================
       // Per stream S is double-buffered (2 x 64 TMEM columns; P aliases S), so Q.K^T runs two key tiles
       // ahead of P.V: the order is QK(0) QK(1) PV(0) QK(2) PV(1) QK(3) ... and the softmax of tile i+1
       // never waits for the MMAs of tile i.  Two issuing threads keep one stream's wait for its softmax
       // from holding up the other stream's MMAs; both arrive on the K/V/Q stage barriers (count 2).
+      // The whole warp runs the loop (uniform control flow keeps descriptors and addresses in uniform
+      // registers); one elected lane issues the tcgen05 instructions.
+      const bool leader = elect_one();
       const int b = warp - 1;
       const uint32_t ts = tmem + b * 128, to = tmem + 256 + b * 128;
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
@@ -595,7 +598,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         const int n = w.kt_end - w.kt_begin;
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
-        if (b == 0) TRACE(3);
+        if (b == 0 && leader) TRACE(3);
         int owed0 = 0, owed1 = 0;              // steps (of the piece) of the up to two key tiles whose P.V is owed, oldest first
         bool first = true;
         // O_b (+)= P . V of the oldest owed key tile
@@ -604,9 +607,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           const uint32_t it_ = kv_it + owed0;                                                                  \
           const int sv_ = it_ % kStagesV;                                                                      \
           const uint32_t u_ = c_pv & 1;                                                                        \
-          TRACE_TILE(8 + b, it_);                                                                              \
+          if (leader) TRACE_TILE(8 + b, it_);                                                                              \
           mbar_wait(&sm.p_full[b][u_], (c_pv >> 1) & 1);                                                       \
-          TRACE_TILE(10 + b, it_);                                                                             \
+          if (leader) TRACE_TILE(10 + b, it_);                                                                             \
           mbar_wait(&sm.v_full[sv_], (it_ / kStagesV) & 1);                                                    \
           /* O_b of the stream's previous piece has been read out.  Only pieces in which the stream had     */ \
           /* key tiles complete a phase of o_empty[b] (oe counts them), so neither side can run ahead.      */ \
@@ -620,10 +623,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           const uint64_t dv_ = dv + (uint64_t)(sv_ * (kTileBytes >> 4));                                       \
           _Pragma("unroll")                                                                                    \
           for (int k = 0; k < kBN / 16; ++k)                                                                   \
-            if (k < ksteps_) mma_ts(to, ts + u_ * 64 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
-          mma_commit(&sm.v_empty[sv_]);                                                                        \
-          mma_commit(&sm.pv_done[b]);                                                                          \
-          TRACE_TILE(3 + 4 * b, it_);                                                                          \
+            if (leader && k < ksteps_) mma_ts(to, ts + u_ * 64 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+          if (leader) { mma_commit(&sm.v_empty[sv_]); mma_commit(&sm.pv_done[b]); }                            \
+          if (leader) TRACE_TILE(3 + 4 * b, it_);                                                                          \
           first = false; ++c_pv; owed0 = owed1;                                                                \
         } while (0)
         for (int i = 0; i < n; ++i) {
@@ -633,16 +635,15 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           if (takes_part(w.T, p.tpt, b, w.kt_begin + i)) {   // ---- S_b[u] = Q_b . K^T of step i
             if (c_qk - c_pv == 2) AL_ISSUE_PV();             // frees the S buffer this Q.K^T writes (P aliases S)
             tc_fence_after();
-            if (b == 0) TRACE(4);
+            if (b == 0 && leader) TRACE(4);
             const uint32_t u = c_qk & 1;
             const uint64_t dk0 = dk + (uint64_t)(sk * (kTileBytes >> 4)), dk1 = dk0 + (uint64_t)(kKvHalfBytes >> 4);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(ts + u * 64, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * 64, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) mma_ss(ts + u * 64, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
-            mma_commit(&sm.s_full[b][u]);
-            mma_commit(&sm.k_empty[sk]);
-            TRACE_TILE(4 * b, it);
+            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * 64, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+            if (leader) { mma_commit(&sm.s_full[b][u]); mma_commit(&sm.k_empty[sk]); }
+            if (leader) TRACE_TILE(4 * b, it);
             if (c_qk == c_pv) owed0 = i; else owed1 = i;
             ++c_qk;
           } else {
@@ -650,16 +651,16 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
             // both stages back -- but only once they have landed, so that this thread can never be two
             // stage phases ahead of the other issuer
             while (c_qk != c_pv) AL_ISSUE_PV();
-            mma_commit(&sm.k_empty[sk]);
+            if (leader) mma_commit(&sm.k_empty[sk]);
             mbar_wait(&sm.v_full[sv], (it / kStagesV) & 1);
-            mma_commit(&sm.v_empty[sv]);
+            if (leader) mma_commit(&sm.v_empty[sv]);
           }
-          if (i == n - 1) mma_commit(&sm.q_empty);
+          if (leader && i == n - 1) mma_commit(&sm.q_empty);
         }
         while (c_qk != c_pv) AL_ISSUE_PV();
-        if (!first) mma_commit(&sm.o_full[b]);               // the piece's accumulator is complete
+        if (leader && !first) mma_commit(&sm.o_full[b]);               // the piece's accumulator is complete
 #undef AL_ISSUE_PV
-        if (b == 0) TRACE(5);
+        if (b == 0 && leader) TRACE(5);
         kv_it += n;
         if (!first) ++oe;
         ++piece_it;
