@@ -353,7 +353,7 @@ __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
 __device__ unsigned long long g_trace[kMaxCtas * 16];
 #define TRACE(i) do { if (g_trace[blockIdx.x * 16 + (i)] == 0) g_trace[blockIdx.x * 16 + (i)] = clock64(); } while (0)
 // CTA 0 only: per step (first 32 of the CTA) stamps of kind k: 0 QK_A issued, 1 S seen by stream A, 2 P_A ready, 3 PV_A issued
-__device__ unsigned long long g_trace_tile[12 * 32];
+__device__ unsigned long long g_trace_tile[16 * 32];
 #define TRACE_TILE(k, i) do { if (blockIdx.x == 0 && (i) < 32) g_trace_tile[(k) * 32 + (i)] = clock64(); } while (0)
 // CTA 0, step 4 of each stream: per warp (8 softmax warps) stamps 0 S seen, 1 S in registers, 2 max done, 3 P stored, 4 arrived
 __device__ unsigned long long g_trace_warp[8 * 8];
@@ -505,7 +505,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
                            const __grid_constant__ CUtensorMap map_vc, const AttnParams p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   AttnSmem& sm = *reinterpret_cast<AttnSmem*>(smem_raw);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // the shuffle tells the compiler that `warp` is warp-uniform: the role branches and everything derived
+  // from it (stream index, TMEM and shared-memory descriptors) then live in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
 
 #ifdef AL_ATTN_TRACE
   if (threadIdx.x == 0) {
@@ -611,6 +613,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           mbar_wait(&sm.p_full[b][u_], (c_pv >> 1) & 1);                                                       \
           if (leader) TRACE_TILE(10 + b, it_);                                                                             \
           mbar_wait(&sm.v_full[sv_], (it_ / kStagesV) & 1);                                                    \
+          if (leader && b == 0) TRACE_TILE(14, it_);                                                           \
           /* O_b of the stream's previous piece has been read out.  Only pieces in which the stream had     */ \
           /* key tiles complete a phase of o_empty[b] (oe counts them), so neither side can run ahead.      */ \
           if (first && oe > 0) mbar_wait(&sm.o_empty[b], (oe - 1) & 1);                                        \
@@ -631,7 +634,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         for (int i = 0; i < n; ++i) {
           const uint32_t it = kv_it + i;
           const int sk = it % kStagesK, sv = it % kStagesV;
+          if (leader && b == 0) TRACE_TILE(12, it);
           mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
+          if (leader && b == 0) TRACE_TILE(13, it);
           if (takes_part(w.T, p.tpt, b, w.kt_begin + i)) {   // ---- S_b[u] = Q_b . K^T of step i
             if (c_qk - c_pv == 2) AL_ISSUE_PV();             // frees the S buffer this Q.K^T writes (P aliases S)
             tc_fence_after();
