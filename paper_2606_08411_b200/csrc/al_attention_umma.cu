@@ -44,10 +44,11 @@ using namespace alptx;
 namespace {
 
 constexpr int kBM = 128;                   // stacked query rows per tile
-constexpr int kBN = 64;                    // keys per key tile (step): S_b is 64 fp32 TMEM columns, double-buffered
+constexpr int kBN = 64;                    // keys per key tile (step); 64 lets S be double-buffered (measured faster than 128)
+constexpr int kSBuf = 128 / kBN;           // S buffers per stream in its 128 TMEM columns (P aliases S)
 constexpr int kD = 128;                    // head_dim
-constexpr int kStagesK = 4;                // K ring depth (a K tile lives until its Q.K^T has run)
-constexpr int kStagesV = 4;                // V ring depth (a V tile lives until its P.V has run)
+constexpr int kStagesK = 256 / kBN;                // K ring depth (a K tile lives until its Q.K^T has run)
+constexpr int kStagesV = 256 / kBN;                // V ring depth (a V tile lives until its P.V has run)
 constexpr int kHalfBytes = kBM * 64 * 2;   // Q: [128 rows][64 bf16] = one 128-byte-swizzled half tile
 constexpr int kKvHalfBytes = kBN * 64 * 2; // K, V: [64 keys][64 bf16]
 constexpr int kTileBytes = 2 * kKvHalfBytes;
@@ -58,7 +59,7 @@ constexpr int kMaxPlanLanes = 1024;
 constexpr int kMaxPlanTiles = 2048;
 constexpr int kPlanThreads = 1024;
 constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
-constexpr int kMinPiece = 4;               // do not cut the work finer than 4 key-tile steps (256 keys) per CTA
+constexpr int kMinPiece = 256 / kBN;       // do not cut the work finer than 256 keys per CTA
 
 struct __align__(16) TileRec {             // 64 bytes
   int q_tok0, n_tok;          // first packed token row, tokens in the tile (<= 2 tpt)
@@ -273,7 +274,7 @@ struct AttnSmem {
   alignas(16) uint8_t stage[2 * kBM * kStagePitch];    // epilogue staging: half row (stream b, row r) at b*128 + r
   uint64_t q_full, q_empty;
   uint64_t k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV];
-  uint64_t s_full[2][2], p_full[2][2];     // [stream][S buffer]
+  uint64_t s_full[2][kSBuf], p_full[2][kSBuf];   // [stream][S buffer]
   uint64_t pv_done[2];                     // per P.V: the lazy rescale of O waits for the stream's previous P.V
   uint64_t o_full[2], o_empty[2];          // per piece: accumulator complete / read out
   uint32_t tmem_base;
@@ -524,7 +525,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 2); }
     for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 2); }
     for (int b = 0; b < 2; ++b) {
-      for (int u = 0; u < 2; ++u) { mbar_init(&sm.s_full[b][u], 1); mbar_init(&sm.p_full[b][u], 128); }
+      for (int u = 0; u < kSBuf; ++u) { mbar_init(&sm.s_full[b][u], 1); mbar_init(&sm.p_full[b][u], 128); }
       mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_full[b], 1); mbar_init(&sm.o_empty[b], 128);
     }
     fence_barrier_init();
@@ -608,9 +609,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         do {                                                                                                   \
           const uint32_t it_ = kv_it + owed0;                                                                  \
           const int sv_ = it_ % kStagesV;                                                                      \
-          const uint32_t u_ = c_pv & 1;                                                                        \
+          const uint32_t u_ = c_pv % kSBuf;                                                                    \
           if (leader) TRACE_TILE(8 + b, it_);                                                                              \
-          mbar_wait(&sm.p_full[b][u_], (c_pv >> 1) & 1);                                                       \
+          mbar_wait(&sm.p_full[b][u_], (c_pv / kSBuf) & 1);                                                    \
           if (leader) TRACE_TILE(10 + b, it_);                                                                             \
           mbar_wait(&sm.v_full[sv_], (it_ / kStagesV) & 1);                                                    \
           if (leader && b == 0) TRACE_TILE(14, it_);                                                           \
@@ -626,7 +627,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           const uint64_t dv_ = dv + (uint64_t)(sv_ * (kTileBytes >> 4));                                       \
           _Pragma("unroll")                                                                                    \
           for (int k = 0; k < kBN / 16; ++k)                                                                   \
-            if (leader && k < ksteps_) mma_ts(to, ts + u_ * 64 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+            if (leader && k < ksteps_) mma_ts(to, ts + u_ * kBN + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
           if (leader) { mma_commit(&sm.v_empty[sv_]); mma_commit(&sm.pv_done[b]); }                            \
           if (leader) TRACE_TILE(3 + 4 * b, it_);                                                                          \
           first = false; ++c_pv; owed0 = owed1;                                                                \
@@ -638,15 +639,15 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
           if (leader && b == 0) TRACE_TILE(13, it);
           if (takes_part(w.T, p.tpt, b, w.kt_begin + i)) {   // ---- S_b[u] = Q_b . K^T of step i
-            if (c_qk - c_pv == 2) AL_ISSUE_PV();             // frees the S buffer this Q.K^T writes (P aliases S)
+            if (c_qk - c_pv == kSBuf) AL_ISSUE_PV();         // frees the S buffer this Q.K^T writes (P aliases S)
             tc_fence_after();
             if (b == 0 && leader) TRACE(4);
-            const uint32_t u = c_qk & 1;
+            const uint32_t u = c_qk % kSBuf;
             const uint64_t dk0 = dk + (uint64_t)(sk * (kTileBytes >> 4)), dk1 = dk0 + (uint64_t)(kKvHalfBytes >> 4);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * 64, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * 64, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
             if (leader) { mma_commit(&sm.s_full[b][u]); mma_commit(&sm.k_empty[sk]); }
             if (leader) TRACE_TILE(4 * b, it);
             if (c_qk == c_pv) owed0 = i; else owed1 = i;
@@ -708,9 +709,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       for (int i = 0; i < n; ++i) {
         const int kt = w.kt_begin + i;
         if (!takes_part(T, p.tpt, b, kt)) continue;
-        const uint32_t u = cnt & 1;                      // S buffer of this key tile
-        const uint32_t t_s = tmem + b * 128 + u * 64;
-        mbar_wait(&sm.s_full[b][u], (cnt >> 1) & 1);
+        const uint32_t u = cnt % kSBuf;                  // S buffer of this key tile
+        const uint32_t t_s = tmem + b * 128 + u * kBN;
+        mbar_wait(&sm.s_full[b][u], (cnt / kSBuf) & 1);
         tc_fence_after();
         if (tid128 == 0 && b == 0) TRACE(6);
         if (tid128 == 0) TRACE_TILE(1 + 4 * b, cnt);
@@ -846,11 +847,11 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
                                   pack_bf16x2(o[4 * e + 2] * inv, o[4 * e + 3] * inv));
           }
           TRACE_E(2 + 5 * rd);
-          bar_sync_stream(b);
+          __syncwarp();                                // a warp stages and copies its own 32 rows
           TRACE_E(3 + 5 * rd);
           copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + rd * 128);
           TRACE_E(4 + 5 * rd);
-          bar_sync_stream(b);                          // the staging rows are rewritten by the next round / piece
+          __syncwarp();                                // the staging rows are rewritten by the next round / piece
           TRACE_E(5 + 5 * rd);
         }
         if (valid && p.lse) p.lse[out_row(p, T, w.g, b, r)] = lse;
@@ -866,9 +867,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           uint2* dst = reinterpret_cast<uint2*>(my_stage);
 #pragma unroll
           for (int e = 0; e < 16; ++e) dst[e] = make_uint2(__float_as_uint(o[2 * e] * inv), __float_as_uint(o[2 * e + 1] * inv));
-          bar_sync_stream(b);
+          __syncwarp();
           copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + rd * 128);
-          bar_sync_stream(b);
+          __syncwarp();
         }
       }
       if (tid128 == 0 && b == 0) TRACE(9);
