@@ -361,8 +361,10 @@ __device__ unsigned long long g_trace_warp[8 * 8];
 #define TRACE_W(k) do { if (blockIdx.x == 0 && cnt == 4 && lane == 0) g_trace_warp[(warp - 4) * 8 + (k)] = clock64(); } while (0)
 __device__ unsigned long long g_trace_epi[16];
 #define TRACE_E(k) do { if (blockIdx.x == 0 && warp == 4 && lane == 0 && g_trace_epi[k] == 0) g_trace_epi[k] = clock64(); } while (0)
+#define TRACE_M(k) do { if (blockIdx.x == 12 && tid128 == 0 && b == 0 && g_trace_epi[k] == 0) g_trace_epi[k] = clock64(); } while (0)
 #else
 #define TRACE_E(k) do { } while (0)
+#define TRACE_M(k) do { } while (0)
 #define TRACE_W(k) do { } while (0)
 #define TRACE(i) do { } while (0)
 #define TRACE_TILE(k, i) do { } while (0)
@@ -424,59 +426,83 @@ __device__ __forceinline__ int sub_rows(const AttnParams& p, const TileRec& T, i
 
 // Merge of the partials of sub-tile b of one split item by the 128 threads of stream b in the CTA
 // that finished last.  Pieces of an item live on consecutive CTAs c0..c1: slot 2*c0+1 (c0's last
-// piece), then 2*c for the rest.  Warp w owns rows [32w, 32w+32) in two passes of 16: lanes 0-15 hold
-// the rows' weights, every lane one float4 column group, so each piece costs 16 independent fully
-// coalesced 512-byte row loads per warp and pass.
-__device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T, int g, int b, int c0, int c1, int tid128) {
+// piece), then 2*c for the rest.  Warp w owns rows [32w, 32w+32) in four passes of 8 rows; a lane holds
+// one float4 column group.  Per pass the loads of up to four pieces (8 coalesced 512-byte rows each,
+// plus the rows' LSE in lanes 0-7) are all issued before any is used, so a pass costs one L2 round
+// trip; further pieces are folded in with a running maximum.  The order of operations is fixed, so
+// the result does not depend on which CTA happens to arrive last.
+__device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T, int g, int b, int c0, int c1,
+                                           int tid128) {
   const int warp = tid128 >> 5, lane = tid128 & 31;
   const int n_rows = sub_rows(p, T, b);
   const int n_pieces = c1 - c0 + 1;
-  for (int pass = 0; pass < 2; ++pass) {
-    const int row0 = warp * 32 + pass * 16;
+  for (int pass = 0; pass < 4; ++pass) {
+    const int row0 = warp * 32 + pass * 8;
     if (row0 >= n_rows) break;
-    const int my_row = row0 + (lane & 15);
+    const int my_row = row0 + (lane & 7);
     const bool has_row = my_row < n_rows;
-    float mx = -INFINITY;
-    for (int j = 0; j < n_pieces; ++j) {
-      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
-      if (has_row) mx = fmaxf(mx, __ldcg(p.plan.part_lse + ((long long)slot * 2 + b) * kBM + my_row));
-    }
-    float wsum = 0.f;
-    float4 acc[16];
+    float mx = -INFINITY, wsum = 0.f;              // running maximum of the LSEs and sum of weights of lane's row
+    float4 acc[8];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int j = 0; j < n_pieces; ++j) {
-      const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
-      const float ls = has_row ? __ldcg(p.plan.part_lse + ((long long)slot * 2 + b) * kBM + my_row) : -INFINITY;
-      const float4* src =
-          reinterpret_cast<const float4*>(p.plan.part_o + (((long long)slot * 2 + b) * kBM + row0) * kD) + lane;
-      float4 v[16];
+    for (int k = 0; k < 8; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    TRACE_M(11 + 0);
+    for (int j0 = 0; j0 < n_pieces; j0 += 4) {
+      float4 v[4][8];
+      float ls[4];
 #pragma unroll
-      for (int k = 0; k < 16; ++k)
-        v[k] = row0 + k < n_rows ? __ldcg(src + k * (kD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-      const float wgt = (ls == -INFINITY) ? 0.f : exp2f((ls - mx) * kLog2e);   // 0: the row saw no key in this piece
-      wsum += wgt;
+      for (int jj = 0; jj < 4; ++jj) {
+        const int j = j0 + jj;
+        const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
+        const bool pj = j < n_pieces;
+        ls[jj] = (pj && has_row) ? __ldcg(p.plan.part_lse + ((long long)slot * 2 + b) * kBM + my_row) : -INFINITY;
+        const float4* src =
+            reinterpret_cast<const float4*>(p.plan.part_o + (((long long)slot * 2 + b) * kBM + row0) * kD) + lane;
 #pragma unroll
-      for (int k = 0; k < 16; ++k) {
-        const float wk = __shfl_sync(0xffffffffu, wgt, k);
-        if (wk > 0.f) {                                // rows without data in this piece hold stale memory
-          acc[k].x = fmaf(wk, v[k].x, acc[k].x); acc[k].y = fmaf(wk, v[k].y, acc[k].y);
-          acc[k].z = fmaf(wk, v[k].z, acc[k].z); acc[k].w = fmaf(wk, v[k].w, acc[k].w);
+        for (int k = 0; k < 8; ++k)
+          v[jj][k] = (pj && row0 + k < n_rows) ? __ldcg(src + k * (kD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+      TRACE_M(12);
+      const float mx_new = fmaxf(fmaxf(mx, fmaxf(ls[0], ls[1])), fmaxf(ls[2], ls[3]));
+      if (mx_new == 123.456f) TRACE_M(15);
+      const float resc = (mx == -INFINITY) ? 0.f : exp2f((mx - mx_new) * kLog2e);     // 1 when the maximum stands
+      wsum *= resc;
+      mx = mx_new;
+      float wj[4];
+#pragma unroll
+      for (int jj = 0; jj < 4; ++jj) {
+        wj[jj] = (ls[jj] == -INFINITY) ? 0.f : exp2f((ls[jj] - mx) * kLog2e);   // 0: the row saw no key in this piece
+        wsum += wj[jj];
+      }
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const float rk = __shfl_sync(0xffffffffu, resc, k);
+        acc[k].x *= rk; acc[k].y *= rk; acc[k].z *= rk; acc[k].w *= rk;
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+          const float wk = __shfl_sync(0xffffffffu, wj[jj], k);
+          const bool on = wk > 0.f;                    // rows without data in this piece hold stale memory
+          acc[k].x = fmaf(wk, on ? v[jj][k].x : 0.f, acc[k].x); acc[k].y = fmaf(wk, on ? v[jj][k].y : 0.f, acc[k].y);
+          acc[k].z = fmaf(wk, on ? v[jj][k].z : 0.f, acc[k].z); acc[k].w = fmaf(wk, on ? v[jj][k].w : 0.f, acc[k].w);
         }
       }
     }
+    TRACE_M(13);
     const float inv = wsum > 0.f ? 1.0f / wsum : 0.f;
+    int tl = row0 / p.n_rep, hl = row0 - tl * p.n_rep;                 // token and head of row0, carried along
+    long long orow = (long long)(T.q_tok0 + b * p.tpt + tl) * p.n_q_heads + g * p.n_rep + hl;
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
+    for (int k = 0; k < 8; ++k) {
       const float ik = __shfl_sync(0xffffffffu, inv, k);
       if (row0 + k < n_rows) {
         uint2 pk;
         pk.x = pack_bf16x2(acc[k].x * ik, acc[k].y * ik);
         pk.y = pack_bf16x2(acc[k].z * ik, acc[k].w * ik);
-        reinterpret_cast<uint2*>(p.out + out_row(p, T, g, b, row0 + k) * kD)[lane] = pk;
+        reinterpret_cast<uint2*>(p.out + orow * kD)[lane] = pk;
       }
+      if (++hl == p.n_rep) { hl = 0; orow += p.n_q_heads - p.n_rep + 1; } else ++orow;
     }
-    if (p.lse && has_row && lane < 16) p.lse[out_row(p, T, g, b, my_row)] = mx + logf(wsum);
+    if (p.lse && has_row && lane < 8) p.lse[out_row(p, T, g, b, my_row)] = mx + logf(wsum);
+    TRACE_M(14);
   }
 }
 
@@ -512,7 +538,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 
 #ifdef AL_ATTN_TRACE
   if (threadIdx.x == 0) {
-    if (blockIdx.x == 0) for (int i = 0; i < 16; ++i) g_trace_epi[i] = 0;
+    if (blockIdx.x == 0 || blockIdx.x == 12) for (int i = (blockIdx.x ? 11 : 0); i < (blockIdx.x ? 16 : 11); ++i) g_trace_epi[i] = 0;
     for (int i = 0; i < 16; ++i) g_trace[blockIdx.x * 16 + i] = 0;
     unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
     g_trace[blockIdx.x * 16 + 15] = gt;
