@@ -60,6 +60,7 @@ constexpr int kMaxPlanTiles = 2048;
 constexpr int kPlanThreads = 1024;
 constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
 constexpr int kMinPiece = 256 / kBN;       // do not cut the work finer than 256 keys per CTA
+constexpr int kSplitCost = 640 / kBN;      // what splitting an item costs (partial epilogue + merge), in steps: measured ~10 us
 
 struct __align__(16) TileRec {             // 64 bytes
   int q_tok0, n_tok;          // first packed token row, tokens in the tile (<= 2 tpt)
@@ -154,7 +155,9 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   __shared__ int s_run_tile_base[kMaxPlanLanes + 1];
   __shared__ int s_bounds[kMaxCtas + 1];
   __shared__ int s_warp[32];
+  __shared__ int s_max_nk;                     // longest item, in steps
   const int tid = threadIdx.x;
+  if (tid == 0) s_max_nk = 0;
 
   // runs
   for (int i = tid; i < n_lanes; i += blockDim.x) {
@@ -212,18 +215,28 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     T.kt_off = 0;
     plan.tiles[t] = T;
     s_a[t] = T.n_key_tiles * n_kv_heads;
+    atomicMax(&s_max_nk, T.n_key_tiles);
   }
   __syncthreads();
   const int k_total = block_exclusive_scan(s_a, n_tiles, s_warp);
   if (tid == 0) s_a[n_tiles] = k_total;
   for (int t = tid; t < n_tiles; t += blockDim.x) plan.tiles[t].kt_off = s_a[t];
   // per-CTA ranges of the flattened step sequence
-  const int n_ctas = max(1, min(min(bounds.grid, kMaxCtas), ceil_div(k_total, kMinPiece)));
-  const bool snap = k_total / n_ctas >= 4;
+  const int grid = min(bounds.grid, kMaxCtas);
+  int n_ctas = max(1, min(grid, ceil_div(k_total, kMinPiece)));
+  // When every item can have a CTA of its own, cutting items only pays if the longest item costs more
+  // than the balanced share plus what a split costs (fp32 partials, tickets, merge).
   __syncthreads();
+  const bool whole_items = n_tiles > 0 && n_tiles * n_kv_heads <= grid &&
+                           s_max_nk <= ceil_div(k_total, n_ctas) + kSplitCost;
+  if (whole_items) n_ctas = n_tiles * n_kv_heads;
+  const bool snap = k_total / n_ctas >= 4;
   for (int c = tid; c <= n_ctas; c += blockDim.x) {
     int f = (int)((long long)c * k_total / n_ctas);
-    if (snap && c > 0 && c < n_ctas) {
+    if (whole_items) {                                 // CTA c = item c = (tile c / n_kv, head c % n_kv)
+      const int t = c / n_kv_heads;
+      f = c == n_ctas ? k_total : s_a[t] + (c - t * n_kv_heads) * ((s_a[t + 1] - s_a[t]) / n_kv_heads);
+    } else if (snap && c > 0 && c < n_ctas) {
       const int t = last_le(s_a, n_tiles, f);
       const int nk = (s_a[t + 1] - s_a[t]) / n_kv_heads;
       const int rem = (f - s_a[t]) % nk;           // steps into the item
