@@ -57,7 +57,8 @@ constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: P <= 2^8 between rescales
 constexpr int kMaxPlanLanes = 1024;
 constexpr int kMaxPlanTiles = 2048;
-constexpr int kPlanThreads = 1024;
+constexpr int kPlanThreads = 256;
+constexpr int kPlanTilesInSmem = 96;
 constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
 constexpr int kMinPiece = 256 / kBN;       // do not cut the work finer than 256 keys per CTA
 constexpr int kSplitCost = 640 / kBN;      // what splitting an item costs (partial epilogue + merge), in steps: measured ~10 us
@@ -149,7 +150,8 @@ __device__ __forceinline__ int last_le(const int* a, int n, int x) {
 __global__ void __launch_bounds__(kPlanThreads)
 lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_heads, int tpt, Bounds bounds,
                  Plan plan) {
-  __shared__ int s_qs[kMaxPlanLanes], s_qe[kMaxPlanLanes], s_pl[kMaxPlanLanes];
+  __shared__ int s_qs[kMaxPlanLanes], s_qe[kMaxPlanLanes], s_pl[kMaxPlanLanes], s_kb[kMaxPlanLanes];
+  __shared__ TileRec s_tiles[kPlanTilesInSmem];   // the first tiles, so that small plans need no global read-back
   __shared__ int s_run_lane0[kMaxPlanLanes + 1];
   __shared__ int s_a[kMaxPlanTiles + 1];       // scan scratch: run flags, tiles per run, steps per tile
   __shared__ int s_run_tile_base[kMaxPlanLanes + 1];
@@ -157,12 +159,15 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   __shared__ int s_warp[32];
   __shared__ int s_max_nk;                     // longest item, in steps
   const int tid = threadIdx.x;
+  // programmatic dependent launch: the attention kernel may start its prologue (barriers, TMEM) now; it
+  // waits for this grid's completion before it reads the plan
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (tid == 0) s_max_nk = 0;
 
   // runs
   for (int i = tid; i < n_lanes; i += blockDim.x) {
     const al_lane_desc b = lanes[i];
-    s_qs[i] = b.q_start; s_qe[i] = b.q_start + b.q_len; s_pl[i] = b.prefix_len;
+    s_qs[i] = b.q_start; s_qe[i] = b.q_start + b.q_len; s_pl[i] = b.prefix_len; s_kb[i] = b.kv_base_row;
     int start = 1;
     if (i > 0) {
       const al_lane_desc a = lanes[i - 1];
@@ -193,7 +198,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     TileRec T;
     T.q_tok0 = s_qs[l0] + (t - s_run_tile_base[r]) * 2 * tpt;
     T.n_tok = min(2 * tpt, s_qe[l1 - 1] - T.q_tok0);
-    T.kv_base_row = lanes[l0].kv_base_row;
+    T.kv_base_row = s_kb[l0];
     T.kv_len_max = 0; T.kv_len_min = 0x7fffffff; T.lk0 = 0x7fffffff; T.lk1 = 0;
     T.sub_lk0[0] = T.sub_lk0[1] = 0x7fffffff; T.sub_lk1[0] = T.sub_lk1[1] = 0;
     const int lf = l0 + last_le(s_qs + l0, l1 - l0, T.q_tok0);    // lane that holds the tile's first token
@@ -214,6 +219,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     T.n_key_tiles = T.n_pref_tiles + ceil_div(T.lk1 - T.lk0, kBN);
     T.kt_off = 0;
     plan.tiles[t] = T;
+    if (t < kPlanTilesInSmem) s_tiles[t] = T;
     s_a[t] = T.n_key_tiles * n_kv_heads;
     atomicMax(&s_max_nk, T.n_key_tiles);
   }
@@ -253,7 +259,10 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
       C.tile0 = n_tiles ? last_le(s_a, n_tiles, C.f_begin) : 0;
       C.first_c0 = C.first_c1 = C.last_c0 = C.last_c1 = c;
       C.pad = 0;
-      if (n_tiles) { C.first = plan.tiles[C.tile0]; C.first.kt_off = s_a[C.tile0]; }   // written by this block above
+      if (n_tiles) {
+        C.first = C.tile0 < kPlanTilesInSmem ? s_tiles[C.tile0] : plan.tiles[C.tile0];   // written by this block above
+        C.first.kt_off = s_a[C.tile0];
+      }
       if (n_tiles && C.f_begin < C.f_end) {
         for (int e = 0; e < 2; ++e) {            // e = 0: item of the first step, 1: item of the last step
           const int f = e ? C.f_end - 1 : C.f_begin;
@@ -577,6 +586,11 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   // TMEM columns: S of stream b, buffer u at (2 b + u) * 64; O of stream b at 256 + 128 b
+  // programmatic dependent launch: everything above overlapped the previous kernel in the stream (the
+  // plan, or the previous layer); its memory is visible after the wait.  The next launch in the stream
+  // that opts in (the next layer) may then begin its own prologue as SMs free up.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const bool active = (int)blockIdx.x < p.plan.hdr->n_ctas;
   if (threadIdx.x == 0) TRACE(1);
 
@@ -1081,8 +1095,17 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   p.q_box_bytes = (uint32_t)(2 * tpt * n_rep * 64 * 2);
   const size_t smem = sizeof(AttnSmem);
   AL_CUDA_OK(cudaFuncSetAttribute(lane_attention_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  lane_attention_umma_kernel<<<b.grid, kThreads, smem, st>>>(mq, mkn, mvn, mkc, mvc, p);
-  AL_CUDA_OK(cudaGetLastError());
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)b.grid);
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.wait in the kernel
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lane_attention_umma_kernel, mq, mkn, mvn, mkc, mvc, p));
   h->launches += 1;
   return AL_OK;
 }
