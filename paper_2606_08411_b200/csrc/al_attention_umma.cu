@@ -301,6 +301,7 @@ struct AttnSmem {
   uint64_t o_full[2], o_empty[2];          // per piece: accumulator complete / read out
   uint32_t tmem_base;
   int ticket[2][3];
+  int alt_has[2];                          // alt mode: did stream b have key tiles in this piece
 };
 static_assert(sizeof(AttnSmem) <= 232448, "AttnSmem exceeds the 227 KB opt-in shared memory of sm_100");
 
@@ -356,9 +357,12 @@ struct PieceWalk {
   __device__ __forceinline__ int item() const { return t * n_kv + g; }
 };
 
-// Does sub-tile b of tile T have work in key tile kt?  (prefix tiles: always; local tiles: only
-// those that hold rows of the lanes the sub-tile's tokens belong to)
+// Does stream b have work in key tile kt of tile T?  Two sub-tiles: stream b = sub-tile b (prefix tiles:
+// always; local tiles: only those that hold rows of the lanes the sub-tile's tokens belong to).  One
+// sub-tile ("alt" mode): even key tiles go to stream 0, odd ones to stream 1, each with its own running
+// max, row sum and accumulator; the epilogue merges the two.
 __device__ __forceinline__ bool takes_part(const TileRec& T, int tpt, int b, int kt) {
+  if (T.n_tok <= tpt) return (kt & 1) == b;  // a tile of one sub-tile: the two streams take alternate key tiles of it
   if (b * tpt >= T.n_tok) return false;
   if (kt < T.n_pref_tiles) return true;
   const int k0 = T.lk0 + (kt - T.n_pref_tiles) * kBN;
@@ -391,6 +395,7 @@ __device__ unsigned long long g_trace_epi[16];
 #define TRACE(i) do { } while (0)
 #define TRACE_TILE(k, i) do { } while (0)
 #endif
+__device__ __forceinline__ void bar_sync_both() { asm volatile("bar.sync 3, 256;" ::: "memory"); }
 __device__ __forceinline__ void bar_sync_stream(int b) { asm volatile("bar.sync %0, 128;" ::"r"(1 + b) : "memory"); }
 __device__ __forceinline__ float ex2(float x) {             // x <= 8 here (or -inf)
   float y;
@@ -597,7 +602,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   if (warp < 4) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
     if (warp == 0 && lane == 0 && active) {
-      // ===================== TMA producer =====================
+      // ===================== TMA producer of Q and the K tiles =====================
       uint32_t kv_it = 0, piece_it = 0;
       PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
@@ -611,22 +616,37 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         }
         TRACE(2);
         for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
-          const int sk = kv_it % kStagesK, sv = kv_it % kStagesV;
+          const int sk = kv_it % kStagesK;
           const bool pref = kt < T.n_pref_tiles;
           const int row = pref ? T.kv_base_row + kt * kBN : T.lk0 + (kt - T.n_pref_tiles) * kBN;
           const CUtensorMap* mk = pref ? &map_kc : &map_knew;
-          const CUtensorMap* mv = pref ? &map_vc : &map_vnew;
           const int c1 = pref ? row : w.g, c2 = pref ? w.g : row;   // cache [g][row][d]; new rows [row][g][d]
           mbar_wait(&sm.k_empty[sk], ((kv_it / kStagesK) & 1) ^ 1);
           mbar_arrive_expect_tx(&sm.k_full[sk], kTileBytes);
           tma_load_3d(sm.k[sk][0], mk, &sm.k_full[sk], 0, c1, c2);
           tma_load_3d(sm.k[sk][1], mk, &sm.k_full[sk], 64, c1, c2);
+        }
+        ++piece_it;
+      }
+    } else if (warp == 3 && lane == 0 && active) {
+      // ===================== TMA producer of the V tiles =====================
+      // (its own thread: a V stage is freed by P.V, long after the K stage of the same step, and K loads
+      // must not queue behind it)
+      uint32_t kv_it = 0;
+      PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
+      while (w.next()) {
+        const TileRec& T = w.T;
+        for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
+          const int sv = kv_it % kStagesV;
+          const bool pref = kt < T.n_pref_tiles;
+          const int row = pref ? T.kv_base_row + kt * kBN : T.lk0 + (kt - T.n_pref_tiles) * kBN;
+          const CUtensorMap* mv = pref ? &map_vc : &map_vnew;
+          const int c1 = pref ? row : w.g, c2 = pref ? w.g : row;
           mbar_wait(&sm.v_empty[sv], ((kv_it / kStagesV) & 1) ^ 1);
           mbar_arrive_expect_tx(&sm.v_full[sv], kTileBytes);
           tma_load_3d(sm.v[sv][0], mv, &sm.v_full[sv], 0, c1, c2);
           tma_load_3d(sm.v[sv][1], mv, &sm.v_full[sv], 64, c1, c2);
         }
-        ++piece_it;
       }
     } else if ((warp == 1 || warp == 2) && active) {
       // ===================== MMA issuers: warp 1 for stream A, warp 2 for stream B =====================
@@ -642,8 +662,10 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
       const uint32_t idesc_pv = make_idesc_bf16(kBM, kD, 0, 1);
       // every descriptor is a constant plus a small address offset: build the bases once
-      const uint64_t dq0 = make_desc_sw128(smem_u32(sm.q[b][0]), 16, 1024);
-      const uint64_t dq1 = make_desc_sw128(smem_u32(sm.q[b][1]), 16, 1024);
+      const uint64_t dq_own0 = make_desc_sw128(smem_u32(sm.q[b][0]), 16, 1024);
+      const uint64_t dq_own1 = make_desc_sw128(smem_u32(sm.q[b][1]), 16, 1024);
+      const uint64_t dq_a0 = make_desc_sw128(smem_u32(sm.q[0][0]), 16, 1024);
+      const uint64_t dq_a1 = make_desc_sw128(smem_u32(sm.q[0][1]), 16, 1024);
       const uint64_t dk = make_desc_sw128(smem_u32(sm.k[0][0]), 16, 1024);               // + stage * (16 KB >> 4) + half * (8 KB >> 4)
       const uint64_t dv = make_desc_sw128(smem_u32(sm.v[0][0]), kKvHalfBytes, 1024);     // + stage * (16 KB >> 4)
       uint32_t kv_it = 0, piece_it = 0;
@@ -652,20 +674,24 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
+        const bool alt = w.T.n_tok <= p.tpt;               // one sub-tile: both streams work on Q of sub-tile A
+        const uint64_t dq0 = alt ? dq_a0 : dq_own0, dq1 = alt ? dq_a1 : dq_own1;
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
         if (b == 0 && leader) TRACE(3);
         int owed0 = 0, owed1 = 0;              // steps (of the piece) of the up to two key tiles whose P.V is owed, oldest first
+        bool solo0 = false, solo1 = false;     // ... and whether this stream is the only one working on that key tile
         bool first = true;
-        // O_b (+)= P . V of the oldest owed key tile
+        // O_b (+)= P . V of the oldest owed key tile.  The K/V stage barriers expect two arrivals per
+        // step: one from each issuer, or both from the only stream that takes part in the step.
 #define AL_ISSUE_PV()                                                                                          \
         do {                                                                                                   \
           const uint32_t it_ = kv_it + owed0;                                                                  \
           const int sv_ = it_ % kStagesV;                                                                      \
           const uint32_t u_ = c_pv % kSBuf;                                                                    \
-          if (leader) TRACE_TILE(8 + b, it_);                                                                              \
+          if (leader) TRACE_TILE(8 + b, it_);                                                                  \
           mbar_wait(&sm.p_full[b][u_], (c_pv / kSBuf) & 1);                                                    \
-          if (leader) TRACE_TILE(10 + b, it_);                                                                             \
+          if (leader) TRACE_TILE(10 + b, it_);                                                                 \
           mbar_wait(&sm.v_full[sv_], (it_ / kStagesV) & 1);                                                    \
           if (leader && b == 0) TRACE_TILE(14, it_);                                                           \
           /* O_b of the stream's previous piece has been read out.  Only pieces in which the stream had     */ \
@@ -681,43 +707,48 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           _Pragma("unroll")                                                                                    \
           for (int k = 0; k < kBN / 16; ++k)                                                                   \
             if (leader && k < ksteps_) mma_ts(to, ts + u_ * kBN + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
-          if (leader) { mma_commit(&sm.v_empty[sv_]); mma_commit(&sm.pv_done[b]); }                            \
-          if (leader) TRACE_TILE(3 + 4 * b, it_);                                                                          \
-          first = false; ++c_pv; owed0 = owed1;                                                                \
+          if (leader) {                                                                                        \
+            mma_commit(&sm.v_empty[sv_]);                                                                      \
+            if (solo0) mma_commit(&sm.v_empty[sv_]);                                                           \
+            mma_commit(&sm.pv_done[b]);                                                                        \
+          }                                                                                                    \
+          if (leader) TRACE_TILE(3 + 4 * b, it_);                                                              \
+          first = false; ++c_pv; owed0 = owed1; solo0 = solo1;                                                 \
         } while (0)
         for (int i = 0; i < n; ++i) {
+          const int kt = w.kt_begin + i;
+          if (!takes_part(w.T, p.tpt, b, kt)) continue;      // the other issuer hands this step's stages back
+          const bool solo = !takes_part(w.T, p.tpt, b ^ 1, kt);
           const uint32_t it = kv_it + i;
-          const int sk = it % kStagesK, sv = it % kStagesV;
+          const int sk = it % kStagesK;
+          // The producer issues K(i) only after V(i-1), whose stage V(i-1-kStagesV) used: everything owed
+          // from that far back has to be paid before waiting for K(i).
+          while (c_qk != c_pv && owed0 + kStagesV < i) AL_ISSUE_PV();
           if (leader && b == 0) TRACE_TILE(12, it);
           mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
           if (leader && b == 0) TRACE_TILE(13, it);
-          if (takes_part(w.T, p.tpt, b, w.kt_begin + i)) {   // ---- S_b[u] = Q_b . K^T of step i
-            if (c_qk - c_pv == kSBuf) AL_ISSUE_PV();         // frees the S buffer this Q.K^T writes (P aliases S)
-            tc_fence_after();
-            if (b == 0 && leader) TRACE(4);
-            const uint32_t u = c_qk % kSBuf;
-            const uint64_t dk0 = dk + (uint64_t)(sk * (kTileBytes >> 4)), dk1 = dk0 + (uint64_t)(kKvHalfBytes >> 4);
+          // ---- S_b[u] = Q_b . K^T of step i
+          if (c_qk - c_pv == kSBuf) AL_ISSUE_PV();           // frees the S buffer this Q.K^T writes (P aliases S)
+          tc_fence_after();
+          if (b == 0 && leader) TRACE(4);
+          const uint32_t u = c_qk % kSBuf;
+          const uint64_t dk0 = dk + (uint64_t)(sk * (kTileBytes >> 4)), dk1 = dk0 + (uint64_t)(kKvHalfBytes >> 4);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+          for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
-            if (leader) { mma_commit(&sm.s_full[b][u]); mma_commit(&sm.k_empty[sk]); }
-            if (leader) TRACE_TILE(4 * b, it);
-            if (c_qk == c_pv) owed0 = i; else owed1 = i;
-            ++c_qk;
-          } else {
-            // not this stream's step: pay what is owed (a V stage is reused four steps later), then hand
-            // both stages back -- but only once they have landed, so that this thread can never be two
-            // stage phases ahead of the other issuer
-            while (c_qk != c_pv) AL_ISSUE_PV();
-            if (leader) mma_commit(&sm.k_empty[sk]);
-            mbar_wait(&sm.v_full[sv], (it / kStagesV) & 1);
-            if (leader) mma_commit(&sm.v_empty[sv]);
+          for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+          if (leader) {
+            mma_commit(&sm.s_full[b][u]);
+            mma_commit(&sm.k_empty[sk]);
+            if (solo) mma_commit(&sm.k_empty[sk]);
           }
-          if (leader && i == n - 1) mma_commit(&sm.q_empty);
+          if (leader) TRACE_TILE(4 * b, it);
+          if (c_qk == c_pv) { owed0 = i; solo0 = solo; } else { owed1 = i; solo1 = solo; }   // at most kSBuf (<= 2) key tiles are owed
+          ++c_qk;
         }
+        if (leader) mma_commit(&sm.q_empty);                 // this issuer's Q.K^T of the piece are all issued
         while (c_qk != c_pv) AL_ISSUE_PV();
-        if (leader && !first) mma_commit(&sm.o_full[b]);               // the piece's accumulator is complete
+        if (leader && !first) mma_commit(&sm.o_full[b]);     // the piece's accumulator is complete
 #undef AL_ISSUE_PV
         if (b == 0 && leader) TRACE(5);
         kv_it += n;
@@ -743,10 +774,12 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     while (w.next()) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
-      const int n_rows = sub_rows(p, T, b);
+      const bool alt = T.n_tok <= p.tpt;               // one sub-tile: this stream takes every other key tile of it
+      const int sb = alt ? 0 : b;                      // sub-tile whose rows this stream holds
+      const int n_rows = sub_rows(p, T, sb);
       // ---- this row's token and lane ----
       const int tok_local = r / p.n_rep;
-      const int tok = T.q_tok0 + b * p.tpt + tok_local;
+      const int tok = T.q_tok0 + sb * p.tpt + tok_local;
       bool valid = r < n_rows;
       int prefix_len = 0, ls = 0, le = 0;
       if (valid) {
@@ -877,6 +910,74 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
       const bool whole = w.whole();
       const int slot = 2 * (int)blockIdx.x + (w.kt_begin == 0 ? 1 : 0);
+      bool do_ticket = !whole && n_rows > 0;           // a piece of a split item: publish, count, maybe merge
+      if (alt) {
+        // ---- one sub-tile, two streams (even / odd key tiles): merge them, each storing 64 columns ----
+        if (tid128 == 0) sm.alt_has[b] = n_mine > 0;
+        *reinterpret_cast<float2*>(my_stage) = make_float2(m_used, l_sum);   // exchanged through the staging rows
+        bar_sync_both();
+        const float2 oth = *reinterpret_cast<const float2*>(sm.stage + ((b ^ 1) * kBM + r) * kStagePitch);
+        const bool has0 = sm.alt_has[0] != 0, has1 = sm.alt_has[1] != 0;
+        const float m0 = b ? oth.x : m_used, l0 = b ? oth.y : l_sum;
+        const float m1 = b ? m_used : oth.x, l1 = b ? l_sum : oth.y;
+        const float M = fmaxf(m0, m1);
+        const float w0 = l0 > 0.f ? ex2((m0 - M) * p.scale_log2) : 0.f;
+        const float w1 = l1 > 0.f ? ex2((m1 - M) * p.scale_log2) : 0.f;
+        const float L = w0 * l0 + w1 * l1;
+        const float rL = L > 0.f ? 1.0f / L : 0.f;
+        const float f0 = w0 * rL, f1 = w1 * rL;
+        const float lse2 = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
+        bar_sync_both();                               // the exchanged values have been read: the rows may be staged over
+        *reinterpret_cast<uint32_t*>(my_stage + 128) =
+            whole ? (uint32_t)(out_row(p, T, w.g, 0, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
+        const uint32_t t_o0 = tmem + 256, t_o1 = tmem + 384;
+        float* prow0 = p.plan.part_o + ((long long)slot * 2) * kBM * kD;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {                  // this stream's columns [64 b + 32 c, +32)
+          float o[32];
+#pragma unroll
+          for (int e = 0; e < 32; ++e) o[e] = 0.f;
+          if (has0) {                                  // warp-uniform
+            float a[32];
+            tmem_ld32_f(t_o0 + lane_addr + b * 64 + c * 32, a);
+            tmem_wait_ld();
+#pragma unroll
+            for (int e = 0; e < 32; ++e) o[e] = f0 > 0.f ? a[e] * f0 : 0.f;
+          }
+          if (has1) {
+            float a[32];
+            tmem_ld32_f(t_o1 + lane_addr + b * 64 + c * 32, a);
+            tmem_wait_ld();
+#pragma unroll
+            for (int e = 0; e < 32; ++e) o[e] = f1 > 0.f ? fmaf(a[e], f1, o[e]) : o[e];
+          }
+          if (whole) {                                 // bf16: both chunks make one 128-byte round
+            uint2* dst = reinterpret_cast<uint2*>(my_stage + c * 64);
+#pragma unroll
+            for (int e = 0; e < 8; ++e)
+              dst[e] = make_uint2(pack_bf16x2(o[4 * e], o[4 * e + 1]), pack_bf16x2(o[4 * e + 2], o[4 * e + 3]));
+            if (c == 1) {
+              __syncwarp();
+              copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + b * 128);
+              __syncwarp();
+            }
+          } else {                                     // fp32 partial (rows of sub-tile 0): one round per chunk
+            uint2* dst = reinterpret_cast<uint2*>(my_stage);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) dst[e] = make_uint2(__float_as_uint(o[2 * e]), __float_as_uint(o[2 * e + 1]));
+            __syncwarp();
+            copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + (b * 64 + c * 32) * 4);
+            __syncwarp();
+          }
+        }
+        if (whole && b == 0 && valid && p.lse) p.lse[out_row(p, T, w.g, 0, r)] = lse2;
+        if (do_ticket && b == 0) p.plan.part_lse[((long long)slot * 2) * kBM + r] = valid ? lse2 : -INFINITY;
+        if (do_ticket) __threadfence();
+        tc_fence_before();
+        bar_sync_both();                               // both streams have read both accumulators (and published)
+        if (n_mine > 0) mbar_arrive(&sm.o_empty[b]);
+        do_ticket = do_ticket && b == 0;               // stream 0 counts and merges for the tile
+      } else {
       // global offset of this row's output in units of 128 bytes, for the copy loop (pad of the staging row)
       *reinterpret_cast<uint32_t*>(my_stage + 128) =
           whole ? (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
@@ -925,10 +1026,13 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           __syncwarp();
         }
       }
-      if (tid128 == 0 && b == 0) TRACE(9);
-      if (!whole && n_rows > 0) {
+      if (do_ticket) {
         p.plan.part_lse[((long long)slot * 2 + b) * kBM + r] = (valid && n_mine > 0) ? lse : -INFINITY;
         __threadfence();
+      }
+      }
+      if (tid128 == 0 && b == 0) TRACE(9);
+      if (do_ticket) {
         bar_sync_stream(b);
         if (tid128 == 0 && b == 0) TRACE(10);
         if (tid128 == 0) {
