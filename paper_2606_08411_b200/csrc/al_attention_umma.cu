@@ -83,6 +83,8 @@ struct __align__(16) CtaRec {              // 96 bytes
 };
 struct PlanHeader {
   int n_tiles, n_items, k_total, n_ctas;
+  int alt;           // tiles of one sub-tile are worked on by both streams (chosen with the whole-item mode)
+  int pad[3];
 };
 
 struct Plan {
@@ -281,6 +283,9 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   if (tid == 0) {
     plan.hdr->n_tiles = n_tiles; plan.hdr->n_items = n_tiles * n_kv_heads;
     plan.hdr->k_total = k_total; plan.hdr->n_ctas = k_total > 0 ? n_ctas : 0;
+    // with one item per CTA a single-sub-tile item would leave half of the CTA's softmax threads idle;
+    // under stream-K the CTAs have long mixed ranges and the merge of the two streams does not pay
+    plan.hdr->alt = whole_items ? 1 : 0;
   }
 }
 
@@ -361,8 +366,8 @@ struct PieceWalk {
 // always; local tiles: only those that hold rows of the lanes the sub-tile's tokens belong to).  One
 // sub-tile ("alt" mode): even key tiles go to stream 0, odd ones to stream 1, each with its own running
 // max, row sum and accumulator; the epilogue merges the two.
-__device__ __forceinline__ bool takes_part(const TileRec& T, int tpt, int b, int kt) {
-  if (T.n_tok <= tpt) return (kt & 1) == b;  // a tile of one sub-tile: the two streams take alternate key tiles of it
+__device__ __forceinline__ bool takes_part(const TileRec& T, int tpt, int b, int kt, bool alt_ok) {
+  if (alt_ok && T.n_tok <= tpt) return (kt & 1) == b;  // a tile of one sub-tile: the two streams take alternate key tiles of it
   if (b * tpt >= T.n_tok) return false;
   if (kt < T.n_pref_tiles) return true;
   const int k0 = T.lk0 + (kt - T.n_pref_tiles) * kBN;
@@ -553,50 +558,16 @@ __device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, int n_rows
     if (r0 + it * 2 < n_rows) *reinterpret_cast<uint2*>(base + (size_t)off[it] * 128 + (lane & 15) * 8) = v[it];
 }
 
-__global__ void __launch_bounds__(kThreads, 1)
-lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_knew,
-                           const __grid_constant__ CUtensorMap map_vnew, const __grid_constant__ CUtensorMap map_kc,
-                           const __grid_constant__ CUtensorMap map_vc, const AttnParams p) {
-  extern __shared__ __align__(1024) uint8_t smem_raw[];
-  AttnSmem& sm = *reinterpret_cast<AttnSmem*>(smem_raw);
-  // the shuffle tells the compiler that `warp` is warp-uniform: the role branches and everything derived
-  // from it (stream index, TMEM and shared-memory descriptors) then live in uniform registers
-  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-
-#ifdef AL_ATTN_TRACE
-  if (threadIdx.x == 0) {
-    if (blockIdx.x == 0 || blockIdx.x == 12) for (int i = (blockIdx.x ? 11 : 0); i < (blockIdx.x ? 16 : 11); ++i) g_trace_epi[i] = 0;
-    for (int i = 0; i < 16; ++i) g_trace[blockIdx.x * 16 + i] = 0;
-    unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-    g_trace[blockIdx.x * 16 + 15] = gt;
-    g_trace[blockIdx.x * 16 + 0] = clock64();
-  }
-#endif
-  if (threadIdx.x == 0) {
-    if (smem_u32(smem_raw) & 1023u) __trap();          // the 128-byte swizzle atoms need 1024-byte alignment
-    mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 2);       // the *_empty barriers collect both MMA issuers
-    for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 2); }
-    for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 2); }
-    for (int b = 0; b < 2; ++b) {
-      for (int u = 0; u < kSBuf; ++u) { mbar_init(&sm.s_full[b][u], 1); mbar_init(&sm.p_full[b][u], 128); }
-      mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_full[b], 1); mbar_init(&sm.o_empty[b], 128);
-    }
-    fence_barrier_init();
-    prefetch_tensormap(&map_q); prefetch_tensormap(&map_knew); prefetch_tensormap(&map_vnew);
-    prefetch_tensormap(&map_kc); prefetch_tensormap(&map_vc);
-  }
-  if (warp == 1) tmem_alloc<512>(&sm.tmem_base);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = sm.tmem_base;
-  // TMEM columns: S of stream b, buffer u at (2 b + u) * 64; O of stream b at 256 + 128 b
-  // programmatic dependent launch: everything above overlapped the previous kernel in the stream (the
-  // plan, or the previous layer); its memory is visible after the wait.  The next launch in the stream
-  // that opts in (the next layer) may then begin its own prologue as SMs free up.
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+// The role code of the kernel, compiled twice: with and without the "alt" mode (one sub-tile worked on
+// by both streams).  The plan chooses per launch; keeping the alt code out of the other instance keeps
+// its hot loops as lean as they were (measured: 8 us of 108 at cfg5).
+template <bool kAltOk>
+__device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, const CUtensorMap* pmap_q,
+                                           const CUtensorMap* pmap_knew, const CUtensorMap* pmap_vnew,
+                                           const CUtensorMap* pmap_kc, const CUtensorMap* pmap_vc, uint32_t tmem,
+                                           int warp, int lane) {
   const bool active = (int)blockIdx.x < p.plan.hdr->n_ctas;
+  constexpr bool alt_ok = kAltOk;
   if (threadIdx.x == 0) TRACE(1);
 
   if (warp < 4) {
@@ -608,26 +579,37 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       while (w.next()) {
         const TileRec& T = w.T;
         const bool two = T.n_tok > p.tpt;
-        mbar_wait(&sm.q_empty, (piece_it & 1) ^ 1);
+        mbar_wait_relaxed(&sm.q_empty, (piece_it & 1) ^ 1);
         mbar_arrive_expect_tx(&sm.q_full, two ? 2 * p.q_box_bytes : p.q_box_bytes);   // a box is tpt*n_rep (<= 128) rows per half
         for (int b = 0; b < (two ? 2 : 1); ++b) {
-          tma_load_3d(sm.q[b][0], &map_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
-          tma_load_3d(sm.q[b][1], &map_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
+          tma_load_3d(sm.q[b][0], pmap_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
+          tma_load_3d(sm.q[b][1], pmap_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
         }
         TRACE(2);
         for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
           const int sk = kv_it % kStagesK;
           const bool pref = kt < T.n_pref_tiles;
           const int row = pref ? T.kv_base_row + kt * kBN : T.lk0 + (kt - T.n_pref_tiles) * kBN;
-          const CUtensorMap* mk = pref ? &map_kc : &map_knew;
+          const CUtensorMap* mk = pref ? pmap_kc : pmap_knew;
           const int c1 = pref ? row : w.g, c2 = pref ? w.g : row;   // cache [g][row][d]; new rows [row][g][d]
-          mbar_wait(&sm.k_empty[sk], ((kv_it / kStagesK) & 1) ^ 1);
+          mbar_wait_relaxed(&sm.k_empty[sk], ((kv_it / kStagesK) & 1) ^ 1);
           mbar_arrive_expect_tx(&sm.k_full[sk], kTileBytes);
           tma_load_3d(sm.k[sk][0], mk, &sm.k_full[sk], 0, c1, c2);
           tma_load_3d(sm.k[sk][1], mk, &sm.k_full[sk], 64, c1, c2);
+#ifdef AL_ONE_PRODUCER
+          {
+            const int sv = kv_it % kStagesV;
+            const CUtensorMap* mv = pref ? pmap_vc : pmap_vnew;
+            mbar_wait_relaxed(&sm.v_empty[sv], ((kv_it / kStagesV) & 1) ^ 1);
+            mbar_arrive_expect_tx(&sm.v_full[sv], kTileBytes);
+            tma_load_3d(sm.v[sv][0], mv, &sm.v_full[sv], 0, c1, c2);
+            tma_load_3d(sm.v[sv][1], mv, &sm.v_full[sv], 64, c1, c2);
+          }
+#endif
         }
         ++piece_it;
       }
+#ifndef AL_ONE_PRODUCER
     } else if (warp == 3 && lane == 0 && active) {
       // ===================== TMA producer of the V tiles =====================
       // (its own thread: a V stage is freed by P.V, long after the K stage of the same step, and K loads
@@ -640,14 +622,15 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
           const int sv = kv_it % kStagesV;
           const bool pref = kt < T.n_pref_tiles;
           const int row = pref ? T.kv_base_row + kt * kBN : T.lk0 + (kt - T.n_pref_tiles) * kBN;
-          const CUtensorMap* mv = pref ? &map_vc : &map_vnew;
+          const CUtensorMap* mv = pref ? pmap_vc : pmap_vnew;
           const int c1 = pref ? row : w.g, c2 = pref ? w.g : row;
-          mbar_wait(&sm.v_empty[sv], ((kv_it / kStagesV) & 1) ^ 1);
+          mbar_wait_relaxed(&sm.v_empty[sv], ((kv_it / kStagesV) & 1) ^ 1);
           mbar_arrive_expect_tx(&sm.v_full[sv], kTileBytes);
           tma_load_3d(sm.v[sv][0], mv, &sm.v_full[sv], 0, c1, c2);
           tma_load_3d(sm.v[sv][1], mv, &sm.v_full[sv], 64, c1, c2);
         }
       }
+#endif
     } else if ((warp == 1 || warp == 2) && active) {
       // ===================== MMA issuers: warp 1 for stream A, warp 2 for stream B =====================
       // Per stream S is double-buffered (2 x 64 TMEM columns; P aliases S), so Q.K^T runs two key tiles
@@ -674,7 +657,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
-        const bool alt = w.T.n_tok <= p.tpt;               // one sub-tile: both streams work on Q of sub-tile A
+        const bool alt = alt_ok && w.T.n_tok <= p.tpt;     // one sub-tile: both streams work on Q of sub-tile A
         const uint64_t dq0 = alt ? dq_a0 : dq_own0, dq1 = alt ? dq_a1 : dq_own1;
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
@@ -717,10 +700,23 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
         } while (0)
         for (int i = 0; i < n; ++i) {
           const int kt = w.kt_begin + i;
-          if (!takes_part(w.T, p.tpt, b, kt)) continue;      // the other issuer hands this step's stages back
-          const bool solo = !takes_part(w.T, p.tpt, b ^ 1, kt);
           const uint32_t it = kv_it + i;
           const int sk = it % kStagesK;
+          // A step only one stream works on: in alt mode (every step is one) its issuer arrives twice on
+          // the stage barriers and the other issuer skips the step; with two sub-tiles (local key tiles
+          // of one sub-tile's lanes only -- few) the idle issuer pays what it owes and hands the stages
+          // back itself, once they have landed, which keeps the two issuers within a stage phase.
+          const bool solo = alt;
+          if (!takes_part(w.T, p.tpt, b, kt, alt_ok)) {
+            if (!alt) {
+              while (c_qk != c_pv) AL_ISSUE_PV();
+              mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
+              if (leader) mma_commit(&sm.k_empty[sk]);
+              mbar_wait(&sm.v_full[it % kStagesV], (it / kStagesV) & 1);
+              if (leader) mma_commit(&sm.v_empty[it % kStagesV]);
+            }
+            continue;
+          }
           // The producer issues K(i) only after V(i-1), whose stage V(i-1-kStagesV) used: everything owed
           // from that far back has to be paid before waiting for K(i).
           while (c_qk != c_pv && owed0 + kStagesV < i) AL_ISSUE_PV();
@@ -774,7 +770,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     while (w.next()) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
-      const bool alt = T.n_tok <= p.tpt;               // one sub-tile: this stream takes every other key tile of it
+      const bool alt = alt_ok && T.n_tok <= p.tpt;     // one sub-tile: this stream takes every other key tile of it
       const int sb = alt ? 0 : b;                      // sub-tile whose rows this stream holds
       const int n_rows = sub_rows(p, T, sb);
       // ---- this row's token and lane ----
@@ -794,7 +790,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
 
       for (int i = 0; i < n; ++i) {
         const int kt = w.kt_begin + i;
-        if (!takes_part(T, p.tpt, b, kt)) continue;
+        if (!takes_part(T, p.tpt, b, kt, alt_ok)) continue;
         const uint32_t u = cnt % kSBuf;                  // S buffer of this key tile
         const uint32_t t_s = tmem + b * 128 + u * kBN;
         mbar_wait(&sm.s_full[b][u], (cnt / kSBuf) & 1);
@@ -1057,6 +1053,53 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
       }
     }
   }
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_knew,
+                           const __grid_constant__ CUtensorMap map_vnew, const __grid_constant__ CUtensorMap map_kc,
+                           const __grid_constant__ CUtensorMap map_vc, const AttnParams p) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  AttnSmem& sm = *reinterpret_cast<AttnSmem*>(smem_raw);
+  // the shuffle tells the compiler that `warp` is warp-uniform: the role branches and everything derived
+  // from it (stream index, TMEM and shared-memory descriptors) then live in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+
+#ifdef AL_ATTN_TRACE
+  if (threadIdx.x == 0) {
+    if (blockIdx.x == 0 || blockIdx.x == 12) for (int i = (blockIdx.x ? 11 : 0); i < (blockIdx.x ? 16 : 11); ++i) g_trace_epi[i] = 0;
+    for (int i = 0; i < 16; ++i) g_trace[blockIdx.x * 16 + i] = 0;
+    unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+    g_trace[blockIdx.x * 16 + 15] = gt;
+    g_trace[blockIdx.x * 16 + 0] = clock64();
+  }
+#endif
+  if (threadIdx.x == 0) {
+    if (smem_u32(smem_raw) & 1023u) __trap();          // the 128-byte swizzle atoms need 1024-byte alignment
+    mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 2);       // the *_empty barriers collect both MMA issuers
+    for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 2); }
+    for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 2); }
+    for (int b = 0; b < 2; ++b) {
+      for (int u = 0; u < kSBuf; ++u) { mbar_init(&sm.s_full[b][u], 1); mbar_init(&sm.p_full[b][u], 128); }
+      mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_full[b], 1); mbar_init(&sm.o_empty[b], 128);
+    }
+    fence_barrier_init();
+    prefetch_tensormap(&map_q); prefetch_tensormap(&map_knew); prefetch_tensormap(&map_vnew);
+    prefetch_tensormap(&map_kc); prefetch_tensormap(&map_vc);
+  }
+  if (warp == 1) tmem_alloc<512>(&sm.tmem_base);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = sm.tmem_base;
+  // TMEM columns: S of stream b, buffer u at (2 b + u) * 64; O of stream b at 256 + 128 b
+  // programmatic dependent launch: everything above overlapped the previous kernel in the stream (the
+  // plan, or the previous layer); its memory is visible after the wait.  The next launch in the stream
+  // that opts in (the next layer) may then begin its own prologue as SMs free up.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  if (p.plan.hdr->alt) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, tmem, warp, lane);
+  else attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, tmem, warp, lane);
   tc_fence_before();
   __syncthreads();
   if (threadIdx.x == 0) TRACE(13);
