@@ -12,8 +12,9 @@ What is timed (DESIGN.md "Measurement"):
   value     K steps, inputs resident in HBM, each step one CUDA-graph replay; consecutive steps run
             on DISTINCT copies of every streamed buffer (rotation set > 2x L2) so nothing is served
             from L2.  Device time from CUDA events on the launching stream, max over ranks.
-  roofline  per-part device time from timing events captured INSIDE those graphs (external event
-            record nodes), read for the last replay of every copy in the timed region.
+  roofline  per-part device time: every part (attention = plan + all layers, refresh, confidence) has
+            its own graph per copy, replayed over the same rotation right after the timed region and
+            timed with CUDA events on the stream.
   e2e       the same step through the C-ABI host entry al_lane_step_host: every step copies its
             inputs from pinned host memory, runs the kernels and copies the results back.
   cpu_baseline / --impl reference   the CPU oracle (oracle/, fp64, as it stands) on the host cores.
@@ -202,22 +203,31 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     copies = [first] + [first.replicate() for _ in range(n_copies - 1)]
     stream = torch.cuda.Stream(device=dev)
 
-    # ---- one CUDA graph per copy, timing marks captured as external event-record nodes ---------
-    graphs, marks = [], []
+    # ---- one CUDA graph of the whole step per copy, plus one graph per part for the part times ------
+    graphs, marked_graphs = [], []
     launches_per_step = None
     stream.wait_stream(torch.cuda.current_stream())
     with torch.cuda.stream(stream):
         copies[0].run(stream)                                  # load modules / set attributes before capture
         stream.synchronize()
         for st in copies:
-            ev = [torch.cuda.Event(enable_timing=True, external=True) for _ in range(4)] if args.kernel_events else None
-            g = torch.cuda.CUDAGraph()
+            g = torch.cuda.CUDAGraph()                         # the step as a user runs it: kernels only
             before = h.al_launch_count
             with torch.cuda.graph(g, stream=stream):
-                st.run(stream, marks=ev)
+                st.run(stream)
             launches_per_step = h.al_launch_count - before
             graphs.append(g)
-            marks.append(ev)
+            # one graph per part (attention = plan + every layer, refresh, confidence) for the per-part
+            # times: event nodes inside the step graph would cost a few us per step and break the
+            # programmatic-dependent-launch edges between the kernels
+            if args.kernel_events:
+                pg = {}
+                for name, fn in (("attention", st.attention), ("refresh", st.refresh), ("confidence", st.confidence)):
+                    gp = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(gp, stream=stream):
+                        fn(stream)
+                    pg[name] = gp
+                marked_graphs.append(pg)
     stream.synchronize()
 
     sampler = ClockSampler(local_rank)
@@ -245,13 +255,25 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     sampler.active.clear()
     step_ms = e0.elapsed_time(e1) / args.steps
 
-    # per-part device times: the marks of every copy hold its LAST replay inside the timed region
+    # per-part device times: right after the timed region, every part's own graph is replayed over the
+    # same rotation of copies (so its inputs come from HBM, not L2) and timed with CUDA events on the stream
     part_ms = None
     if args.kernel_events:
-        used = [c for c in range(n_copies) if c < args.steps]
-        a = np.array([[marks[c][j].elapsed_time(marks[c][j + 1]) for j in range(3)] for c in used])
-        part_ms = dict(zip(("attention", "refresh", "confidence"), a.mean(axis=0).tolist()))
-        part_ms["n_samples"] = len(used)
+        reps = max(4 * n_copies, 40)
+        part_ms = {}
+        sampler.active.set()
+        for name in ("attention", "refresh", "confidence"):
+            with torch.cuda.stream(stream):
+                for i in range(n_copies):
+                    marked_graphs[i % n_copies][name].replay()
+                e0.record(stream)
+                for i in range(reps):
+                    marked_graphs[i % n_copies][name].replay()
+                e1.record(stream)
+            barrier()
+            part_ms[name] = e0.elapsed_time(e1) / reps
+        sampler.active.clear()
+        part_ms["n_samples"] = reps
 
     t = torch.tensor([step_ms], dtype=torch.float64, device=dev)
     if dist is not None:
@@ -352,7 +374,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         dom = max(parts, key=lambda k: parts[k]["ms"])
         roofline = {k: parts[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")}
         roofline.update(kernel=dom, peak_source=peaks["source"], avg_launch_ms=parts[dom]["ms"] / parts[dom]["launches"],
-                        timed_with="CUDA events captured in the step graphs, last replay of each copy in the timed region")
+                        timed_with="CUDA events on the stream around replays of the part's own graph over the same rotating copies, right after the timed region")
     else:
         roofline = None
 

@@ -218,6 +218,10 @@ confidence_select_kernel(const T* __restrict__ logits, int n_rows, int vocab, lo
   constexpr int E = Vec<T>::kElems;
   __shared__ Triple s_warp[kWarps];
   __shared__ Triple s_cta[kMaxCluster];                    // leader CTA: one slot per cluster rank
+  // programmatic dependent launch: overlaps the launch with the tail of the previous kernel in the
+  // stream; everything that kernel wrote (the logits, in a real step) is visible after the wait
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int row = blockIdx.x / k_cluster;
   const int rank = blockIdx.x - row * k_cluster;
@@ -350,13 +354,15 @@ cudaError_t launch_select(int k, int n_rows, cudaStream_t cs, const T* logits, i
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = 0;
   cfg.stream = cs;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = (unsigned)k;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.wait in the kernel
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   return cudaLaunchKernelEx(&cfg, confidence_select_kernel<T, kVector>, logits, n_rows, vocab, row_stride, k, eos_id,
                             lanes, n_lanes, out);
 }

@@ -28,6 +28,11 @@ kv_refresh_kernel(int4* __restrict__ k_cache, int4* __restrict__ v_cache,
                   const int32_t* __restrict__ pos, int n_pos, int kv_base_row, int n_kv_heads,
                   long long cache_rows, int vecs_per_row, long long layer_stride_cache_vecs,
                   long long layer_stride_src_vecs, long long items_per_layer, long long total_items) {
+  // programmatic dependent launch: the launch overlaps the tail of the previous kernel in the stream
+  // (the attention that still reads the cache rows this kernel overwrites); its memory operations are
+  // complete and visible after the wait.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const long long stride = (long long)gridDim.x * kThreads;
   long long i0 = (long long)blockIdx.x * kThreads + threadIdx.x;
   for (; i0 < total_items; i0 += stride * kUnroll) {
@@ -90,10 +95,18 @@ extern "C" al_status al_kv_refresh(al_handle* h, const al_attn_shape* s, void* k
   const long long cap = (long long)h->sm_count * 16;       // grid-stride beyond 16 CTAs per SM
   if (blocks > cap) blocks = cap;
   h->launches++;
-  kv_refresh_kernel<<<(unsigned)blocks, kThreads, 0, static_cast<cudaStream_t>(stream)>>>(
-      (int4*)k_cache, (int4*)v_cache, (const int4*)k_src, (const int4*)v_src, pos_dev, n_pos,
-      kv_base_row, s->n_kv_heads, (long long)s->cache_rows, vpr, layer_stride_cache * esz / 16,
-      layer_stride_src * esz / 16, items_per_layer, total);
-  AL_CUDA_OK(cudaGetLastError());
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)blocks);
+  cfg.blockDim = dim3(kThreads);
+  cfg.stream = static_cast<cudaStream_t>(stream);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.wait in the kernel
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, kv_refresh_kernel, (int4*)k_cache, (int4*)v_cache, (const int4*)k_src,
+                                (const int4*)v_src, pos_dev, (int)n_pos, (int)kv_base_row, (int)s->n_kv_heads,
+                                (long long)s->cache_rows, vpr, (long long)(layer_stride_cache * esz / 16),
+                                (long long)(layer_stride_src * esz / 16), items_per_layer, total));
   return AL_OK;
 }
