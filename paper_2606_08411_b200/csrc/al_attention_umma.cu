@@ -61,7 +61,7 @@ constexpr int kPlanThreads = 256;
 constexpr int kPlanTilesInSmem = 96;
 constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
 constexpr int kMinPiece = 256 / kBN;       // do not cut the work finer than 256 keys per CTA
-constexpr int kSplitCost = 640 / kBN;      // what splitting an item costs (partial epilogue + merge), in steps: measured ~10 us
+constexpr int kSplitCost = 1280 / kBN;     // what splitting an item costs (partial epilogue, ticket, merge by the last CTA), in steps: measured 12-20 us
 
 struct __align__(16) TileRec {             // 64 bytes
   int q_tok0, n_tok;          // first packed token row, tokens in the tile (<= 2 tpt)
