@@ -117,6 +117,22 @@ class ClockSampler(threading.Thread):
 
 
 # --------------------------------------------------------------------------------------------------
+def max_over_ranks(ms: float, dist, device) -> float:
+    """Replicas only: every rank times its own replica on its own device; the job's step time is the
+    slowest rank's (one all_reduce(MAX) of a scalar -- the only collective, and it is not on the data path)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank: float, world: int, step_ms: float) -> float:
+    """Aggregate throughput of `world` independent replicas: all ranks' units over the slowest rank's time."""
+    return world * units_per_rank / (step_ms * 1e-3)
+
+
+# --------------------------------------------------------------------------------------------------
 def oracle_step(oracle, wl, lanes, rows):
     """One pass of the hot path on the CPU oracle over whole lanes `lanes` / logits rows `rows`."""
     for layer in range(wl.n_layers):
@@ -275,11 +291,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         sampler.active.clear()
         part_ms["n_samples"] = reps
 
-    t = torch.tensor([step_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    step_ms_max = float(t.item())
-    value = world * acc["query_tokens"] / (step_ms_max * 1e-3)
+    step_ms_max = max_over_ranks(step_ms, dist, dev)
+    value = whole_job_value(acc["query_tokens"], world, step_ms_max)
 
     # ---- e2e: host buffers through al_lane_step_host ----------------------------------------------
     hs = binding.al_host_step()
@@ -334,10 +347,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     wall_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
     sampler.active.clear()
     e2e_ms = max(e0.elapsed_time(e1) / e2e_steps, wall_ms)       # host-visible completion time
-    t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, dist, dev)
     e2e_tokens = wl.total_q_rows                                  # one layer of the workload per host step
     sampler.stop_flag.set()
     sampler.join(timeout=2)
@@ -393,7 +403,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                    "l2": f"rotating {n_copies} resident copies of every streamed buffer "
                          f"({n_copies * per_copy / 1e6:.0f} MB > 2x 126 MB L2), one CUDA graph per step"},
         "clocks": sampler.summary(),
-        "e2e": {"value": world * e2e_tokens / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        "e2e": {"value": whole_job_value(e2e_tokens, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "api": "al_lane_step_host (pinned host buffers; H2D + kernels + D2H per step)",
                 "gpu_launches_per_step": e2e_launches},
