@@ -292,13 +292,14 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
 // ---------------------------------------------------------------------------------------------
 // main kernel
 // ---------------------------------------------------------------------------------------------
-constexpr int kStagePitch = 136;           // 128 data bytes + 8 pad: conflict-free 8-byte row-per-thread writes
+constexpr int kStagePitch = 128;           // 128 data bytes per staged row; 16-byte chunk c of row r sits at chunk c ^ (r & 7)
 
 struct AttnSmem {
   alignas(1024) uint8_t q[2][2][kHalfBytes];           // [sub-tile][64-column half]
   alignas(1024) uint8_t k[kStagesK][2][kKvHalfBytes];
   alignas(1024) uint8_t v[kStagesV][2][kKvHalfBytes];
-  alignas(16) uint8_t stage[2 * kBM * kStagePitch];    // epilogue staging: half row (stream b, row r) at b*128 + r
+  alignas(128) uint8_t stage[2 * kBM * kStagePitch];   // epilogue staging: 128 bytes of (stream b, row r) at row b*128 + r
+  uint32_t stage_off[2 * kBM];                         // ... and where they go: global offset in units of 128 bytes
   uint64_t q_full, q_empty;
   uint64_t k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV];
   uint64_t s_full[2][kSBuf], p_full[2][kSBuf];   // [stream][S buffer]
@@ -538,24 +539,32 @@ __device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T
   }
 }
 
-// Copies the staged 128-byte half rows [0, n_rows) of stream b to global memory with coalesced
-// 8-byte accesses: 16 lanes per half row, two half rows per warp instruction.  The 8-byte pad of a
-// staging row holds the row's global offset in units of 128 bytes (written by the row's own thread,
-// which knows its token and head), so the copy loop is address arithmetic free.
-__device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, int n_rows, int tid128, uint8_t* base) {
+// Epilogue staging.  A thread writes the 128 bytes of its own row as eight 16-byte chunks; chunk c
+// of row r is stored at chunk position c ^ (r & 7), which makes both the row-per-thread writes and the
+// chunk-per-lane reads of the copy loop conflict-free without padding.
+__device__ __forceinline__ void stage_chunk(uint8_t* my_stage, int r, int c, uint4 v) {
+  *reinterpret_cast<uint4*>(my_stage + ((c ^ (r & 7)) << 4)) = v;
+}
+// Copies the staged rows [0, n_rows) of a stream to global memory with coalesced 16-byte accesses:
+// 8 lanes per row, four rows per warp instruction; a warp copies the 32 rows its own threads staged.
+// stage_off holds each row's global offset in units of 128 bytes (written by the row's own thread,
+// which knows its token and head), so the loop is address-arithmetic free.
+__device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, const uint32_t* off_b, int n_rows, int tid128,
+                                              uint8_t* base) {
   const int warp = tid128 >> 5, lane = tid128 & 31;
-  const uint8_t* src = stage_b + (warp * 32 + (lane >> 4)) * kStagePitch + (lane & 15) * 8;
-  const int r0 = warp * 32 + (lane >> 4);
-  uint2 v[16];
-  uint32_t off[16];
+  const int chunk = lane & 7;
+  const int r0 = warp * 32 + (lane >> 3);
+  uint4 v[8];
+  uint32_t off[8];
 #pragma unroll
-  for (int it = 0; it < 16; ++it) {
-    v[it] = *reinterpret_cast<const uint2*>(src + it * 2 * kStagePitch);
-    off[it] = *reinterpret_cast<const uint32_t*>(src + it * 2 * kStagePitch - (lane & 15) * 8 + 128);
+  for (int it = 0; it < 8; ++it) {
+    const int r = r0 + it * 4;
+    v[it] = *reinterpret_cast<const uint4*>(stage_b + r * kStagePitch + ((chunk ^ (r & 7)) << 4));
+    off[it] = off_b[r];
   }
 #pragma unroll
-  for (int it = 0; it < 16; ++it)
-    if (r0 + it * 2 < n_rows) *reinterpret_cast<uint2*>(base + (size_t)off[it] * 128 + (lane & 15) * 8) = v[it];
+  for (int it = 0; it < 8; ++it)
+    if (r0 + it * 4 < n_rows) *reinterpret_cast<uint4*>(base + (size_t)off[it] * 128 + chunk * 16) = v[it];
 }
 
 // The role code of the kernel, compiled twice: with and without the "alt" mode (one sub-tile worked on
@@ -764,6 +773,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
     const uint64_t scale2 = pack2(p.scale_log2, p.scale_log2);
     uint8_t* stage_b = sm.stage + b * kBM * kStagePitch;
     uint8_t* my_stage = stage_b + r * kStagePitch;
+    uint32_t* off_b = sm.stage_off + b * kBM;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
     uint32_t pieces_done = 0;                          // pieces in which it had key tiles: o_full phase
     PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
@@ -924,7 +934,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         const float f0 = w0 * rL, f1 = w1 * rL;
         const float lse2 = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
         bar_sync_both();                               // the exchanged values have been read: the rows may be staged over
-        *reinterpret_cast<uint32_t*>(my_stage + 128) =
+        off_b[r] =
             whole ? (uint32_t)(out_row(p, T, w.g, 0, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
         const uint32_t t_o0 = tmem + 256, t_o1 = tmem + 384;
         float* prow0 = p.plan.part_o + ((long long)slot * 2) * kBM * kD;
@@ -948,21 +958,23 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             for (int e = 0; e < 32; ++e) o[e] = f1 > 0.f ? fmaf(a[e], f1, o[e]) : o[e];
           }
           if (whole) {                                 // bf16: both chunks make one 128-byte round
-            uint2* dst = reinterpret_cast<uint2*>(my_stage + c * 64);
 #pragma unroll
-            for (int e = 0; e < 8; ++e)
-              dst[e] = make_uint2(pack_bf16x2(o[4 * e], o[4 * e + 1]), pack_bf16x2(o[4 * e + 2], o[4 * e + 3]));
+            for (int e = 0; e < 4; ++e)
+              stage_chunk(my_stage, r, c * 4 + e,
+                          make_uint4(pack_bf16x2(o[8 * e], o[8 * e + 1]), pack_bf16x2(o[8 * e + 2], o[8 * e + 3]),
+                                     pack_bf16x2(o[8 * e + 4], o[8 * e + 5]), pack_bf16x2(o[8 * e + 6], o[8 * e + 7])));
             if (c == 1) {
               __syncwarp();
-              copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + b * 128);
+              copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + b * 128);
               __syncwarp();
             }
           } else {                                     // fp32 partial (rows of sub-tile 0): one round per chunk
-            uint2* dst = reinterpret_cast<uint2*>(my_stage);
 #pragma unroll
-            for (int e = 0; e < 16; ++e) dst[e] = make_uint2(__float_as_uint(o[2 * e]), __float_as_uint(o[2 * e + 1]));
+            for (int e = 0; e < 8; ++e)
+              stage_chunk(my_stage, r, e, make_uint4(__float_as_uint(o[4 * e]), __float_as_uint(o[4 * e + 1]),
+                                                     __float_as_uint(o[4 * e + 2]), __float_as_uint(o[4 * e + 3])));
             __syncwarp();
-            copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + (b * 64 + c * 32) * 4);
+            copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + (b * 64 + c * 32) * 4);
             __syncwarp();
           }
         }
@@ -975,7 +987,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         do_ticket = do_ticket && b == 0;               // stream 0 counts and merges for the tile
       } else {
       // global offset of this row's output in units of 128 bytes, for the copy loop (pad of the staging row)
-      *reinterpret_cast<uint32_t*>(my_stage + 128) =
+      off_b[r] =
           whole ? (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
       if (n_mine == 0) {
         // nothing accumulated: no key tile of this piece concerns the sub-tile (or it is empty)
@@ -990,16 +1002,16 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             tmem_ld32_f(t_o + lane_addr + rd * 64 + c * 32, o);
             tmem_wait_ld();
             if (rd == 1 && c == 1) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }   // O_b is in registers
-            uint2* dst = reinterpret_cast<uint2*>(my_stage + c * 64);
 #pragma unroll
-            for (int e = 0; e < 8; ++e)
-              dst[e] = make_uint2(pack_bf16x2(o[4 * e] * inv, o[4 * e + 1] * inv),
-                                  pack_bf16x2(o[4 * e + 2] * inv, o[4 * e + 3] * inv));
+            for (int e = 0; e < 4; ++e)
+              stage_chunk(my_stage, r, c * 4 + e,
+                          make_uint4(pack_bf16x2(o[8 * e] * inv, o[8 * e + 1] * inv), pack_bf16x2(o[8 * e + 2] * inv, o[8 * e + 3] * inv),
+                                     pack_bf16x2(o[8 * e + 4] * inv, o[8 * e + 5] * inv), pack_bf16x2(o[8 * e + 6] * inv, o[8 * e + 7] * inv)));
           }
           TRACE_E(2 + 5 * rd);
           __syncwarp();                                // a warp stages and copies its own 32 rows
           TRACE_E(3 + 5 * rd);
-          copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + rd * 128);
+          copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + rd * 128);
           TRACE_E(4 + 5 * rd);
           __syncwarp();                                // the staging rows are rewritten by the next round / piece
           TRACE_E(5 + 5 * rd);
@@ -1014,11 +1026,12 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           tmem_ld32_f(t_o + lane_addr + rd * 32, o);
           tmem_wait_ld();
           if (rd == 3) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }
-          uint2* dst = reinterpret_cast<uint2*>(my_stage);
 #pragma unroll
-          for (int e = 0; e < 16; ++e) dst[e] = make_uint2(__float_as_uint(o[2 * e] * inv), __float_as_uint(o[2 * e + 1] * inv));
+          for (int e = 0; e < 8; ++e)
+            stage_chunk(my_stage, r, e, make_uint4(__float_as_uint(o[4 * e] * inv), __float_as_uint(o[4 * e + 1] * inv),
+                                                   __float_as_uint(o[4 * e + 2] * inv), __float_as_uint(o[4 * e + 3] * inv)));
           __syncwarp();
-          copy_out_rows(stage_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + rd * 128);
+          copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + rd * 128);
           __syncwarp();
         }
       }
