@@ -881,7 +881,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             for (int e = 0; e < 16; ++e) {
               const uint64_t x2 = ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2);
               float p0, p1;
-              if ((e & 3) == 1) {                         // every fourth pair: FMA pipes instead of the MUFU
+              if ((0x52 >> (e & 7)) & 1) {                 // three pairs of eight: FMA pipes instead of the MUFU
                 exp2_poly_pair(x2, p0, p1);
               } else {
                 float t0, t1;
