@@ -605,20 +605,9 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           mbar_arrive_expect_tx(&sm.k_full[sk], kTileBytes);
           tma_load_3d(sm.k[sk][0], mk, &sm.k_full[sk], 0, c1, c2);
           tma_load_3d(sm.k[sk][1], mk, &sm.k_full[sk], 64, c1, c2);
-#ifdef AL_ONE_PRODUCER
-          {
-            const int sv = kv_it % kStagesV;
-            const CUtensorMap* mv = pref ? pmap_vc : pmap_vnew;
-            mbar_wait_relaxed(&sm.v_empty[sv], ((kv_it / kStagesV) & 1) ^ 1);
-            mbar_arrive_expect_tx(&sm.v_full[sv], kTileBytes);
-            tma_load_3d(sm.v[sv][0], mv, &sm.v_full[sv], 0, c1, c2);
-            tma_load_3d(sm.v[sv][1], mv, &sm.v_full[sv], 64, c1, c2);
-          }
-#endif
         }
         ++piece_it;
       }
-#ifndef AL_ONE_PRODUCER
     } else if (warp == 3 && lane == 0 && active) {
       // ===================== TMA producer of the V tiles =====================
       // (its own thread: a V stage is freed by P.V, long after the K stage of the same step, and K loads
@@ -639,7 +628,6 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           tma_load_3d(sm.v[sv][1], mv, &sm.v_full[sv], 64, c1, c2);
         }
       }
-#endif
     } else if ((warp == 1 || warp == 2) && active) {
       // ===================== MMA issuers: warp 1 for stream A, warp 2 for stream B =====================
       // Per stream S is double-buffered (2 x 64 TMEM columns; P aliases S), so Q.K^T runs two key tiles
