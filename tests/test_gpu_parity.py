@@ -220,6 +220,31 @@ def test_attention_many_lanes_limits(handle):
     assert e.value.status == B.AL_ERR_UNSUPPORTED
 
 
+@pytest.mark.parametrize("case", [
+    # (Hq, Hkv, groups as (prefix_len(s), q_lens), note)
+    dict(Hq=16, Hkv=1, groups=[(300, [32, 32, 7])], note="n_rep 16: 8 tokens per sub-tile, many tiles per run"),
+    dict(Hq=6, Hkv=2, groups=[(130, [32] * 9), (64, [5])], note="n_rep 3 (126-row tiles), a run of 288 tokens: 4 two-sub-tile tiles"),
+    dict(Hq=2, Hkv=2, groups=[(63, [32] * 5), ([65, 64, 1], [32, 32, 32])], note="MHA, prefixes around the 64-key tile edge"),
+    dict(Hq=8, Hkv=8, groups=[(0, [32] * 6), (200, [32] * 6)], note="no prefix at all next to a prefixed group, 192-token runs"),
+    dict(Hq=4, Hkv=4, groups=[(40 + 3 * i, [24, 11]) for i in range(45)], note="180 items: more items than SMs, stream-K with whole items"),
+    dict(Hq=1, Hkv=1, groups=[(1500, [32] * 4)], note="one head, one long item: stream-K over every SM, then merged"),
+    dict(Hq=28, Hkv=4, groups=[(700, [32] * 26)], note="832-token run: more than 96 tiles' worth of plan records per head"),
+])
+def test_attention_shape_sweep(handle, case):
+    """Shapes chosen to reach the corners of the work decomposition: tokens per sub-tile from 8 to 128,
+    one / two sub-tiles per tile, whole-item / alt / stream-K plans, split items merged from 2 to ~100
+    partials, local key ranges that span several 64-key tiles."""
+    groups, base = [], 0
+    for pl, q_lens in case["groups"]:
+        mx = max(pl) if isinstance(pl, list) else pl
+        groups.append(dict(kv_base_row=base, prefix_len=pl, q_lens=q_lens))
+        base += mx + 3
+    wl = W.build_workload("sweep", 900 + case["Hq"], "bf16", case["Hq"], case["Hkv"], 128, 1, base + 64, groups,
+                          n_refresh=1, refresh_base_row=0, refresh_span=8, vocab=64, logit_sigma=1.0,
+                          planted_frac=0.0, mask_id=63, eos_id=-1, threshold=0.9)
+    check_attention(handle, wl, tol=1e-2, lse_tol=1e-3)
+
+
 # ------------------------------------------------------------------------------------------------
 # refresh
 # ------------------------------------------------------------------------------------------------
