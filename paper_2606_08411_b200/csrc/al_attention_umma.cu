@@ -459,31 +459,31 @@ __device__ __forceinline__ int sub_rows(const AttnParams& p, const TileRec& T, i
 
 // Merge of the partials of sub-tile b of one split item by the 128 threads of stream b in the CTA
 // that finished last.  Pieces of an item live on consecutive CTAs c0..c1: slot 2*c0+1 (c0's last
-// piece), then 2*c for the rest.  Warp w owns rows [32w, 32w+32) in four passes of 8 rows; a lane holds
-// one float4 column group.  Per pass the loads of up to four pieces (8 coalesced 512-byte rows each,
-// plus the rows' LSE in lanes 0-7) are all issued before any is used, so a pass costs one L2 round
-// trip; further pieces are folded in with a running maximum.  The order of operations is fixed, so
-// the result does not depend on which CTA happens to arrive last.
-__device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T, int g, int b, int c0, int c1,
+// piece), then 2*c for the rest.  Warp w owns rows [32w, 32w+32) in passes of kRows rows; a lane holds
+// one float4 column group.  Per pass the loads of kBatch pieces (kRows coalesced 512-byte rows each,
+// plus the rows' LSE in the low lanes) are all issued before any is used -- 32 loads in flight per
+// lane, one L2 round trip; further pieces are folded in with a running maximum.  The order of
+// operations is fixed, so the result does not depend on which CTA happens to arrive last.
+template <int kBatch, int kRows>
+__device__ __forceinline__ void merge_rows(const AttnParams& p, const TileRec& T, int g, int b, int c0, int n_pieces,
                                            int tid128) {
   const int warp = tid128 >> 5, lane = tid128 & 31;
   const int n_rows = sub_rows(p, T, b);
-  const int n_pieces = c1 - c0 + 1;
-  for (int pass = 0; pass < 4; ++pass) {
-    const int row0 = warp * 32 + pass * 8;
+  for (int pass = 0; pass < 32 / kRows; ++pass) {
+    const int row0 = warp * 32 + pass * kRows;
     if (row0 >= n_rows) break;
-    const int my_row = row0 + (lane & 7);
+    const int my_row = row0 + (lane & (kRows - 1));
     const bool has_row = my_row < n_rows;
     float mx = -INFINITY, wsum = 0.f;              // running maximum of the LSEs and sum of weights of lane's row
-    float4 acc[8];
+    float4 acc[kRows];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = 0; k < kRows; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
     TRACE_M(11 + 0);
-    for (int j0 = 0; j0 < n_pieces; j0 += 4) {
-      float4 v[4][8];
-      float ls[4];
+    for (int j0 = 0; j0 < n_pieces; j0 += kBatch) {
+      float4 v[kBatch][kRows];
+      float ls[kBatch];
 #pragma unroll
-      for (int jj = 0; jj < 4; ++jj) {
+      for (int jj = 0; jj < kBatch; ++jj) {
         const int j = j0 + jj;
         const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
         const bool pj = j < n_pieces;
@@ -491,31 +491,39 @@ __device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T
         const float4* src =
             reinterpret_cast<const float4*>(p.plan.part_o + (((long long)slot * 2 + b) * kBM + row0) * kD) + lane;
 #pragma unroll
-        for (int k = 0; k < 8; ++k)
+        for (int k = 0; k < kRows; ++k)
           v[jj][k] = (pj && row0 + k < n_rows) ? __ldcg(src + k * (kD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
       }
       TRACE_M(12);
-      const float mx_new = fmaxf(fmaxf(mx, fmaxf(ls[0], ls[1])), fmaxf(ls[2], ls[3]));
-      if (mx_new == 123.456f) TRACE_M(15);
+      float mx_new = mx;
+#pragma unroll
+      for (int jj = 0; jj < kBatch; ++jj) mx_new = fmaxf(mx_new, ls[jj]);
       const float resc = (mx == -INFINITY) ? 0.f : exp2f((mx - mx_new) * kLog2e);     // 1 when the maximum stands
       wsum *= resc;
       mx = mx_new;
-      float wj[4];
+      float wj[kBatch];
 #pragma unroll
-      for (int jj = 0; jj < 4; ++jj) {
+      for (int jj = 0; jj < kBatch; ++jj) {
         wj[jj] = (ls[jj] == -INFINITY) ? 0.f : exp2f((ls[jj] - mx) * kLog2e);   // 0: the row saw no key in this piece
         wsum += wj[jj];
       }
+      if (j0 > 0) {                                  // (the accumulators are zero before the first batch)
 #pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const float rk = __shfl_sync(0xffffffffu, resc, k);
-        acc[k].x *= rk; acc[k].y *= rk; acc[k].z *= rk; acc[k].w *= rk;
+        for (int k = 0; k < kRows; ++k) {
+          const float rk = __shfl_sync(0xffffffffu, resc, k);
+          acc[k].x *= rk; acc[k].y *= rk; acc[k].z *= rk; acc[k].w *= rk;
+        }
+      }
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) {
+      for (int jj = 0; jj < kBatch; ++jj) {
+        // a piece in which none of these rows saw a key may hold stale memory (a stream without key tiles
+        // in a piece writes nothing): skip it; rows without data inside a written piece hold zeros
+        if (!__any_sync(0xffffffffu, wj[jj] > 0.f)) continue;
+#pragma unroll
+        for (int k = 0; k < kRows; ++k) {
           const float wk = __shfl_sync(0xffffffffu, wj[jj], k);
-          const bool on = wk > 0.f;                    // rows without data in this piece hold stale memory
-          acc[k].x = fmaf(wk, on ? v[jj][k].x : 0.f, acc[k].x); acc[k].y = fmaf(wk, on ? v[jj][k].y : 0.f, acc[k].y);
-          acc[k].z = fmaf(wk, on ? v[jj][k].z : 0.f, acc[k].z); acc[k].w = fmaf(wk, on ? v[jj][k].w : 0.f, acc[k].w);
+          acc[k].x = fmaf(wk, v[jj][k].x, acc[k].x); acc[k].y = fmaf(wk, v[jj][k].y, acc[k].y);
+          acc[k].z = fmaf(wk, v[jj][k].z, acc[k].z); acc[k].w = fmaf(wk, v[jj][k].w, acc[k].w);
         }
       }
     }
@@ -524,7 +532,7 @@ __device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T
     int tl = row0 / p.n_rep, hl = row0 - tl * p.n_rep;                 // token and head of row0, carried along
     long long orow = (long long)(T.q_tok0 + b * p.tpt + tl) * p.n_q_heads + g * p.n_rep + hl;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < kRows; ++k) {
       const float ik = __shfl_sync(0xffffffffu, inv, k);
       if (row0 + k < n_rows) {
         uint2 pk;
@@ -534,9 +542,15 @@ __device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T
       }
       if (++hl == p.n_rep) { hl = 0; orow += p.n_q_heads - p.n_rep + 1; } else ++orow;
     }
-    if (p.lse && has_row && lane < 8) p.lse[out_row(p, T, g, b, my_row)] = mx + logf(wsum);
+    if (p.lse && has_row && lane < kRows) p.lse[out_row(p, T, g, b, my_row)] = mx + logf(wsum);
     TRACE_M(14);
   }
+}
+__device__ __forceinline__ void merge_item(const AttnParams& p, const TileRec& T, int g, int b, int c0, int c1,
+                                           int tid128) {
+  const int n_pieces = c1 - c0 + 1;
+  if (n_pieces <= 2) merge_rows<2, 16>(p, T, g, b, c0, n_pieces, tid128);   // the usual case: an item cut once
+  else merge_rows<4, 8>(p, T, g, b, c0, n_pieces, tid128);
 }
 
 // Epilogue staging.  A thread writes the 128 bytes of its own row as eight 16-byte chunks; chunk c
