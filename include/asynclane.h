@@ -107,7 +107,7 @@ int32_t al_sm_count(const al_handle* handle);
  * Lanes of one group that are adjacent in the array and contiguous in q_start are stacked into
  * common 128-row tensor-core tiles.
  * Limits of the tensor-core path (bf16, head_dim 128): at most 1024 lanes per call and at most 2048
- * query tiles (total_q_rows / (2 * floor(128 / n_rep)) + n_lanes); beyond them AL_ERR_UNSUPPORTED.
+ * query tiles (ceil(total_q_rows / (2 * floor(128 / n_rep))) + n_lanes); beyond them AL_ERR_UNSUPPORTED.
  * Results are deterministic: the same inputs give bit-identical outputs from call to call.
  * Rows of Q not covered by any lane are not written in `out`.
  * Cache rows of a group up to its largest prefix_len rounded up to 16 must hold finite values

@@ -16,6 +16,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libasynclane.so")
+FLAGS_FILE = LIB + ".flags"                       # the flags the library was built with: a change rebuilds it
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 FLAGS = [
@@ -33,8 +34,11 @@ def sources():
 
 
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(FLAGS_FILE):
         return True
+    with open(FLAGS_FILE) as f:
+        if f.read() != " ".join(FLAGS):
+            return True
     t = os.path.getmtime(LIB)
     deps = sources() + glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + \
         [os.path.join(ROOT, "include", "asynclane.h"), os.path.abspath(__file__)]
@@ -68,6 +72,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     subprocess.check_call([NVCC, "-shared", "-o", tmp, *objs, "-cudart", "static",
                            "-gencode", "arch=compute_100a,code=sm_100a"])
     os.replace(tmp, LIB)
+    with open(FLAGS_FILE, "w") as f:
+        f.write(" ".join(FLAGS))
     return LIB
 
 

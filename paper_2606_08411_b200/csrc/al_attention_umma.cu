@@ -363,17 +363,33 @@ struct PieceWalk {
   __device__ __forceinline__ int item() const { return t * n_kv + g; }
 };
 
-// Does stream b have work in key tile kt of tile T?  Two sub-tiles: stream b = sub-tile b (prefix tiles:
+// Which steps of a piece does stream b work on?  Two sub-tiles: stream b = sub-tile b (prefix tiles:
 // always; local tiles: only those that hold rows of the lanes the sub-tile's tokens belong to).  One
 // sub-tile ("alt" mode): even key tiles go to stream 0, odd ones to stream 1, each with its own running
-// max, row sum and accumulator; the epilogue merges the two.
-__device__ __forceinline__ bool takes_part(const TileRec& T, int tpt, int b, int kt, bool alt_ok) {
-  if (alt_ok && T.n_tok <= tpt) return (kt & 1) == b;  // a tile of one sub-tile: the two streams take alternate key tiles of it
-  if (b * tpt >= T.n_tok) return false;
-  if (kt < T.n_pref_tiles) return true;
-  const int k0 = T.lk0 + (kt - T.n_pref_tiles) * kBN;
-  return T.sub_lk0[b] < k0 + kBN && T.sub_lk1[b] > k0;
-}
+// max, row sum and accumulator; the epilogue merges the two.  Worked out once per piece, so that the
+// per-step test is two compares on registers (step i of the piece = key tile kt_begin + i).
+struct StreamSteps {
+  int pref;                                // steps [0, pref) are prefix tiles the stream takes
+  int lo, n_loc;                           // steps [lo, lo + n_loc) are local tiles it takes
+  int par;                                 // alt mode: it takes the steps with (i & 1) == par; else -1
+  __device__ __forceinline__ StreamSteps(const TileRec& T, int tpt, int b, int kt_begin, bool alt_ok) {
+    pref = 0; lo = 0; n_loc = 0; par = -1;
+    if (alt_ok && T.n_tok <= tpt) {        // a tile of one sub-tile: the two streams take alternate key tiles of it
+      par = (kt_begin ^ b) & 1;
+    } else if (b * tpt < T.n_tok) {
+      const int s0 = b ? T.sub_lk0[1] : T.sub_lk0[0], s1 = b ? T.sub_lk1[1] : T.sub_lk1[0];
+      pref = T.n_pref_tiles - kt_begin;
+      if (s1 > s0) {                       // local tile j holds rows [lk0 + 64 j, +64): those that meet [s0, s1)
+        const int j0 = (s0 - T.lk0) / kBN, j1 = (s1 - T.lk0 + kBN - 1) / kBN;
+        lo = T.n_pref_tiles + j0 - kt_begin; n_loc = j1 - j0;
+      }
+    }
+  }
+  __device__ __forceinline__ bool takes(int i) const {
+    if (par >= 0) return (i & 1) == par;
+    return i < pref || (unsigned)(i - lo) < (unsigned)n_loc;
+  }
+};
 
 __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
   uint32_t r[32];
@@ -669,6 +685,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
         const bool alt = alt_ok && w.T.n_tok <= p.tpt;     // one sub-tile: both streams work on Q of sub-tile A
+        const StreamSteps mine(w.T, p.tpt, b, w.kt_begin, alt_ok);
         const uint64_t dq0 = alt ? dq_a0 : dq_own0, dq1 = alt ? dq_a1 : dq_own1;
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
@@ -698,9 +715,15 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
                                                     : min(kBN, w.T.lk1 - w.T.lk0 - (kt_ - w.T.n_pref_tiles) * kBN); \
           const int ksteps_ = (valid_ + 15) >> 4;                                                              \
           const uint64_t dv_ = dv + (uint64_t)(sv_ * (kTileBytes >> 4));                                       \
-          _Pragma("unroll")                                                                                    \
-          for (int k = 0; k < kBN / 16; ++k)                                                                   \
-            if (leader && k < ksteps_) mma_ts(to, ts + u_ * kBN + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+          if (ksteps_ == kBN / 16) {                /* the usual case: no per-MMA predicates */                \
+            _Pragma("unroll")                                                                                  \
+            for (int k = 0; k < kBN / 16; ++k)                                                                 \
+              if (leader) mma_ts(to, ts + u_ * kBN + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+          } else {                                                                                             \
+            _Pragma("unroll")                                                                                  \
+            for (int k = 0; k < kBN / 16; ++k)                                                                 \
+              if (leader && k < ksteps_) mma_ts(to, ts + u_ * kBN + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+          }                                                                                                    \
           if (leader) {                                                                                        \
             mma_commit(&sm.v_empty[sv_]);                                                                      \
             if (solo0) mma_commit(&sm.v_empty[sv_]);                                                           \
@@ -718,7 +741,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           // of one sub-tile's lanes only -- few) the idle issuer pays what it owes and hands the stages
           // back itself, once they have landed, which keeps the two issuers within a stage phase.
           const bool solo = alt;
-          if (!takes_part(w.T, p.tpt, b, kt, alt_ok)) {
+          if (!mine.takes(i)) {
             if (!alt) {
               while (c_qk != c_pv) AL_ISSUE_PV();
               mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
@@ -784,6 +807,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       const int n = w.kt_end - w.kt_begin;
       const bool alt = alt_ok && T.n_tok <= p.tpt;     // one sub-tile: this stream takes every other key tile of it
       const int sb = alt ? 0 : b;                      // sub-tile whose rows this stream holds
+      const StreamSteps mine(T, p.tpt, b, w.kt_begin, alt_ok);
       const int n_rows = sub_rows(p, T, sb);
       // ---- this row's token and lane ----
       const int tok_local = r / p.n_rep;
@@ -802,7 +826,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
 
       for (int i = 0; i < n; ++i) {
         const int kt = w.kt_begin + i;
-        if (!takes_part(T, p.tpt, b, kt, alt_ok)) continue;
+        if (!mine.takes(i)) continue;
         const uint32_t u = cnt % kSBuf;                  // S buffer of this key tile
         const uint32_t t_s = tmem + b * 128 + u * kBN;
         mbar_wait(&sm.s_full[b][u], (cnt / kSBuf) & 1);
@@ -924,6 +948,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         if (tid128 == 0) sm.alt_has[b] = n_mine > 0;
         *reinterpret_cast<float2*>(my_stage) = make_float2(m_used, l_sum);   // exchanged through the staging rows
         bar_sync_both();
+        TRACE_E(1);
         const float2 oth = *reinterpret_cast<const float2*>(sm.stage + ((b ^ 1) * kBM + r) * kStagePitch);
         const bool has0 = sm.alt_has[0] != 0, has1 = sm.alt_has[1] != 0;
         const float m0 = b ? oth.x : m_used, l0 = b ? oth.y : l_sum;
@@ -936,6 +961,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         const float f0 = w0 * rL, f1 = w1 * rL;
         const float lse2 = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
         bar_sync_both();                               // the exchanged values have been read: the rows may be staged over
+        TRACE_E(2);
         off_b[r] =
             whole ? (uint32_t)(out_row(p, T, w.g, 0, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
         const uint32_t t_o0 = tmem + 256, t_o1 = tmem + 384;
@@ -965,9 +991,11 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
               stage_chunk(my_stage, r, c * 4 + e,
                           make_uint4(pack_bf16x2(o[8 * e], o[8 * e + 1]), pack_bf16x2(o[8 * e + 2], o[8 * e + 3]),
                                      pack_bf16x2(o[8 * e + 4], o[8 * e + 5]), pack_bf16x2(o[8 * e + 6], o[8 * e + 7])));
+            TRACE_E(3 + c);
             if (c == 1) {
               __syncwarp();
               copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + b * 128);
+              TRACE_E(5);
               __syncwarp();
             }
           } else {                                     // fp32 partial (rows of sub-tile 0): one round per chunk
@@ -984,7 +1012,9 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         if (do_ticket && b == 0) p.plan.part_lse[((long long)slot * 2) * kBM + r] = valid ? lse2 : -INFINITY;
         if (do_ticket) __threadfence();
         tc_fence_before();
+        TRACE_E(6);
         bar_sync_both();                               // both streams have read both accumulators (and published)
+        TRACE_E(7);
         if (n_mine > 0) mbar_arrive(&sm.o_empty[b]);
         do_ticket = do_ticket && b == 0;               // stream 0 counts and merges for the tile
       } else {
