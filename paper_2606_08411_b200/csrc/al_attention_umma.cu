@@ -45,7 +45,6 @@ namespace {
 
 constexpr int kBM = 128;                   // stacked query rows per tile
 constexpr int kBN = 64;                    // keys per key tile (step); 64 lets S be double-buffered (measured faster than 128)
-constexpr int kSBuf = 128 / kBN;           // S buffers per stream in its 128 TMEM columns (P aliases S)
 constexpr int kD = 128;                    // head_dim
 constexpr int kStagesK = 256 / kBN;                // K ring depth (a K tile lives until its Q.K^T has run)
 constexpr int kStagesV = 256 / kBN;                // V ring depth (a V tile lives until its P.V has run)
@@ -302,8 +301,8 @@ struct AttnSmem {
   uint32_t stage_off[2 * kBM];                         // ... and where they go: global offset in units of 128 bytes
   uint64_t q_full, q_empty;
   uint64_t k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV];
-  uint64_t s_full[2][kSBuf], p_full[2][kSBuf];   // [stream][S buffer]
-  uint64_t pv_done[2];                     // per P.V: the lazy rescale of O waits for the stream's previous P.V
+  uint64_t s_full[2], s_free[2];           // [stream]: S written by Q.K^T / S in the softmax threads' registers
+  uint64_t p_full[2][2], pv_done[2][2];    // [stream][P buffer]: P written / the P.V that read it has completed
   uint64_t o_full[2], o_empty[2];          // per piece: accumulator complete / read out
   uint32_t tmem_base;
   int ticket[2][3];
@@ -660,15 +659,17 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       }
     } else if ((warp == 1 || warp == 2) && active) {
       // ===================== MMA issuers: warp 1 for stream A, warp 2 for stream B =====================
-      // Per stream S is double-buffered (2 x 64 TMEM columns; P aliases S), so Q.K^T runs two key tiles
-      // ahead of P.V: the order is QK(0) QK(1) PV(0) QK(2) PV(1) QK(3) ... and the softmax of tile i+1
-      // never waits for the MMAs of tile i.  Two issuing threads keep one stream's wait for its softmax
-      // from holding up the other stream's MMAs; both arrive on the K/V/Q stage barriers (count 2).
-      // The whole warp runs the loop (uniform control flow keeps descriptors and addresses in uniform
-      // registers); one elected lane issues the tcgen05 instructions.
+      // Per stream: S has one 64-column TMEM buffer, P (bf16, 32 columns) has two of its own.  The
+      // softmax hands S back as soon as it holds the tile in registers, so Q.K^T of the stream's next
+      // key tile runs under the softmax of the current one and depends on no P.V:
+      //   QK(0) | QK(1) PV(0) | QK(2) PV(1) | ...      QK(i) waits for "S(i-1) read", PV(i) for P(i)
+      // Two issuing threads keep one stream's wait for its softmax from holding up the other stream's
+      // MMAs; both arrive on the K/V/Q stage barriers (count 2).  The whole warp runs the loop (uniform
+      // control flow keeps descriptors and addresses in uniform registers); one elected lane issues the
+      // tcgen05 instructions.
       const bool leader = elect_one();
       const int b = warp - 1;
-      const uint32_t ts = tmem + b * 128, to = tmem + 256 + b * 128;
+      const uint32_t ts = tmem + b * kBN, tp = tmem + 128 + b * 64, to = tmem + 256 + b * 128;
       const uint32_t idesc_qk = make_idesc_bf16(kBM, kBN, 0, 0);
       const uint32_t idesc_pv = make_idesc_bf16(kBM, kD, 0, 1);
       // every descriptor is a constant plus a small address offset: build the bases once
@@ -690,18 +691,19 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         mbar_wait(&sm.q_full, piece_it & 1);
         tc_fence_after();
         if (b == 0 && leader) TRACE(3);
-        int owed0 = 0, owed1 = 0;              // steps (of the piece) of the up to two key tiles whose P.V is owed, oldest first
-        bool solo0 = false, solo1 = false;     // ... and whether this stream is the only one working on that key tile
+        int owed = -1;                         // step (of the piece) of the key tile whose P.V is owed
         bool first = true;
-        // O_b (+)= P . V of the oldest owed key tile.  The K/V stage barriers expect two arrivals per
-        // step: one from each issuer, or both from the only stream that takes part in the step.
+        // A step only one stream works on (alt mode: every step): its issuer arrives twice on the K/V
+        // stage barriers, which expect one arrival from each issuer, and the other issuer skips the step.
+        const bool solo = alt;
+        // O_b (+)= P . V of the owed key tile
 #define AL_ISSUE_PV()                                                                                          \
         do {                                                                                                   \
-          const uint32_t it_ = kv_it + owed0;                                                                  \
+          const uint32_t it_ = kv_it + owed;                                                                   \
           const int sv_ = it_ % kStagesV;                                                                      \
-          const uint32_t u_ = c_pv % kSBuf;                                                                    \
+          const uint32_t u_ = c_pv & 1;                                                                        \
           if (leader) TRACE_TILE(8 + b, it_);                                                                  \
-          mbar_wait(&sm.p_full[b][u_], (c_pv / kSBuf) & 1);                                                    \
+          mbar_wait(&sm.p_full[b][u_], (c_pv >> 1) & 1);                                                       \
           if (leader) TRACE_TILE(10 + b, it_);                                                                 \
           mbar_wait(&sm.v_full[sv_], (it_ / kStagesV) & 1);                                                    \
           if (leader && b == 0) TRACE_TILE(14, it_);                                                           \
@@ -710,7 +712,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           if (first && oe > 0) mbar_wait(&sm.o_empty[b], (oe - 1) & 1);                                        \
           tc_fence_after();                                                                                    \
           /* keys of this tile that any row may see, rounded up to the MMA K step */                           \
-          const int kt_ = w.kt_begin + owed0;                                                                  \
+          const int kt_ = w.kt_begin + owed;                                                                   \
           const int valid_ = kt_ < w.T.n_pref_tiles ? min(kBN, w.T.kv_len_max - kt_ * kBN)                     \
                                                     : min(kBN, w.T.lk1 - w.T.lk0 - (kt_ - w.T.n_pref_tiles) * kBN); \
           const int ksteps_ = (valid_ + 15) >> 4;                                                              \
@@ -718,32 +720,29 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           if (ksteps_ == kBN / 16) {                /* the usual case: no per-MMA predicates */                \
             _Pragma("unroll")                                                                                  \
             for (int k = 0; k < kBN / 16; ++k)                                                                 \
-              if (leader) mma_ts(to, ts + u_ * kBN + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+              if (leader) mma_ts(to, tp + u_ * 32 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
           } else {                                                                                             \
             _Pragma("unroll")                                                                                  \
             for (int k = 0; k < kBN / 16; ++k)                                                                 \
-              if (leader && k < ksteps_) mma_ts(to, ts + u_ * kBN + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
+              if (leader && k < ksteps_) mma_ts(to, tp + u_ * 32 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
           }                                                                                                    \
           if (leader) {                                                                                        \
             mma_commit(&sm.v_empty[sv_]);                                                                      \
-            if (solo0) mma_commit(&sm.v_empty[sv_]);                                                           \
-            mma_commit(&sm.pv_done[b]);                                                                        \
+            if (solo) mma_commit(&sm.v_empty[sv_]);                                                            \
+            mma_commit(&sm.pv_done[b][u_]);                                                                    \
           }                                                                                                    \
           if (leader) TRACE_TILE(3 + 4 * b, it_);                                                              \
-          first = false; ++c_pv; owed0 = owed1; solo0 = solo1;                                                 \
+          first = false; ++c_pv; owed = -1;                                                                    \
         } while (0)
         for (int i = 0; i < n; ++i) {
-          const int kt = w.kt_begin + i;
           const uint32_t it = kv_it + i;
           const int sk = it % kStagesK;
-          // A step only one stream works on: in alt mode (every step is one) its issuer arrives twice on
-          // the stage barriers and the other issuer skips the step; with two sub-tiles (local key tiles
-          // of one sub-tile's lanes only -- few) the idle issuer pays what it owes and hands the stages
-          // back itself, once they have landed, which keeps the two issuers within a stage phase.
-          const bool solo = alt;
           if (!mine.takes(i)) {
+            // With two sub-tiles (local key tiles of one sub-tile's lanes only -- few) the idle issuer pays
+            // what it owes and hands the stages back itself, once they have landed, which keeps the two
+            // issuers within a stage phase.
             if (!alt) {
-              while (c_qk != c_pv) AL_ISSUE_PV();
+              if (owed >= 0) AL_ISSUE_PV();
               mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
               if (leader) mma_commit(&sm.k_empty[sk]);
               mbar_wait(&sm.v_full[it % kStagesV], (it / kStagesV) & 1);
@@ -751,33 +750,30 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             }
             continue;
           }
-          // The producer issues K(i) only after V(i-1), whose stage V(i-1-kStagesV) used: everything owed
-          // from that far back has to be paid before waiting for K(i).
-          while (c_qk != c_pv && owed0 + kStagesV < i) AL_ISSUE_PV();
           if (leader && b == 0) TRACE_TILE(12, it);
           mbar_wait(&sm.k_full[sk], (it / kStagesK) & 1);
           if (leader && b == 0) TRACE_TILE(13, it);
-          // ---- S_b[u] = Q_b . K^T of step i
-          if (c_qk - c_pv == kSBuf) AL_ISSUE_PV();           // frees the S buffer this Q.K^T writes (P aliases S)
+          // ---- S_b = Q_b . K^T of step i, once the softmax holds the stream's previous S in registers
+          if (c_qk > 0) mbar_wait(&sm.s_free[b], (c_qk - 1) & 1);
           tc_fence_after();
           if (b == 0 && leader) TRACE(4);
-          const uint32_t u = c_qk % kSBuf;
           const uint64_t dk0 = dk + (uint64_t)(sk * (kTileBytes >> 4)), dk1 = dk0 + (uint64_t)(kKvHalfBytes >> 4);
 #pragma unroll
-          for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
+          for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts, dq0 + (uint64_t)(2 * k), dk0 + (uint64_t)(2 * k), idesc_qk, k ? 1u : 0u);
 #pragma unroll
-          for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts + u * kBN, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
+          for (int k = 0; k < 4; ++k) if (leader) mma_ss(ts, dq1 + (uint64_t)(2 * k), dk1 + (uint64_t)(2 * k), idesc_qk, 1u);
           if (leader) {
-            mma_commit(&sm.s_full[b][u]);
+            mma_commit(&sm.s_full[b]);
             mma_commit(&sm.k_empty[sk]);
             if (solo) mma_commit(&sm.k_empty[sk]);
           }
           if (leader) TRACE_TILE(4 * b, it);
-          if (c_qk == c_pv) { owed0 = i; solo0 = solo; } else { owed1 = i; solo1 = solo; }   // at most kSBuf (<= 2) key tiles are owed
           ++c_qk;
+          if (owed >= 0) AL_ISSUE_PV();                      // P.V of the stream's previous key tile, behind this Q.K^T
+          owed = i;
         }
         if (leader) mma_commit(&sm.q_empty);                 // this issuer's Q.K^T of the piece are all issued
-        while (c_qk != c_pv) AL_ISSUE_PV();
+        if (owed >= 0) AL_ISSUE_PV();
         if (leader && !first) mma_commit(&sm.o_full[b]);     // the piece's accumulator is complete
 #undef AL_ISSUE_PV
         if (b == 0 && leader) TRACE(5);
@@ -827,9 +823,9 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       for (int i = 0; i < n; ++i) {
         const int kt = w.kt_begin + i;
         if (!mine.takes(i)) continue;
-        const uint32_t u = cnt % kSBuf;                  // S buffer of this key tile
-        const uint32_t t_s = tmem + b * 128 + u * kBN;
-        mbar_wait(&sm.s_full[b][u], (cnt / kSBuf) & 1);
+        const uint32_t u = cnt & 1;                      // P buffer of this key tile
+        const uint32_t t_s = tmem + b * kBN, t_p = tmem + 128 + b * 64 + u * 32;
+        mbar_wait(&sm.s_full[b], cnt & 1);
         tc_fence_after();
         if (tid128 == 0 && b == 0) TRACE(6);
         if (tid128 == 0) TRACE_TILE(1 + 4 * b, cnt);
@@ -838,6 +834,8 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
 #pragma unroll
         for (int c = 0; c < kBN / 32; ++c) tmem_ld32_f(t_s + lane_addr + c * 32, s + c * 32);
         tmem_wait_ld();
+        tc_fence_before();
+        mbar_arrive(&sm.s_free[b]);                      // S is in registers: the stream's next Q.K^T may overwrite it
         TRACE_W(1);
         // visible columns of this tile for this row: [lo, hi).  Rows beyond the sub-tile's last token are
         // never stored: they run unmasked on whatever their Q row holds.
@@ -875,10 +873,10 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         if (m_used == -INFINITY) m_used = m_new;         // nothing accumulated yet (O row is 0 or unwritten)
         else grow = valid && (m_new - m_used) * p.scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, grow)) {             // warp-uniform: tcgen05.ld/st are .sync.aligned
-          // rare: O of this stream must be rescaled, so its previous P.V has to have landed.  pv_done[b]
-          // completes once per P.V; at most cnt of them can have completed here and all before cnt - 1
-          // have (the commit behind s_full covers them), so the parity wait cannot alias.
-          if (n_mine > 0) { mbar_wait(&sm.pv_done[b], (cnt - 1) & 1); tc_fence_after(); }
+          // rare: O of this stream must be rescaled, so its previous P.V has to have landed.  The next
+          // phase of that barrier belongs to the P.V of tile cnt + 1, which cannot be issued before this
+          // thread has stored P of tile cnt, so the parity wait cannot alias.
+          if (n_mine > 0) { mbar_wait(&sm.pv_done[b][(cnt - 1) & 1], ((cnt - 1) >> 1) & 1); tc_fence_after(); }
           const float alpha = grow ? ex2((m_used - m_new) * p.scale_log2) : 1.0f;
           if (grow) { l_sum *= alpha; m_used = m_new; }
           if (n_mine > 0) {
@@ -896,6 +894,8 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         const float negmb = (m_used == -INFINITY) ? 0.f : -m_used * p.scale_log2;
         const uint64_t negmb2 = pack2(negmb, negmb);
         uint64_t sum_a = pack2(0.f, 0.f), sum_b = sum_a;
+        // the P.V that read this P buffer two tiles ago has completed (long ago, as a rule)
+        if (cnt >= 2) { mbar_wait(&sm.pv_done[b][u], ((cnt - 2) >> 1) & 1); tc_fence_after(); }
 #pragma unroll
         for (int c = 0; c < kBN / 32; ++c) {
           uint32_t pk[16];
@@ -918,7 +918,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
               pk[e] = pack_bf16x2(p0, p1);
             }
           }
-          tmem_st16(t_s + lane_addr + c * 16, pk);
+          tmem_st16(t_p + lane_addr + c * 16, pk);
         }
         float l0, l1;
         unpack2(fadd2(sum_a, sum_b), l0, l1);
@@ -1125,8 +1125,9 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     for (int s = 0; s < kStagesK; ++s) { mbar_init(&sm.k_full[s], 1); mbar_init(&sm.k_empty[s], 2); }
     for (int s = 0; s < kStagesV; ++s) { mbar_init(&sm.v_full[s], 1); mbar_init(&sm.v_empty[s], 2); }
     for (int b = 0; b < 2; ++b) {
-      for (int u = 0; u < kSBuf; ++u) { mbar_init(&sm.s_full[b][u], 1); mbar_init(&sm.p_full[b][u], 128); }
-      mbar_init(&sm.pv_done[b], 1); mbar_init(&sm.o_full[b], 1); mbar_init(&sm.o_empty[b], 128);
+      mbar_init(&sm.s_full[b], 1); mbar_init(&sm.s_free[b], 128);
+      for (int u = 0; u < 2; ++u) { mbar_init(&sm.p_full[b][u], 128); mbar_init(&sm.pv_done[b][u], 1); }
+      mbar_init(&sm.o_full[b], 1); mbar_init(&sm.o_empty[b], 128);
     }
     fence_barrier_init();
     prefetch_tensormap(&map_q); prefetch_tensormap(&map_knew); prefetch_tensormap(&map_vnew);
@@ -1137,7 +1138,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
-  // TMEM columns: S of stream b, buffer u at (2 b + u) * 64; O of stream b at 256 + 128 b
+  // TMEM columns: S of stream b at 64 b; P of stream b, buffer u at 128 + 64 b + 32 u; O of stream b at 256 + 128 b
   // programmatic dependent launch: everything above overlapped the previous kernel in the stream (the
   // plan, or the previous layer); its memory is visible after the wait.  The next launch in the stream
   // that opts in (the next layer) may then begin its own prologue as SMs free up.
