@@ -60,6 +60,10 @@ constexpr int kPlanThreads = 256;
 constexpr int kPlanTilesInSmem = 96;
 constexpr int kMaxCtas = 256;              // >= SMs of any sm_100 part
 constexpr int kMinPiece = 256 / kBN;       // do not cut the work finer than 256 keys per CTA
+#ifndef AL_EPI_COST
+#define AL_EPI_COST 4
+#endif
+constexpr int kEpiCost = AL_EPI_COST;      // what the epilogue of an item costs, in 64-key steps, when the step ranges are cut
 constexpr int kSplitCost = 1280 / kBN;     // what splitting an item costs (partial epilogue, ticket, merge by the last CTA), in steps: measured 12-20 us
 
 struct __align__(16) TileRec {             // 64 bytes
@@ -243,7 +247,21 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     if (whole_items) {                                 // CTA c = item c = (tile c / n_kv, head c % n_kv)
       const int t = c / n_kv_heads;
       f = c == n_ctas ? k_total : s_a[t] + (c - t * n_kv_heads) * ((s_a[t + 1] - s_a[t]) / n_kv_heads);
-    } else if (snap && c > 0 && c < n_ctas) {
+    } else if (kEpiCost > 0 && c > 0 && c < n_ctas) {
+      // equal shares of (steps + kEpiCost per item): the CTA that finishes an item also pays its epilogue.
+      // Tile t starts at cost s_a[t] + kEpiCost * n_kv * t; inside it every item costs nk + kEpiCost.
+      const long long x = (long long)c * (k_total + (long long)kEpiCost * n_tiles * n_kv_heads) / n_ctas;
+      int lo = 0, hi = n_tiles - 1;
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if ((long long)s_a[mid] + (long long)kEpiCost * n_kv_heads * mid <= x) lo = mid; else hi = mid - 1;
+      }
+      const int nk = (s_a[lo + 1] - s_a[lo]) / n_kv_heads;
+      const int within = (int)(x - ((long long)s_a[lo] + (long long)kEpiCost * n_kv_heads * lo));
+      const int g = within / (nk + kEpiCost), rem = within - g * (nk + kEpiCost);
+      f = s_a[lo] + g * nk + min(rem, nk);
+    }
+    if (!whole_items && snap && c > 0 && c < n_ctas) {
       const int t = last_le(s_a, n_tiles, f);
       const int nk = (s_a[t + 1] - s_a[t]) / n_kv_heads;
       const int rem = (f - s_a[t]) % nk;           // steps into the item
@@ -291,6 +309,11 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
 // ---------------------------------------------------------------------------------------------
 // main kernel
 // ---------------------------------------------------------------------------------------------
+// Of every eight column pairs of a key tile, those whose exp2 runs on the FMA pipes instead of the MUFU.
+// With two sub-tiles per step both streams' softmax warps load each SM sub-partition's MUFU and three
+// of eight pay; when the streams take alternate key tiles (whole-item plans) one of eight is enough and
+// the instruction count matters more (cfg4: 648 -> 617 us with one, cfg5: 88.6 -> 90.9 us).
+constexpr int kPolyMaskTwoSubTiles = 0x52, kPolyMaskAlt = 0x10;
 constexpr int kStagePitch = 128;           // 128 data bytes per staged row; 16-byte chunk c of row r sits at chunk c ^ (r & 7)
 
 struct AttnSmem {
@@ -907,7 +930,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             for (int e = 0; e < 16; ++e) {
               const uint64_t x2 = ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), scale2, negmb2);
               float p0, p1;
-              if ((0x52 >> (e & 7)) & 1) {                 // three pairs of eight: FMA pipes instead of the MUFU
+              if (((kAltOk ? kPolyMaskAlt : kPolyMaskTwoSubTiles) >> (e & 7)) & 1) {                 // three pairs of eight: FMA pipes instead of the MUFU
                 exp2_poly_pair(x2, p0, p1);
               } else {
                 float t0, t1;
