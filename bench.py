@@ -401,7 +401,11 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                    "max_prefix": wl.max_prefix_len, "refresh_rows": int(wl.refresh_pos.size),
                    "logits": list(wl.logits.shape), "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "l2": f"rotating {n_copies} resident copies of every streamed buffer "
-                         f"({n_copies * per_copy / 1e6:.0f} MB > 2x 126 MB L2), one CUDA graph per step"},
+                         f"({n_copies * per_copy / 1e6:.0f} MB > 2x 126 MB L2), one CUDA graph per step",
+                   "graph": ("plan -> attention per layer -> {refresh on a side stream || confidence/select}"
+                             if first.logits.numel() * first.logits.element_size() <= first.OVERLAP_MAX_LOGITS_BYTES
+                             else "plan -> attention per layer -> refresh -> confidence/select")
+                            + "; the parts are also timed alone on graphs of their own"},
         "clocks": sampler.summary(),
         "e2e": {"value": whole_job_value(e2e_tokens, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps,

@@ -70,6 +70,9 @@ class LaneStep:
         self.ws_conf = torch.empty(max(ws_c, 16), dtype=torch.uint8, device=dev)
         self.flags = B.AL_SELECT_FORCE_TOP1 if force_top1 else 0
         self.gpu_launches_per_step = None   # filled by callers that count (bench)
+        # side stream of run(overlap=True); made here (not under a graph capture) and shared by replicas
+        self._side = torch.cuda.Stream(device=dev)
+        self._fork, self._join = torch.cuda.Event(), torch.cuda.Event()
 
     def replicate(self) -> "LaneStep":
         """A second instance on DISTINCT device allocations of every streamed buffer (same values):
@@ -116,16 +119,36 @@ class LaneStep:
                                     float(wl.threshold), self.lanes, wl.n_lanes, self.flags, self.conf,
                                     self.argmax, self.commit, self.tokens_out, self.ws_conf, stream)
 
-    def run(self, stream=None, marks=None) -> None:
+    # Above this many logits bytes the confidence kernel saturates HBM on its own (cfg5: 98 % of the copy
+    # bandwidth) and a concurrent refresh only disturbs its cluster scheduling (measured: +10 us at cfg5,
+    # -3.5 us at cfg2, -3 us at cfg3): the refresh then runs in line.
+    OVERLAP_MAX_LOGITS_BYTES = 256 << 20
+
+    def run(self, stream=None, marks=None, overlap: Optional[bool] = None) -> None:
         """The whole hot path once.  Attention reads the cache BEFORE this step's refresh writes it
         (kappa_l is the state the lanes were forked from; refresh is periodic, L176).
-        `marks`: optional 4 timing events recorded before/between/after the three parts."""
+        Refresh (writes the cache) and confidence/select (reads the logits) are independent of each
+        other: with `overlap` (default: when the logits are small enough for it to pay) the refresh runs
+        on a side stream, forked after the attention and joined after the confidence kernel -- plain
+        edges when the step is captured into a CUDA graph.
+        `marks`: optional 4 timing events recorded before/between/after the three parts (serial order)."""
         s = torch.cuda.current_stream() if stream is None else stream
+        if overlap is None:
+            overlap = self.logits.numel() * self.logits.element_size() <= self.OVERLAP_MAX_LOGITS_BYTES
         if marks is not None:
+            overlap = False
             marks[0].record(s)
         self.attention(stream)
         if marks is not None:
             marks[1].record(s)
+        if overlap:
+            self._fork.record(s)
+            self._side.wait_event(self._fork)
+            self.refresh(self._side)
+            self._join.record(self._side)
+            self.confidence(stream)
+            s.wait_event(self._join)
+            return
         self.refresh(stream)
         if marks is not None:
             marks[2].record(s)
