@@ -10,30 +10,34 @@
 //              a kv-head stacked under every token it is a 128-row M tile of the tensor core
 //   tile     = two consecutive sub-tiles A, B of a run (B may be empty): they share every prefix
 //              K/V tile, so each K/V tile staged in shared memory feeds 2 x (128x128x128) MMAs
-//   keys     = [prefix key tiles of 128 cache rows] ++ [local key tiles of 128 K_new rows covering the
+//   keys     = [prefix key tiles of 64 cache rows] ++ [local key tiles of 64 K_new rows covering the
 //              lanes that intersect the tile]; every row masks what its own lane may not see
 //   item     = (tile, kv-head): n_key_tiles steps of the main loop
-// The steps of all items, flattened item-major, form one sequence of K key-tile steps that is cut
-// into n_ctas contiguous, equal ranges ("stream-K"): every CTA gets the same number of steps (+-1)
-// whatever the lane structure is.  A range boundary that falls within one step of an item boundary
-// snaps to it.  An item whose steps are spread over several CTAs leaves one normalised fp32 partial
-// + LSE per CTA in the workspace; the CTA that finishes last (a ticket counter per item) merges
-// them -- no combine launch.
+// The 64-key steps of all items, flattened item-major, are cut into per-CTA ranges: one CTA per item
+// ("whole items") when every item can have a CTA of its own and splitting would not pay, else
+// n_ctas contiguous ranges of equal cost ("stream-K": steps + kEpiCost per item finished, whatever
+// the lane structure is), a boundary within one step of an item boundary snapping to it.  An item
+// whose steps are spread over several CTAs leaves one normalised fp32 partial + LSE per CTA in the
+// workspace; the CTA that finishes last (a ticket counter per (item, sub-tile)) merges them in a
+// fixed order -- no combine launch, bit-identical results from call to call.
 // All CTAs that share (group, kv-head) read the same K/V tiles: HBM sees them once, L2 serves the
 // rest -- "the prefix is read once per lane group" (BASELINE north_star).
 //
 // Main kernel, persistent, 384 threads, warp-specialised, one CTA per SM:
-//   warp 0      TMA producer: both Q sub-tiles once per piece, K and V tiles through 2-stage rings
-//   warp 1      MMA issuer (one elected lane): S_b = Q_b.K^T (SS form) into TMEM buffer S_b;
-//               O_b += P_b.V with P_b read from TMEM (TS form) and V MN-major in shared memory;
-//               per stream b the order is P.V of its previous key tile, then Q.K^T of the next
-//   warps 4-7   softmax of sub-tile A, one thread per stacked row
-//   warps 8-11  softmax of sub-tile B
-//               the exponentials of one sub-tile overlap the MMAs of the other; O is rescaled lazily
-//               (only when the running max grows by more than 2^8).  Epilogue per stream: normalise,
-//               stage 128-byte half rows in shared memory, store coalesced (bf16 output, or fp32
-//               partial for a split item).
-// TMEM: S_A | S_B | O_A | O_B, 128 fp32 columns each (P aliases S as packed bf16).
+//   warp 0      TMA producer: both Q sub-tiles once per piece, K tiles through a 4-stage ring
+//   warp 3      TMA producer of the V tiles (their stages are freed much later than the K stages)
+//   warps 1, 2  MMA issuer of stream A / B (warp-uniform, one elected lane): S_b = Q_b.K^T (SS form)
+//               into the stream's S buffer as soon as the softmax holds the previous S in registers;
+//               O_b += P_b.V with P_b read from one of the stream's two P buffers in TMEM (TS form)
+//               and V MN-major in shared memory
+//   warps 4-7   softmax of stream A (sub-tile A), one thread per stacked row
+//   warps 8-11  softmax of stream B (sub-tile B; with one sub-tile per tile under a whole-item plan
+//               the two streams take alternate key tiles of it and the epilogue merges them)
+//               O is rescaled lazily (only when the running max grows by more than 2^8).  Epilogue
+//               per stream: normalise, stage 128-byte half rows in shared memory, store coalesced
+//               (bf16 output, or fp32 partial for a split item).
+// TMEM (512 columns): S_A | S_B (64 fp32 columns each) | P_A[2] | P_B[2] (32 columns of packed bf16
+// each) | O_A | O_B (128 fp32 columns each).
 #include <cuda_bf16.h>
 
 #include "al_internal.h"
@@ -44,7 +48,7 @@ using namespace alptx;
 namespace {
 
 constexpr int kBM = 128;                   // stacked query rows per tile
-constexpr int kBN = 64;                    // keys per key tile (step); 64 lets S be double-buffered (measured faster than 128)
+constexpr int kBN = 64;                    // keys per key tile (step); 64 leaves TMEM room for P buffers of their own (measured faster than 128)
 constexpr int kD = 128;                    // head_dim
 constexpr int kStagesK = 256 / kBN;                // K ring depth (a K tile lives until its Q.K^T has run)
 constexpr int kStagesV = 256 / kBN;                // V ring depth (a V tile lives until its P.V has run)
