@@ -245,6 +245,27 @@ def test_attention_shape_sweep(handle, case):
     check_attention(handle, wl, tol=1e-2, lse_tol=1e-3)
 
 
+@pytest.mark.parametrize("seed", [11, 12, 13, 14, 15, 16])
+def test_attention_random_lane_trees(handle, seed):
+    """Seeded random lane trees: head layout, number of groups, per-lane prefix lengths (nested inside a
+    group, as after forks at different depths) and window lengths all drawn at random.  Every barrier
+    wait in the kernel traps after a bounded spin, so a protocol error shows up as a failed call."""
+    rng = np.random.default_rng(7000 + seed)
+    hq, hkv = [(4, 4), (8, 2), (12, 4), (16, 2), (28, 4), (32, 32)][seed % 6]
+    groups, base = [], 0
+    for _ in range(int(rng.integers(1, 6))):
+        n_l = int(rng.integers(1, 9))
+        top = int(rng.integers(0, 700))
+        pl = sorted(int(x) for x in rng.integers(max(0, top - 200), top + 1, size=n_l))
+        q_lens = [int(x) for x in rng.integers(1, 41, size=n_l)]
+        groups.append(dict(kv_base_row=base, prefix_len=pl, q_lens=q_lens))
+        base += top + 5
+    wl = W.build_workload("random_tree", 7100 + seed, "bf16", hq, hkv, 128, 1, base + 64, groups, n_refresh=1,
+                          refresh_base_row=0, refresh_span=8, vocab=64, logit_sigma=1.0, planted_frac=0.0,
+                          mask_id=63, eos_id=-1, threshold=0.9)
+    check_attention(handle, wl, tol=1e-2, lse_tol=1e-3)
+
+
 # ------------------------------------------------------------------------------------------------
 # refresh
 # ------------------------------------------------------------------------------------------------
