@@ -510,7 +510,7 @@ template <int kBatch, int kRows>
 __device__ __forceinline__ void merge_rows(const AttnParams& p, const TileRec& T, int g, int b, int c0, int n_pieces,
                                            int tid128) {
   const int warp = tid128 >> 5, lane = tid128 & 31;
-  const int n_rows = sub_rows(p, T, b);
+  const int n_rows = __shfl_sync(0xffffffffu, sub_rows(p, T, b), 0);
   for (int pass = 0; pass < 32 / kRows; ++pass) {
     const int row0 = warp * 32 + pass * kRows;
     if (row0 >= n_rows) break;
@@ -574,12 +574,16 @@ __device__ __forceinline__ void merge_rows(const AttnParams& p, const TileRec& T
     int tl = row0 / p.n_rep, hl = row0 - tl * p.n_rep;                 // token and head of row0, carried along
     long long orow = (long long)(T.q_tok0 + b * p.tpt + tl) * p.n_q_heads + g * p.n_rep + hl;
 #pragma unroll
-    for (int k = 0; k < kRows; ++k) {
+    for (int k = 0; k < kRows; ++k) {                // all the shuffles first: the stores then do not wait for one each
       const float ik = __shfl_sync(0xffffffffu, inv, k);
+      acc[k].x *= ik; acc[k].y *= ik; acc[k].z *= ik; acc[k].w *= ik;
+    }
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
       if (row0 + k < n_rows) {
         uint2 pk;
-        pk.x = pack_bf16x2(acc[k].x * ik, acc[k].y * ik);
-        pk.y = pack_bf16x2(acc[k].z * ik, acc[k].w * ik);
+        pk.x = pack_bf16x2(acc[k].x, acc[k].y);
+        pk.y = pack_bf16x2(acc[k].z, acc[k].w);
         reinterpret_cast<uint2*>(p.out + orow * kD)[lane] = pk;
       }
       if (++hl == p.n_rep) { hl = 0; orow += p.n_q_heads - p.n_rep + 1; } else ++orow;
