@@ -1,12 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- the lane-batched denoising step of AsyncLane on B200, measured.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 A "step" is ONE pass of the whole hot path (lane attention for every layer of the
 workload, compact KV refresh, confidence/argmax/threshold select) over one batch of seeded
-synthetic input.  The default workload is BASELINE.json configs[1] (LLaDA-8B-shaped single layer).
+synthetic input.  The default workload is BASELINE.json configs[4] (16 Dream-shaped sequences), the
+largest single-GPU configuration; configs[1..3] are measured in the same run with fewer steps and
+reported under the extra key `workloads` (step time, per-part time and roofline fraction).
 
 What is timed:
   value     K steps, inputs resident in HBM, each step one CUDA-graph replay; consecutive steps run
@@ -193,34 +195,42 @@ def run_reference(args, rank: int):
 
 
 # --------------------------------------------------------------------------------------------------
-def run_ours(args, rank: int, local_rank: int, world: int):
-    import numpy as np
+def part_rooflines(wl, acc, part_ms, step_ms, peaks, traffic):
+    """Roofline of every part from its own device time (algorithmic numerators of accounting.py)."""
+    parts = {}
+    ai = acc["attn_flops"] / acc["attn_bytes"]
+    ridge = peaks["tensor"] * 1e12 / (peaks["hbm"] * 1e9)
+    ta, tr, tc = (part_ms[k] * 1e-3 for k in ("attention", "refresh", "confidence"))
+    if ai < ridge:
+        parts["attention"] = dict(bound="hbm", achieved=acc["attn_bytes"] / ta / 1e9, peak=peaks["hbm"], unit="GB/s")
+    else:
+        parts["attention"] = dict(bound="tensor", achieved=acc["attn_flops"] / ta / 1e12, peak=peaks["tensor"],
+                                  unit="TFLOP/s")
+    parts["attention"].update(ms=ta * 1e3, launches=wl.n_layers, tflops=acc["attn_flops"] / ta / 1e12,
+                              gbs=acc["attn_bytes"] / ta / 1e9, arithmetic_intensity=ai,
+                              note="time of al_lane_plan (1 launch) + al_lane_attention_planned (1 launch per layer)")
+    parts["refresh"] = dict(bound="hbm", achieved=acc["refresh_bytes"] / tr / 1e9, peak=peaks["hbm"], unit="GB/s",
+                            ms=tr * 1e3, launches=1)
+    parts["confidence"] = dict(bound="hbm", achieved=acc["confidence_bytes"] / tc / 1e9, peak=peaks["hbm"],
+                               unit="GB/s", ms=tc * 1e3, launches=1)
+    for k, p in parts.items():
+        p["frac"] = p["achieved"] / p["peak"]
+        p["traffic"] = traffic.get(k)
+        p["share_of_step"] = p["ms"] / step_ms
+    return parts
+
+
+def measure_resident(h, wl, dev, stream, dist, sampler, steps, warmup, kernel_events=True):
+    """`steps` timed replays of the whole-step CUDA graph over rotating resident copies of `wl`, then the
+    per-part times on the parts' own graphs.  Returns the copies too (the e2e leg reuses their caches)."""
     import torch
-    from paper_2606_08411_b200 import accounting, binding, workloads as W
-    from paper_2606_08411_b200.step import LaneStep, to_host_pinned
+    from paper_2606_08411_b200.step import LaneStep
 
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the library has no CPU path")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
-    peaks = load_peaks()
-    wl = W.CONFIGS[args.workload]()
-    acc = accounting.summary(wl)
-    h = binding.Handle(local_rank)
-
-    # ---- resident copies: rotation set larger than 2x L2 ---------------------------------------
     first = LaneStep(h, wl, device=dev, want_lse=False)
     per_copy = first.streamed_bytes()
     n_copies = max(2, int(math.ceil(2.2 * L2_BYTES / per_copy)))
     copies = [first] + [first.replicate() for _ in range(n_copies - 1)]
-    stream = torch.cuda.Stream(device=dev)
-
-    # ---- one CUDA graph of the whole step per copy, plus one graph per part for the part times ------
-    graphs, marked_graphs = [], []
+    graphs, part_graphs = [], []
     launches_per_step = None
     stream.wait_stream(torch.cuda.current_stream())
     with torch.cuda.stream(stream):
@@ -236,18 +246,15 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             # one graph per part (attention = plan + every layer, refresh, confidence) for the per-part
             # times: event nodes inside the step graph would cost a few us per step and break the
             # programmatic-dependent-launch edges between the kernels
-            if args.kernel_events:
+            if kernel_events:
                 pg = {}
                 for name, fn in (("attention", st.attention), ("refresh", st.refresh), ("confidence", st.confidence)):
                     gp = torch.cuda.CUDAGraph()
                     with torch.cuda.graph(gp, stream=stream):
                         fn(stream)
                     pg[name] = gp
-                marked_graphs.append(pg)
+                part_graphs.append(pg)
     stream.synchronize()
-
-    sampler = ClockSampler(local_rank)
-    sampler.start()
 
     def barrier():
         torch.cuda.synchronize()
@@ -255,100 +262,118 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- warm-up, then EXACTLY K timed steps ------------------------------------------------------
+    # ---- warm-up, then EXACTLY `steps` timed steps ---------------------------------------------
     with torch.cuda.stream(stream):
-        for i in range(args.warmup):
+        for i in range(warmup):
             graphs[i % n_copies].replay()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler.active.set()
     with torch.cuda.stream(stream):
         e0.record(stream)
-        for i in range(args.steps):
+        for i in range(steps):
             graphs[i % n_copies].replay()
         e1.record(stream)
     barrier()
     sampler.active.clear()
-    step_ms = e0.elapsed_time(e1) / args.steps
+    step_ms = e0.elapsed_time(e1) / steps
 
     # per-part device times: right after the timed region, every part's own graph is replayed over the
     # same rotation of copies (so its inputs come from HBM, not L2) and timed with CUDA events on the stream
     part_ms = None
-    if args.kernel_events:
+    if kernel_events:
         reps = max(4 * n_copies, 40)
         part_ms = {}
         sampler.active.set()
         for name in ("attention", "refresh", "confidence"):
             with torch.cuda.stream(stream):
                 for i in range(n_copies):
-                    marked_graphs[i % n_copies][name].replay()
+                    part_graphs[i % n_copies][name].replay()
                 e0.record(stream)
                 for i in range(reps):
-                    marked_graphs[i % n_copies][name].replay()
+                    part_graphs[i % n_copies][name].replay()
                 e1.record(stream)
             barrier()
             part_ms[name] = e0.elapsed_time(e1) / reps
         sampler.active.clear()
         part_ms["n_samples"] = reps
+    return dict(step_ms=step_ms, part_ms=part_ms, launches_per_step=launches_per_step, copies=copies,
+                n_copies=n_copies, per_copy=per_copy, barrier=barrier, graphs=graphs, part_graphs=part_graphs)
 
+
+def run_ours(args, rank: int, local_rank: int, world: int):
+    import gc
+    import torch
+    from paper_2606_08411_b200 import accounting, binding, workloads as W
+    from paper_2606_08411_b200.step import HostStep
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the library has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    peaks = load_peaks()
+    h = binding.Handle(local_rank)
+    stream = torch.cuda.Stream(device=dev)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+
+    # ---- the other single-GPU configs first (extra key `workloads`; fewer steps), then the headline one ----
+    extra = {}
+    if args.extra_workloads and world == 1:
+        for name in [w for w in args.extra_workloads.split(",") if w and w != args.workload]:
+            wl_x = W.CONFIGS[name]()
+            acc_x = accounting.summary(wl_x)
+            m = measure_resident(h, wl_x, dev, stream, None, sampler, min(args.steps, args.extra_steps), args.warmup)
+            parts_x = part_rooflines(wl_x, acc_x, m["part_ms"], m["step_ms"], peaks, load_traffic(wl_x.name))
+            extra[wl_x.name] = {
+                "step_us": m["step_ms"] * 1e3, "query_tok_per_s": acc_x["query_tokens"] / (m["step_ms"] * 1e-3),
+                "steps": min(args.steps, args.extra_steps), "layers": wl_x.n_layers, "query_rows": wl_x.total_q_rows,
+                "copies": m["n_copies"], "gpu_launches_per_step": m["launches_per_step"],
+                "parts": {k: {kk: p[kk] for kk in ("bound", "ms", "achieved", "peak", "unit", "frac", "traffic")}
+                          for k, p in parts_x.items()}}
+            del m, wl_x
+            gc.collect()
+            torch.cuda.empty_cache()
+
+    wl = W.CONFIGS[args.workload]()
+    acc = accounting.summary(wl)
+    m = measure_resident(h, wl, dev, stream, dist, sampler, args.steps, args.warmup, args.kernel_events)
+    step_ms, part_ms, launches_per_step = m["step_ms"], m["part_ms"], m["launches_per_step"]
+    copies, n_copies, per_copy, barrier, first = m["copies"], m["n_copies"], m["per_copy"], m["barrier"], m["copies"][0]
     step_ms_max = max_over_ranks(step_ms, dist, dev)
     value = whole_job_value(acc["query_tokens"], world, step_ms_max)
 
-    # ---- e2e: host buffers through al_lane_step_host ----------------------------------------------
-    hs = binding.al_host_step()
-    host = {}
-
-    def pin(name, arr, dtype=None):
-        tt = to_host_pinned(arr, dtype) if dtype else torch.from_numpy(np.ascontiguousarray(arr)).pin_memory()
-        host[name] = tt
-        return tt.data_ptr()
-
-    layer0 = 0
-    hs.q = pin("q", wl.q[layer0], wl.dtype)
-    hs.k_new = pin("k_new", wl.k_new[layer0], wl.dtype)
-    hs.v_new = pin("v_new", wl.v_new[layer0], wl.dtype)
-    hs.lanes = pin("lanes", wl.lanes.astype(np.int32))
-    hs.n_lanes, hs.total_q_rows, hs.max_prefix_len = wl.n_lanes, wl.total_q_rows, wl.max_prefix_len
-    hs.k_src = pin("k_src", wl.k_src[layer0], wl.dtype)
-    hs.v_src = pin("v_src", wl.v_src[layer0], wl.dtype)
-    hs.pos = pin("pos", wl.refresh_pos.astype(np.int32))
-    hs.n_pos, hs.refresh_base_row = int(wl.refresh_pos.size), wl.refresh_base_row
-    hs.logits = pin("logits", wl.logits, wl.dtype)
-    hs.n_rows, hs.vocab = wl.logits.shape
-    hs.tokens_in = pin("tokens", wl.tokens.astype(np.int32))
-    hs.mask_id, hs.eos_id, hs.threshold, hs.select_flags = wl.mask_id, wl.eos_id, float(wl.threshold), 0
-    tdt = torch.bfloat16 if wl.dtype == "bf16" else torch.float32
-    host["out"] = torch.empty((wl.total_q_rows, wl.n_q_heads, wl.head_dim), dtype=tdt).pin_memory()
-    host["conf"] = torch.empty(hs.n_rows, dtype=torch.float32).pin_memory()
-    host["argmax"] = torch.empty(hs.n_rows, dtype=torch.int32).pin_memory()
-    host["commit"] = torch.empty(hs.n_rows, dtype=torch.uint8).pin_memory()
-    host["tokens_out"] = torch.empty(hs.n_rows, dtype=torch.int32).pin_memory()
-    hs.out, hs.conf, hs.argmax = host["out"].data_ptr(), host["conf"].data_ptr(), host["argmax"].data_ptr()
-    hs.commit, hs.tokens_out = host["commit"].data_ptr(), host["tokens_out"].data_ptr()
-    arena = torch.empty(h.al_lane_step_host_arena_bytes(first.shape, hs) + 256, dtype=torch.uint8, device=dev)
-    h2d, d2h = h.al_lane_step_host_traffic(first.shape, hs)
+    # ---- e2e: host buffers through al_lane_step_host (every layer of the workload, like `value`) --------
+    hstep = HostStep(h, wl, device=dev)
+    h2d, d2h = hstep.h2d_bytes, hstep.d2h_bytes
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    e2e_warm = min(3, args.warmup) or 1
     before = h.al_launch_count
     with torch.cuda.stream(stream):
-        for i in range(min(3, args.warmup) or 1):
+        for i in range(e2e_warm):
             c = copies[i % n_copies]
-            h.al_lane_step_host(first.shape, hs, c.k_cache[layer0], c.v_cache[layer0], arena, stream)
-    e2e_launches = (h.al_launch_count - before) // (min(3, args.warmup) or 1)
+            hstep.run(c.k_cache, c.v_cache, stream)
+    e2e_launches = (h.al_launch_count - before) // e2e_warm
     barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler.active.set()
     t0 = time.perf_counter()
     with torch.cuda.stream(stream):
         e0.record(stream)
         for i in range(e2e_steps):
             c = copies[i % n_copies]
-            h.al_lane_step_host(first.shape, hs, c.k_cache[layer0], c.v_cache[layer0], arena, stream)
+            hstep.run(c.k_cache, c.v_cache, stream)
         e1.record(stream)
     barrier()
     wall_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
     sampler.active.clear()
     e2e_ms = max(e0.elapsed_time(e1) / e2e_steps, wall_ms)       # host-visible completion time
     e2e_ms = max_over_ranks(e2e_ms, dist, dev)
-    e2e_tokens = wl.total_q_rows                                  # one layer of the workload per host step
+    e2e_tokens = wl.total_q_rows                                  # all layers of the workload per host step
     sampler.stop_flag.set()
     sampler.join(timeout=2)
 
@@ -358,29 +383,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         return
 
     # ---- roofline of every part; `roofline` = the part with the largest share of the step ------
-    traffic = load_traffic(wl.name)
     parts = {}
     if part_ms:
-        ai = acc["attn_flops"] / acc["attn_bytes"]
-        ridge = peaks["tensor"] * 1e12 / (peaks["hbm"] * 1e9)
-        ta, tr, tc = (part_ms[k] * 1e-3 for k in ("attention", "refresh", "confidence"))
-        n_attn_launch = wl.n_layers                     # lane_attention_umma launches (+ 1 lane_plan launch per step)
-        if ai < ridge:
-            parts["attention"] = dict(bound="hbm", achieved=acc["attn_bytes"] / ta / 1e9, peak=peaks["hbm"], unit="GB/s")
-        else:
-            parts["attention"] = dict(bound="tensor", achieved=acc["attn_flops"] / ta / 1e12, peak=peaks["tensor"],
-                                      unit="TFLOP/s")
-        parts["attention"].update(ms=ta * 1e3, launches=n_attn_launch, tflops=acc["attn_flops"] / ta / 1e12,
-                                  gbs=acc["attn_bytes"] / ta / 1e9, arithmetic_intensity=ai,
-                                  note="time of al_lane_plan (1 launch) + al_lane_attention_planned (1 launch per layer)")
-        parts["refresh"] = dict(bound="hbm", achieved=acc["refresh_bytes"] / tr / 1e9, peak=peaks["hbm"], unit="GB/s",
-                                ms=tr * 1e3, launches=1)
-        parts["confidence"] = dict(bound="hbm", achieved=acc["confidence_bytes"] / tc / 1e9, peak=peaks["hbm"],
-                                   unit="GB/s", ms=tc * 1e3, launches=1)
-        for k, p in parts.items():
-            p["frac"] = p["achieved"] / p["peak"]
-            p["traffic"] = traffic.get(k)
-            p["share_of_step"] = p["ms"] / (step_ms)
+        parts = part_rooflines(wl, acc, part_ms, step_ms, peaks, load_traffic(wl.name))
         dom = max(parts, key=lambda k: parts[k]["ms"])
         roofline = {k: parts[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")}
         roofline.update(kernel=dom, peak_source=peaks["source"], avg_launch_ms=parts[dom]["ms"] / parts[dom]["launches"],
@@ -408,11 +413,12 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                             + "; the parts are also timed alone on graphs of their own"},
         "clocks": sampler.summary(),
         "e2e": {"value": whole_job_value(e2e_tokens, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps,
-                "api": "al_lane_step_host (pinned host buffers; H2D + kernels + D2H per step)",
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps, "layers": wl.n_layers,
+                "api": "al_lane_step_host (pinned host buffers; H2D + plan + attention per layer + refresh + "
+                       "confidence + D2H per step)",
                 "gpu_launches_per_step": e2e_launches},
         "gpu_launches": launches_per_step * args.steps,
-        "roofline": roofline, "parts": parts, "cpu_baseline": cpu,
+        "roofline": roofline, "parts": parts, "workloads": extra, "cpu_baseline": cpu,
         "algorithmic": acc, "peaks": peaks,
     }
     print(json.dumps(line), flush=True)
@@ -426,8 +432,11 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
-    ap.add_argument("--e2e-steps", type=int, default=100)
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--extra-workloads", default="cfg2,cfg3,cfg4",
+                    help="other configs measured in the same run and reported under `workloads` (N=1 only; '' = none)")
+    ap.add_argument("--extra-steps", type=int, default=400)
+    ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

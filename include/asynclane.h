@@ -17,7 +17,8 @@
  *  - Every hot call only ENQUEUES work on `cuda_stream` (a cudaStream_t passed as void*): no device
  *    synchronisation, no host read of device descriptors; all calls are CUDA-graph capturable.
  *  - Every call returns an al_status; nothing throws.  On error nothing has been launched, except
- *    AL_ERR_CUDA which reports a failed launch.  `al_last_error()` gives a thread-local message.
+ *    AL_ERR_CUDA which reports a failed launch or copy.  The calling thread's current CUDA device
+ *    must be the handle's device (al_create does not change it); otherwise AL_ERR_INVALID_ARG.  `al_last_error()` gives a thread-local message.
  *  - Sizes of 0 lanes / 0 positions / 0 rows are valid no-ops returning AL_OK.
  *  - 16-byte alignment is required of q, k_new, v_new, caches, out, k_src, v_src, logits rows
  *    (row_stride * element size % 16 == 0 for the vector path; otherwise a scalar path is used)
@@ -110,8 +111,12 @@ int32_t al_sm_count(const al_handle* handle);
  * query tiles (ceil(total_q_rows / (2 * floor(128 / n_rep))) + n_lanes); beyond them AL_ERR_UNSUPPORTED.
  * Results are deterministic: the same inputs give bit-identical outputs from call to call.
  * Rows of Q not covered by any lane are not written in `out`.
- * Cache rows of a group up to its largest prefix_len rounded up to 16 must hold finite values
- * (they are multiplied by exact zeros where a lane may not see them).
+ * Finite-input contract (reading C14): every row of q, k_new and v_new in [0, total_q_rows) and every
+ * cache row that SOME lane of the call may see must hold finite values -- lanes share 128-row tensor-core
+ * tiles, so a NaN/Inf in one lane's K_new/V_new rows reaches the rows stacked with it (0 x NaN).  Cache rows
+ * that NO lane sees (beyond the longest prefix_len of the lanes addressing that region: unwritten or
+ * recycled memory) may hold anything, NaN included: their scores are masked by selection, their
+ * probabilities are exact zeros and the V rows the last key tile rounds up to are zeroed on chip.
  */
 size_t al_lane_attention_workspace_bytes(const al_attn_shape* shape, int32_t n_lanes,
                                          int32_t total_q_rows, int32_t max_prefix_len);
@@ -152,7 +157,8 @@ al_status al_lane_attention_planned(al_handle* handle, const al_attn_shape* shap
  * Bit copy; every other byte of the caches is untouched.  Layouts: caches [H_kv][cache_rows][d] per
  * layer, layers `layer_stride_cache` ELEMENTS apart; src [R][H_kv][d] per layer, layers
  * `layer_stride_src` elements apart.  Precondition: pos strictly increasing (unique), each
- * kv_base_row + pos[r] in [0, cache_rows).  Duplicates make the result order-dependent.
+ * kv_base_row + pos[r] in [0, cache_rows).  Duplicates make the result order-dependent; the hot call
+ * cannot check device-resident positions without synchronising -- al_validate_refresh does.
  * head_dim * element size must be a multiple of 16.
  */
 al_status al_kv_refresh(al_handle* handle, const al_attn_shape* shape, void* k_cache, void* v_cache,
@@ -173,6 +179,9 @@ al_status al_kv_refresh(al_handle* handle, const al_attn_shape* shape, void* k_c
  *     largest confidence (lowest row on ties).  Without lanes, all rows form one generate lane.
  *   tokens_out[i] = commit ? argmax : tokens_in[i]     (tokens_out may alias tokens_in)
  * conf is computed in fp32 from the dtype-rounded logits.  Rows must hold at least one finite value.
+ * No workspace is needed (partials are merged on chip through cluster shared memory):
+ * al_confidence_select_workspace_bytes returns 0 and `workspace` may be NULL; both stay in the
+ * signature so that callers size arenas through one query per call.
  */
 size_t al_confidence_select_workspace_bytes(int32_t n_rows, int32_t vocab);
 al_status al_confidence_select(al_handle* handle, const void* logits, int32_t logits_dtype,
@@ -186,22 +195,24 @@ al_status al_confidence_select(al_handle* handle, const void* logits, int32_t lo
 /* ---- whole step from HOST buffers (end-to-end entry) ------------------------------------------ */
 
 /*
- * One lane-batched denoising step (one layer) whose per-step inputs and
- * results live in HOST memory (pinned for true asynchrony): the call enqueues, on `cuda_stream`,
- * the host->device copies of the inputs into `arena_dev`, then al_lane_attention, al_kv_refresh and
- * al_confidence_select on the device copies, then the device->host copies of the results.  It does
- * not synchronise: the caller synchronises the stream before reading the outputs or reusing the
- * host inputs.  The KV cache is persistent device state (kappa_l is carried between
- * iterations) and is passed as device pointers; attention reads it before this step's refresh
- * writes it.  Every pointer inside al_host_step is a HOST pointer owned by the caller.
+ * One lane-batched denoising step (all n_layers layers) whose per-step inputs
+ * and results live in HOST memory (pinned for true asynchrony): the call validates all three parts
+ * (on error nothing has been enqueued), then enqueues, on `cuda_stream`, the host->device copies of
+ * the inputs into `arena_dev`, al_lane_plan once and al_lane_attention_planned per layer, the
+ * layer-batched al_kv_refresh and al_confidence_select on the device copies, then the device->host
+ * copies of the results.  It does not synchronise: the caller synchronises the stream before reading
+ * the outputs or reusing the host inputs.  The KV cache is persistent device state (PAPER.md L70:
+ * kappa_l is carried between iterations) and is passed as device pointers, layers
+ * `cache_layer_stride` elements apart; attention reads it before this step's refresh writes it.
+ * Every pointer inside al_host_step is a HOST pointer owned by the caller; L = max(n_layers, 1).
  */
 typedef struct {
-  const void* q;            /* [T][H_q][d]                                  */
-  const void* k_new;        /* [T][H_kv][d]                                 */
-  const void* v_new;        /* [T][H_kv][d]                                 */
+  const void* q;            /* [L][T][H_q][d]                               */
+  const void* k_new;        /* [L][T][H_kv][d]                              */
+  const void* v_new;        /* [L][T][H_kv][d]                              */
   const al_lane_desc* lanes;/* [n_lanes]                                    */
   int32_t n_lanes, total_q_rows, max_prefix_len;
-  const void* k_src;        /* [n_pos][H_kv][d] recomputed rows (Eq.12)     */
+  const void* k_src;        /* [L][n_pos][H_kv][d] recomputed rows (Eq.12)  */
   const void* v_src;
   const int32_t* pos;       /* [n_pos] strictly increasing                  */
   int32_t n_pos, refresh_base_row;
@@ -211,11 +222,14 @@ typedef struct {
   int32_t mask_id, eos_id;
   float threshold;
   int32_t select_flags;     /* AL_SELECT_*                                  */
-  void* out;                /* [T][H_q][d]   result, host                   */
+  void* out;                /* [L][T][H_q][d]   result, host                */
   float* conf;              /* [n_rows]                                     */
   int32_t* argmax;          /* [n_rows]                                     */
   uint8_t* commit;          /* [n_rows]                                     */
   int32_t* tokens_out;      /* [n_rows]                                     */
+  int32_t n_layers;         /* layers of the model call; 0 is read as 1     */
+  int32_t reserved;         /* must be 0                                    */
+  int64_t cache_layer_stride; /* elements between layers of k/v_cache_dev   */
 } al_host_step;
 
 /* Bytes of device scratch al_lane_step_host needs for these sizes (0 on invalid arguments). */
@@ -236,6 +250,11 @@ uint64_t al_launch_count(const al_handle* handle);
 /* Copies the descriptors to the host and checks the preconditions listed above.  Synchronises. */
 al_status al_validate_lanes(al_handle* handle, const al_attn_shape* shape,
                             const al_lane_desc* lanes_dev, int32_t n_lanes, int32_t total_q_rows);
+/* Copies the refresh positions to the host and checks al_kv_refresh's preconditions (Eq.12
+ * rewrites each refreshed position once): pos strictly increasing -- hence unique -- and every
+ * kv_base_row + pos[r] inside [0, cache_rows).  Synchronises. */
+al_status al_validate_refresh(al_handle* handle, const al_attn_shape* shape, const int32_t* pos_dev,
+                              int32_t n_pos, int32_t kv_base_row);
 
 /*
  * tcgen05 encoding self-test: one 128x128x128 bf16 tile pipeline through the same TMA maps, shared

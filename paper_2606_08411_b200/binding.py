@@ -22,7 +22,7 @@ EXPORTS = [
     "al_create", "al_destroy", "al_last_error", "al_version", "al_sm_count",
     "al_lane_attention_workspace_bytes", "al_lane_attention", "al_lane_plan", "al_lane_attention_planned",
     "al_kv_refresh",
-    "al_confidence_select_workspace_bytes", "al_confidence_select", "al_validate_lanes",
+    "al_confidence_select_workspace_bytes", "al_confidence_select", "al_validate_lanes", "al_validate_refresh",
     "al_selftest_umma", "al_lane_step_host", "al_lane_step_host_arena_bytes", "al_lane_step_host_traffic",
     "al_launch_count",
 ]
@@ -51,7 +51,8 @@ class al_host_step(ctypes.Structure):
                 ("tokens_in", ctypes.c_void_p), ("mask_id", ctypes.c_int32), ("eos_id", ctypes.c_int32),
                 ("threshold", ctypes.c_float), ("select_flags", ctypes.c_int32),
                 ("out", ctypes.c_void_p), ("conf", ctypes.c_void_p), ("argmax", ctypes.c_void_p),
-                ("commit", ctypes.c_void_p), ("tokens_out", ctypes.c_void_p)]
+                ("commit", ctypes.c_void_p), ("tokens_out", ctypes.c_void_p),
+                ("n_layers", ctypes.c_int32), ("reserved", ctypes.c_int32), ("cache_layer_stride", ctypes.c_int64)]
 
 
 _lib: Optional[ctypes.CDLL] = None
@@ -87,6 +88,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.al_confidence_select.argtypes = [vp, vp, i32, i32, i32, i64, vp, i32, i32, f32, vp, i32, i32,
                                          vp, vp, vp, vp, vp, sz, vp]
     lib.al_validate_lanes.argtypes = [vp, shp, vp, i32, i32]
+    lib.al_validate_refresh.argtypes = [vp, shp, vp, i32, i32]
     lib.al_selftest_umma.argtypes = [vp, vp, vp, vp, f32, vp, vp, vp]
     hsp = ctypes.POINTER(al_host_step)
     lib.al_lane_step_host_arena_bytes.argtypes = [shp, hsp]
@@ -233,6 +235,9 @@ class Handle:
 
     def al_validate_lanes(self, shape, lanes_dev, n_lanes, total_q_rows) -> None:
         _check(self._lib.al_validate_lanes(self._h, ctypes.byref(shape), _ptr(lanes_dev), n_lanes, total_q_rows))
+
+    def al_validate_refresh(self, shape, pos_dev, n_pos, kv_base_row=0) -> None:
+        _check(self._lib.al_validate_refresh(self._h, ctypes.byref(shape), _ptr(pos_dev), n_pos, kv_base_row))
 
     def al_selftest_umma(self, a, b, v, p_scale, s_out, o_out, stream=None) -> None:
         _check(self._lib.al_selftest_umma(self._h, _ptr(a), _ptr(b), _ptr(v), p_scale, _ptr(s_out), _ptr(o_out),

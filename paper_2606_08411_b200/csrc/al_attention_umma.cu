@@ -42,6 +42,7 @@
 
 #include "al_internal.h"
 #include "al_ptx.cuh"
+#include "al_debug.cuh"
 
 using namespace alptx;
 
@@ -423,26 +424,6 @@ __device__ __forceinline__ void tmem_ld32_f(uint32_t taddr, float* dst) {
 #pragma unroll
   for (int i = 0; i < 32; ++i) dst[i] = __uint_as_float(r[i]);
 }
-#ifdef AL_ATTN_TRACE
-// debug build only: per-CTA clock64 stamps of the first piece (slot 15 = globaltimer at entry)
-__device__ unsigned long long g_trace[kMaxCtas * 16];
-#define TRACE(i) do { if (g_trace[blockIdx.x * 16 + (i)] == 0) g_trace[blockIdx.x * 16 + (i)] = clock64(); } while (0)
-// CTA 0 only: per step (first 32 of the CTA) stamps of kind k: 0 QK_A issued, 1 S seen by stream A, 2 P_A ready, 3 PV_A issued
-__device__ unsigned long long g_trace_tile[16 * 32];
-#define TRACE_TILE(k, i) do { if (blockIdx.x == 0 && (i) < 32) g_trace_tile[(k) * 32 + (i)] = clock64(); } while (0)
-// CTA 0, step 4 of each stream: per warp (8 softmax warps) stamps 0 S seen, 1 S in registers, 2 max done, 3 P stored, 4 arrived
-__device__ unsigned long long g_trace_warp[8 * 8];
-#define TRACE_W(k) do { if (blockIdx.x == 0 && cnt == 4 && lane == 0) g_trace_warp[(warp - 4) * 8 + (k)] = clock64(); } while (0)
-__device__ unsigned long long g_trace_epi[16];
-#define TRACE_E(k) do { if (blockIdx.x == 0 && warp == 4 && lane == 0 && g_trace_epi[k] == 0) g_trace_epi[k] = clock64(); } while (0)
-#define TRACE_M(k) do { if (blockIdx.x == 12 && tid128 == 0 && b == 0 && g_trace_epi[k] == 0) g_trace_epi[k] = clock64(); } while (0)
-#else
-#define TRACE_E(k) do { } while (0)
-#define TRACE_M(k) do { } while (0)
-#define TRACE_W(k) do { } while (0)
-#define TRACE(i) do { } while (0)
-#define TRACE_TILE(k, i) do { } while (0)
-#endif
 __device__ __forceinline__ void bar_sync_both() { asm volatile("bar.sync 3, 256;" ::: "memory"); }
 __device__ __forceinline__ void bar_sync_stream(int b) { asm volatile("bar.sync %0, 128;" ::"r"(1 + b) : "memory"); }
 __device__ __forceinline__ float ex2(float x) {             // x <= 8 here (or -inf)
@@ -753,6 +734,19 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             for (int k = 0; k < kBN / 16; ++k)                                                                 \
               if (leader) mma_ts(to, tp + u_ * 32 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
           } else {                                                                                             \
+            /* ragged tail: the key rows [valid_, 16 ksteps_) of the V tile are rows no lane may see (cache  */ \
+            /* rows beyond the group's longest prefix: unwritten or recycled memory).  P is exactly 0 there, */ \
+            /* but 0 x NaN/Inf would still poison every row of the tile, so they are zeroed in shared memory */ \
+            /* before the MMA reads them (both issuers may do it: same zeros).                               */ \
+            if (valid_ & 15) {                                                                                 \
+              const int nz_ = ksteps_ * 16 - valid_;                 /* 1..15 key rows of 128 bytes per half */ \
+              for (int j_ = lane; j_ < nz_ * 16; j_ += 32) {                                                   \
+                const int row_ = valid_ + (j_ >> 4), hc_ = j_ & 15;  /* half = hc_ >> 3, 16-byte chunk hc_ & 7 */ \
+                *reinterpret_cast<uint4*>(sm.v[sv_][hc_ >> 3] + row_ * 128 + (hc_ & 7) * 16) = make_uint4(0u, 0u, 0u, 0u); \
+              }                                                                                                \
+              fence_proxy_async_smem();                                                                        \
+              __syncwarp();                                                                                    \
+            }                                                                                                  \
             _Pragma("unroll")                                                                                  \
             for (int k = 0; k < kBN / 16; ++k)                                                                 \
               if (leader && k < ksteps_) mma_ts(to, tp + u_ * 32 + k * 8, dv_ + (uint64_t)(k * 128), idesc_pv, (!first || k) ? 1u : 0u); \
@@ -879,8 +873,9 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         }
         const bool need_mask = valid && (lo > 0 || hi < kBN);
         uint32_t hidden = 0;                             // bit c: 32-column chunk c is entirely hidden from this row
-        if (__any_sync(0xffffffffu, need_mask)) {        // warp-uniform: only ragged prefix tails and local tiles
-          uint32_t vis[kBN / 32];                        // bit e of vis[c]: column 32 c + e is visible
+        uint32_t vis[kBN / 32] = {0xffffffffu, 0xffffffffu};   // bit e of vis[c]: column 32 c + e is visible
+        const bool masked_tile = __any_sync(0xffffffffu, need_mask);
+        if (masked_tile) {                               // warp-uniform: only ragged prefix tails and local tiles
 #pragma unroll
           for (int c4 = 0; c4 < kBN / 32; ++c4) {
             const int a = min(32, max(0, lo - c4 * 32)), z = min(32, max(0, hi - c4 * 32));   // visible [a, z) of the chunk
@@ -948,6 +943,15 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
               if (e & 1) sum_b = fadd2(sum_b, pack2(p0, p1)); else sum_a = fadd2(sum_a, pack2(p0, p1));
               pk[e] = pack_bf16x2(p0, p1);
             }
+            if (masked_tile) {
+              // the polynomial path clamps masked scores at -126 and returns 2^-126, not 0: hidden columns are
+              // set to exact zeros, so that whatever the V row holds cannot reach this row (0 x finite = 0)
+#pragma unroll
+              for (int e = 0; e < 16; ++e) {
+                const uint32_t two = (vis[c] >> (2 * e)) & 3u;
+                pk[e] &= (two & 1u ? 0x0000ffffu : 0u) | (two & 2u ? 0xffff0000u : 0u);
+              }
+            }
           }
           tmem_st16(t_p + lane_addr + c * 16, pk);
         }
@@ -979,6 +983,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         if (tid128 == 0) sm.alt_has[b] = n_mine > 0;
         *reinterpret_cast<float2*>(my_stage) = make_float2(m_used, l_sum);   // exchanged through the staging rows
         bar_sync_both();
+        tc_fence_after();                              // the other stream's accumulator is read below, behind its thread's o_full wait
         TRACE_E(1);
         const float2 oth = *reinterpret_cast<const float2*>(sm.stage + ((b ^ 1) * kBM + r) * kStagePitch);
         const bool has0 = sm.alt_has[0] != 0, has1 = sm.alt_has[1] != 0;
@@ -1141,15 +1146,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   // from it (stream index, TMEM and shared-memory descriptors) then live in uniform registers
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
 
-#ifdef AL_ATTN_TRACE
-  if (threadIdx.x == 0) {
-    if (blockIdx.x == 0 || blockIdx.x == 12) for (int i = (blockIdx.x ? 11 : 0); i < (blockIdx.x ? 16 : 11); ++i) g_trace_epi[i] = 0;
-    for (int i = 0; i < 16; ++i) g_trace[blockIdx.x * 16 + i] = 0;
-    unsigned long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-    g_trace[blockIdx.x * 16 + 15] = gt;
-    g_trace[blockIdx.x * 16 + 0] = clock64();
-  }
-#endif
+  TRACE_RESET();
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) __trap();          // the 128-byte swizzle atoms need 1024-byte alignment
     mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 2);       // the *_empty barriers collect both MMA issuers
@@ -1183,12 +1180,6 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   if (warp == 1) { __syncwarp(); tmem_dealloc<512>(tmem); }
   if (threadIdx.x == 32) TRACE(14);
 }
-#ifdef AL_ATTN_TRACE
-int trace_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace)); }
-int trace_epi_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_epi, sizeof(g_trace_epi)); }
-int trace_warp_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_warp, sizeof(g_trace_warp)); }
-int trace_tile_read(unsigned long long* host_out) { return (int)cudaMemcpyFromSymbol(host_out, g_trace_tile, sizeof(g_trace_tile)); }
-#endif
 
 // ---------------------------------------------------------------------------------------------
 // host side
@@ -1264,6 +1255,10 @@ bool al_attention_umma_supported(const al_attn_shape* s) {
   return n_rep >= 1 && n_rep <= kBM;
 }
 
+al_status al_attention_umma_check(const al_handle* h, const al_attn_shape* s, int n_lanes, int total_q_rows) {
+  return check_plan_bounds(s, n_lanes, bounds_for(s, n_lanes, total_q_rows, h->sm_count));
+}
+
 size_t al_attention_umma_workspace_bytes(const al_handle* h, const al_attn_shape* s, int n_lanes, int total_q_rows,
                                          int max_prefix_len) {
   (void)max_prefix_len;
@@ -1333,13 +1328,3 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   h->launches += 1;
   return AL_OK;
 }
-
-#ifdef AL_ATTN_TRACE
-extern "C" int al_debug_attn_trace(unsigned long long* host_out) { return trace_read(host_out); }   // [kMaxCtas * 16]
-extern "C" int al_debug_attn_trace_epi(unsigned long long* host_out) { return trace_epi_read(host_out); }   // [16]
-extern "C" int al_debug_attn_trace_warp(unsigned long long* host_out) { return trace_warp_read(host_out); }   // [8 * 8]
-extern "C" int al_debug_attn_trace_tile(unsigned long long* host_out) { return trace_tile_read(host_out); }   // [4 * 32]
-extern "C" int al_debug_mbar_timeout(unsigned int* host_out) {   // [4]; [0] != 0 when a wait timed out
-  return (int)cudaMemcpyFromSymbol(host_out, alptx::g_mbar_timeout, 16);
-}
-#endif

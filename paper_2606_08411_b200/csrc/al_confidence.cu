@@ -369,9 +369,33 @@ cudaError_t launch_select(int k, int n_rows, cudaStream_t cs, const T* logits, i
 
 }  // namespace
 
+// The cluster/DSMEM merge keeps every partial on chip: no HBM workspace is needed.  The entry point stays in
+// the ABI (callers size their arenas through it) and returns 0; al_confidence_select accepts workspace == NULL.
 extern "C" size_t al_confidence_select_workspace_bytes(int32_t n_rows, int32_t vocab) {
-  if (n_rows <= 0 || vocab <= 0) return 0;
-  return (size_t)n_rows * 16;   // reserved (cluster/DSMEM merge needs no HBM partials); kept for ABI stability
+  (void)n_rows; (void)vocab;
+  return 0;
+}
+
+al_status al_confidence_select_check(const char* who, const al_handle* h, const void* logits, int32_t dtype,
+                                     int32_t n_rows, int32_t vocab, int64_t row_stride, const int32_t* tokens_in,
+                                     int32_t eos_id, const al_lane_desc* lanes, int32_t n_lanes, int32_t flags,
+                                     const float* conf_out, const int32_t* argmax_out, const uint8_t* commit_out,
+                                     const int32_t* tokens_out) {
+  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "%s: handle is NULL", who);
+  if (dtype != AL_F32 && dtype != AL_BF16) AL_FAIL(AL_ERR_INVALID_ARG, "%s: bad dtype %d", who, dtype);
+  if (n_rows < 0 || vocab < 0 || n_lanes < 0 || row_stride < vocab)
+    AL_FAIL(AL_ERR_INVALID_ARG, "%s: bad sizes n_rows %d vocab %d row_stride %lld", who, n_rows, vocab, (long long)row_stride);
+  if (flags & ~AL_SELECT_FORCE_TOP1) AL_FAIL(AL_ERR_INVALID_ARG, "%s: unknown flags %d", who, flags);
+  if (n_rows == 0) return AL_OK;
+  const al_status st = al_check_device(h, who);
+  if (st != AL_OK) return st;
+  if (vocab == 0) AL_FAIL(AL_ERR_INVALID_ARG, "%s: vocab is 0", who);
+  if (!logits || !tokens_in || !conf_out || !argmax_out || !commit_out || !tokens_out)
+    AL_FAIL(AL_ERR_INVALID_ARG, "%s: NULL pointer", who);
+  if (n_lanes > 0 && !lanes) AL_FAIL(AL_ERR_INVALID_ARG, "%s: n_lanes > 0 but lanes is NULL", who);
+  if (eos_id >= vocab) AL_FAIL(AL_ERR_INVALID_ARG, "%s: eos_id %d >= vocab %d", who, eos_id, vocab);
+  if ((long long)n_rows * kMaxCluster > 0x7fffffffLL) AL_FAIL(AL_ERR_UNSUPPORTED, "%s: too many rows", who);
+  return AL_OK;
 }
 
 extern "C" al_status al_confidence_select(al_handle* h, const void* logits, int32_t dtype, int32_t n_rows,
@@ -381,21 +405,12 @@ extern "C" al_status al_confidence_select(al_handle* h, const void* logits, int3
                                           float* conf_out, int32_t* argmax_out, uint8_t* commit_out,
                                           int32_t* tokens_out, void* workspace, size_t workspace_bytes,
                                           void* stream) {
-  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: handle is NULL");
-  if (dtype != AL_F32 && dtype != AL_BF16) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: bad dtype %d", dtype);
-  if (n_rows < 0 || vocab < 0 || n_lanes < 0 || row_stride < vocab)
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: bad sizes n_rows %d vocab %d row_stride %lld", n_rows, vocab, (long long)row_stride);
-  if (flags & ~AL_SELECT_FORCE_TOP1) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: unknown flags %d", flags);
+  (void)workspace; (void)workspace_bytes;
+  const al_status st = al_confidence_select_check("al_confidence_select", h, logits, dtype, n_rows, vocab, row_stride,
+                                                  tokens_in, eos_id, lanes, n_lanes, flags, conf_out, argmax_out,
+                                                  commit_out, tokens_out);
+  if (st != AL_OK) return st;
   if (n_rows == 0) return AL_OK;
-  if (vocab == 0) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: vocab is 0");
-  if (!logits || !tokens_in || !conf_out || !argmax_out || !commit_out || !tokens_out)
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: NULL pointer");
-  if (n_lanes > 0 && !lanes) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: n_lanes > 0 but lanes is NULL");
-  if (eos_id >= vocab) AL_FAIL(AL_ERR_INVALID_ARG, "al_confidence_select: eos_id %d >= vocab %d", eos_id, vocab);
-  const size_t need = al_confidence_select_workspace_bytes(n_rows, vocab);
-  if (!workspace || workspace_bytes < need || !al_aligned16(workspace))
-    AL_FAIL(AL_ERR_WORKSPACE, "al_confidence_select: workspace %zu < %zu (or unaligned)", workspace_bytes, need);
-  if ((long long)n_rows * kMaxCluster > 0x7fffffffLL) AL_FAIL(AL_ERR_UNSUPPORTED, "al_confidence_select: too many rows");
   const int esz = al_esize(dtype);
   const bool vec = al_aligned16(logits) && ((row_stride * esz) % 16 == 0);
   cudaStream_t cs = static_cast<cudaStream_t>(stream);

@@ -67,27 +67,41 @@ kv_refresh_kernel(int4* __restrict__ k_cache, int4* __restrict__ v_cache,
 
 }  // namespace
 
+al_status al_kv_refresh_check(const char* who, const al_handle* h, const al_attn_shape* s, const void* k_cache,
+                              const void* v_cache, const void* k_src, const void* v_src, const int32_t* pos_dev,
+                              int32_t n_pos, int32_t kv_base_row, int32_t n_layers, int64_t layer_stride_cache,
+                              int64_t layer_stride_src) {
+  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "%s: handle is NULL", who);
+  al_status st = al_check_shape(s, who);
+  if (st != AL_OK) return st;
+  if (n_pos < 0 || n_layers < 0 || kv_base_row < 0 || layer_stride_cache < 0 || layer_stride_src < 0)
+    AL_FAIL(AL_ERR_INVALID_ARG, "%s: negative size", who);
+  if (n_pos == 0 || n_layers == 0) return AL_OK;
+  if ((st = al_check_device(h, who)) != AL_OK) return st;
+  if (!k_cache || !v_cache || !k_src || !v_src || !pos_dev) AL_FAIL(AL_ERR_INVALID_ARG, "%s: NULL pointer", who);
+  const int esz = al_esize(s->dtype);
+  const long long row_bytes = (long long)s->head_dim * esz;
+  if (row_bytes % 16 != 0) AL_FAIL(AL_ERR_UNSUPPORTED, "%s: head_dim*esize = %lld not a multiple of 16", who, row_bytes);
+  if (!al_aligned16(k_cache) || !al_aligned16(v_cache) || !al_aligned16(k_src) || !al_aligned16(v_src))
+    AL_FAIL(AL_ERR_INVALID_ARG, "%s: pointers must be 16-byte aligned", who);
+  if ((layer_stride_cache * esz) % 16 != 0 || (layer_stride_src * esz) % 16 != 0)
+    AL_FAIL(AL_ERR_INVALID_ARG, "%s: layer strides must be multiples of 16 bytes", who);
+  if (n_layers > 1 && (layer_stride_cache < (int64_t)s->n_kv_heads * s->cache_rows * s->head_dim ||
+                       layer_stride_src < (int64_t)n_pos * s->n_kv_heads * s->head_dim))
+    AL_FAIL(AL_ERR_INVALID_ARG, "%s: layer strides smaller than one layer", who);
+  return AL_OK;
+}
+
 extern "C" al_status al_kv_refresh(al_handle* h, const al_attn_shape* s, void* k_cache, void* v_cache,
                                    const void* k_src, const void* v_src, const int32_t* pos_dev,
                                    int32_t n_pos, int32_t kv_base_row, int32_t n_layers,
                                    int64_t layer_stride_cache, int64_t layer_stride_src, void* stream) {
-  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: handle is NULL");
-  al_status st = al_check_shape(s, "al_kv_refresh");
+  const al_status st = al_kv_refresh_check("al_kv_refresh", h, s, k_cache, v_cache, k_src, v_src, pos_dev, n_pos,
+                                           kv_base_row, n_layers, layer_stride_cache, layer_stride_src);
   if (st != AL_OK) return st;
-  if (n_pos < 0 || n_layers < 0 || kv_base_row < 0 || layer_stride_cache < 0 || layer_stride_src < 0)
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: negative size");
   if (n_pos == 0 || n_layers == 0) return AL_OK;
-  if (!k_cache || !v_cache || !k_src || !v_src || !pos_dev) AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: NULL pointer");
   const int esz = al_esize(s->dtype);
   const long long row_bytes = (long long)s->head_dim * esz;
-  if (row_bytes % 16 != 0) AL_FAIL(AL_ERR_UNSUPPORTED, "al_kv_refresh: head_dim*esize = %lld not a multiple of 16", row_bytes);
-  if (!al_aligned16(k_cache) || !al_aligned16(v_cache) || !al_aligned16(k_src) || !al_aligned16(v_src))
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: pointers must be 16-byte aligned");
-  if ((layer_stride_cache * esz) % 16 != 0 || (layer_stride_src * esz) % 16 != 0)
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: layer strides must be multiples of 16 bytes");
-  if (n_layers > 1 && (layer_stride_cache < (int64_t)s->n_kv_heads * s->cache_rows * s->head_dim ||
-                       layer_stride_src < (int64_t)n_pos * s->n_kv_heads * s->head_dim))
-    AL_FAIL(AL_ERR_INVALID_ARG, "al_kv_refresh: layer strides smaller than one layer");
   const int vpr = (int)(row_bytes / 16);
   const long long items_per_layer = (long long)n_pos * s->n_kv_heads * vpr;
   const long long total = items_per_layer * n_layers;

@@ -155,3 +155,54 @@ class LaneStep:
         self.confidence(stream)
         if marks is not None:
             marks[3].record(s)
+
+
+class HostStep:
+    """Pinned HOST buffers of one workload + the al_host_step struct for al_lane_step_host (the e2e entry):
+    every layer's Q/K_new/V_new and refresh rows, the logits and the result buffers.  Marshalling only."""
+
+    def __init__(self, handle: B.Handle, wl: LaneStepWorkload, device="cuda:0", force_top1: bool = False):
+        self.h, self.wl = handle, wl
+        dev = torch.device(device)
+        dt = wl.dtype
+        code = B.AL_BF16 if dt == "bf16" else B.AL_F32
+        tdt = torch.bfloat16 if dt == "bf16" else torch.float32
+        self.shape = B.Handle.make_shape(wl.n_q_heads, wl.n_kv_heads, wl.head_dim, code, wl.cache_rows)
+        hs = B.al_host_step()
+        self.host = {}
+
+        def pin(name, arr, dtype=None):
+            t = to_host_pinned(arr, dtype) if dtype else torch.from_numpy(np.ascontiguousarray(arr)).pin_memory()
+            self.host[name] = t
+            return t.data_ptr()
+
+        L, T = wl.n_layers, wl.total_q_rows
+        hs.q, hs.k_new, hs.v_new = pin("q", wl.q, dt), pin("k_new", wl.k_new, dt), pin("v_new", wl.v_new, dt)
+        hs.lanes = pin("lanes", wl.lanes.astype(np.int32))
+        hs.n_lanes, hs.total_q_rows, hs.max_prefix_len = wl.n_lanes, T, wl.max_prefix_len
+        hs.k_src, hs.v_src = pin("k_src", wl.k_src, dt), pin("v_src", wl.v_src, dt)
+        hs.pos = pin("pos", wl.refresh_pos.astype(np.int32))
+        hs.n_pos, hs.refresh_base_row = int(wl.refresh_pos.size), wl.refresh_base_row
+        hs.logits = pin("logits", wl.logits, dt)
+        hs.n_rows, hs.vocab = wl.logits.shape
+        hs.tokens_in = pin("tokens", wl.tokens.astype(np.int32))
+        hs.mask_id, hs.eos_id, hs.threshold = wl.mask_id, wl.eos_id, float(wl.threshold)
+        hs.select_flags = B.AL_SELECT_FORCE_TOP1 if force_top1 else 0
+        N = int(hs.n_rows)
+        self.out = torch.empty((L, T, wl.n_q_heads, wl.head_dim), dtype=tdt).pin_memory()
+        self.conf = torch.empty(N, dtype=torch.float32).pin_memory()
+        self.argmax = torch.empty(N, dtype=torch.int32).pin_memory()
+        self.commit = torch.empty(N, dtype=torch.uint8).pin_memory()
+        self.tokens_out = torch.empty(N, dtype=torch.int32).pin_memory()
+        hs.out, hs.conf, hs.argmax = self.out.data_ptr(), self.conf.data_ptr(), self.argmax.data_ptr()
+        hs.commit, hs.tokens_out = self.commit.data_ptr(), self.tokens_out.data_ptr()
+        hs.n_layers, hs.reserved = L, 0
+        hs.cache_layer_stride = wl.n_kv_heads * wl.cache_rows * wl.head_dim
+        self.hs = hs
+        self.arena = torch.empty(handle.al_lane_step_host_arena_bytes(self.shape, hs) + 256, dtype=torch.uint8,
+                                 device=dev)
+        self.h2d_bytes, self.d2h_bytes = handle.al_lane_step_host_traffic(self.shape, hs)
+
+    def run(self, k_cache: torch.Tensor, v_cache: torch.Tensor, stream=None) -> None:
+        """Enqueues one whole step on `stream`; k_cache/v_cache are the resident device caches [L,Hkv,rows,d]."""
+        self.h.al_lane_step_host(self.shape, self.hs, k_cache, v_cache, self.arena, stream)

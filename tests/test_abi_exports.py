@@ -40,6 +40,19 @@ def test_lane_desc_and_shape_struct_layouts():
 
 def test_workspace_queries_need_no_gpu():
     lib = binding.load_library()
+    # the cluster/DSMEM merge keeps no partials in HBM: confidence_select needs no workspace at all
     assert lib.al_confidence_select_workspace_bytes(0, 100) == 0
-    # the cluster/DSMEM merge keeps no partials in HBM: the workspace is a small reserved slot per row
-    assert 0 < lib.al_confidence_select_workspace_bytes(4, 126464) <= 4 * 64
+    assert lib.al_confidence_select_workspace_bytes(4, 126464) == 0
+    shape = binding.Handle.make_shape(28, 4, 128, binding.AL_BF16, 2048)
+    assert lib.al_lane_attention_workspace_bytes(ctypes.byref(shape), 8, 256, 1024) > 0
+
+
+def test_host_step_struct_matches_the_header():
+    """al_host_step mirrors the C struct: 25 pointer/int fields, then n_layers, reserved, cache_layer_stride."""
+    names = [f[0] for f in binding.al_host_step._fields_]
+    assert names[-3:] == ["n_layers", "reserved", "cache_layer_stride"]
+    text = open(os.path.join(ROOT, "include", "asynclane.h")).read()
+    body = text[text.index("typedef struct {\n  const void* q;"):text.index("} al_host_step;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    declared = re.findall(r"\b([a-z_0-9]+)\s*[;,]", body)
+    assert declared == names

@@ -466,10 +466,19 @@ def test_abi_error_codes(handle):
         handle.al_lane_attention(bad, st.q[0], st.k_new[0], st.v_new[0], st.k_cache[0], st.v_cache[0], st.lanes,
                                  2, 16, 64, st.out[0])
     assert e.value.status == B.AL_ERR_INVALID_ARG
+    big = make_step(handle, W.ragged_case(402))                  # tensor-core path: it needs its plan workspace
     with pytest.raises(B.AlError) as e:                          # workspace too small
-        handle.al_confidence_select(st.logits, st.N, st.V, st.V, st.tokens, 511, -1, 0.9, None, 0, 0, st.conf,
-                                    st.argmax, st.commit, st.tokens_out, torch.empty(16, dtype=torch.uint8, device="cuda"))
+        handle.al_lane_attention(big.shape, big.q[0], big.k_new[0], big.v_new[0], big.k_cache[0], big.v_cache[0],
+                                 big.lanes, big.wl.n_lanes, big.T, big.max_prefix, big.out[0], None,
+                                 torch.empty(256, dtype=torch.uint8, device="cuda"))
     assert e.value.status == B.AL_ERR_WORKSPACE
+    # confidence_select keeps its partials on chip: no workspace, NULL is accepted
+    handle.al_confidence_select(st.logits, st.N, st.V, st.V, st.tokens, 511, -1, 0.9, None, 0, 0, st.conf,
+                                st.argmax, st.commit, st.tokens_out, None)
+    with pytest.raises(B.AlError) as e:                          # eos_id outside the vocabulary
+        handle.al_confidence_select(st.logits, st.N, st.V, st.V, st.tokens, 511, st.V, 0.9, None, 0, 0, st.conf,
+                                    st.argmax, st.commit, st.tokens_out, None)
+    assert e.value.status == B.AL_ERR_INVALID_ARG
     with pytest.raises(B.AlError) as e:                          # row_stride < vocab
         handle.al_confidence_select(st.logits, st.N, st.V, st.V - 1, st.tokens, 511, -1, 0.9, None, 0, 0, st.conf,
                                     st.argmax, st.commit, st.tokens_out, st.ws_conf)
