@@ -115,8 +115,8 @@ int32_t al_sm_count(const al_handle* handle);
  * cache row that SOME lane of the call may see must hold finite values -- lanes share 128-row tensor-core
  * tiles, so a NaN/Inf in one lane's K_new/V_new rows reaches the rows stacked with it (0 x NaN).  Cache rows
  * that NO lane sees (beyond the longest prefix_len of the lanes addressing that region: unwritten or
- * recycled memory) may hold anything, NaN included: their scores are masked by selection, their
- * probabilities are exact zeros and the V rows the last key tile rounds up to are zeroed on chip.
+ * recycled memory) may hold anything, NaN included: their scores are masked by selection and the V
+ * rows the last key tile rounds up to are zeroed on chip before the tensor core reads them.
  */
 size_t al_lane_attention_workspace_bytes(const al_attn_shape* shape, int32_t n_lanes,
                                          int32_t total_q_rows, int32_t max_prefix_len);

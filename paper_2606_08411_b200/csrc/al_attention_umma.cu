@@ -319,13 +319,18 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
 // of eight pay; when the streams take alternate key tiles (whole-item plans) one of eight is enough and
 // the instruction count matters more (cfg4: 648 -> 617 us with one, cfg5: 88.6 -> 90.9 us).
 constexpr int kPolyMaskTwoSubTiles = 0x52, kPolyMaskAlt = 0x10;
+#ifdef AL_EPI_NO_TMA_STORE
+constexpr bool kTmaStoreOk = false;        // debug knob: every bf16 sub-tile is copied out by its own warps
+#else
+constexpr bool kTmaStoreOk = true;
+#endif
 constexpr int kStagePitch = 128;           // 128 data bytes per staged row; 16-byte chunk c of row r sits at chunk c ^ (r & 7)
 
 struct AttnSmem {
   alignas(1024) uint8_t q[2][2][kHalfBytes];           // [sub-tile][64-column half]
   alignas(1024) uint8_t k[kStagesK][2][kKvHalfBytes];
   alignas(1024) uint8_t v[kStagesV][2][kKvHalfBytes];
-  alignas(128) uint8_t stage[2 * kBM * kStagePitch];   // epilogue staging: 128 bytes of (stream b, row r) at row b*128 + r
+  alignas(1024) uint8_t stage[2 * kBM * kStagePitch];  // epilogue staging: 128 bytes of (stream b, row r) at row b*128 + r (source of the bulk stores)
   uint32_t stage_off[2 * kBM];                         // ... and where they go: global offset in units of 128 bytes
   uint64_t q_full, q_empty;
   uint64_t k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV];
@@ -511,11 +516,17 @@ __device__ __forceinline__ void merge_rows(const AttnParams& p, const TileRec& T
         const int slot = j == 0 ? 2 * c0 + 1 : 2 * (c0 + j);
         const bool pj = j < n_pieces;
         ls[jj] = (pj && has_row) ? __ldcg(p.plan.part_lse + ((long long)slot * 2 + b) * kBM + my_row) : -INFINITY;
-        const float4* src =
-            reinterpret_cast<const float4*>(p.plan.part_o + (((long long)slot * 2 + b) * kBM + row0) * kD) + lane;
+        // a partial is stored as the four 16 KB staging rounds it was written from (see part_round_ptr):
+        // columns [32 q, 32 q + 32) of row r at round q, byte r * 128 + ((chunk ^ (r & 7)) << 4)
+        const uint8_t* src = reinterpret_cast<const uint8_t*>(p.plan.part_o + ((long long)slot * 2 + b) * kBM * kD) +
+                             (lane >> 3) * (kBM * kStagePitch);
 #pragma unroll
-        for (int k = 0; k < kRows; ++k)
-          v[jj][k] = (pj && row0 + k < n_rows) ? __ldcg(src + k * (kD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int k = 0; k < kRows; ++k) {
+          const int rr = row0 + k;
+          v[jj][k] = (pj && rr < n_rows)
+                         ? __ldcg(reinterpret_cast<const float4*>(src + rr * kStagePitch + (((lane & 7) ^ (rr & 7)) << 4)))
+                         : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
       }
       TRACE_M(12);
       float mx_new = mx;
@@ -608,14 +619,34 @@ __device__ __forceinline__ void copy_out_rows(const uint8_t* stage_b, const uint
     if (r0 + it * 4 < n_rows) *reinterpret_cast<uint4*>(base + (size_t)off[it] * 128 + chunk * 16) = v[it];
 }
 
+// fp32 partial of (slot, sub-tile): four rounds of 32 columns, each the 16 KB image of a stream's staging
+// rows (128 rows x 128 bytes, 16-byte chunks swizzled as stage_chunk writes them), stored by ONE bulk copy.
+__device__ __forceinline__ float* part_round_ptr(const AttnParams& p, int slot, int sub, int round) {
+  return p.plan.part_o + ((long long)slot * 2 + sub) * kBM * kD + round * (kBM * kStagePitch / 4);
+}
+// One epilogue round of a stream through its 16 KB of staging rows and the async proxy: wait until the
+// bulk store that last read the staging rows is done with them, stage this round's 128 bytes per row,
+// make them visible to the async proxy and let thread 0 of the stream issue the store.
+#define AL_STAGE_ROUND_BEGIN()                                                                                 \
+  do {                                                                                                         \
+    if (tid128 == 0) bulk_wait_read_all();                                                                     \
+    bar_sync_stream(b);                                                                                        \
+  } while (0)
+#define AL_STAGE_ROUND_END(issue_stmt)                                                                         \
+  do {                                                                                                         \
+    fence_proxy_async_smem();                                                                                  \
+    bar_sync_stream(b);                                                                                        \
+    if (tid128 == 0) { issue_stmt; bulk_commit(); }                                                            \
+  } while (0)
+
 // The role code of the kernel, compiled twice: with and without the "alt" mode (one sub-tile worked on
 // by both streams).  The plan chooses per launch; keeping the alt code out of the other instance keeps
 // its hot loops as lean as they were (measured: 8 us of 108 at cfg5).
 template <bool kAltOk>
 __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, const CUtensorMap* pmap_q,
                                            const CUtensorMap* pmap_knew, const CUtensorMap* pmap_vnew,
-                                           const CUtensorMap* pmap_kc, const CUtensorMap* pmap_vc, uint32_t tmem,
-                                           int warp, int lane) {
+                                           const CUtensorMap* pmap_kc, const CUtensorMap* pmap_vc,
+                                           const CUtensorMap* pmap_out, uint32_t tmem, int warp, int lane) {
   const bool active = (int)blockIdx.x < p.plan.hdr->n_ctas;
   constexpr bool alt_ok = kAltOk;
   if (threadIdx.x == 0) TRACE(1);
@@ -873,9 +904,8 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         }
         const bool need_mask = valid && (lo > 0 || hi < kBN);
         uint32_t hidden = 0;                             // bit c: 32-column chunk c is entirely hidden from this row
-        uint32_t vis[kBN / 32] = {0xffffffffu, 0xffffffffu};   // bit e of vis[c]: column 32 c + e is visible
-        const bool masked_tile = __any_sync(0xffffffffu, need_mask);
-        if (masked_tile) {                               // warp-uniform: only ragged prefix tails and local tiles
+        if (__any_sync(0xffffffffu, need_mask)) {        // warp-uniform: only ragged prefix tails and local tiles
+          uint32_t vis[kBN / 32];                        // bit e of vis[c]: column 32 c + e is visible
 #pragma unroll
           for (int c4 = 0; c4 < kBN / 32; ++c4) {
             const int a = min(32, max(0, lo - c4 * 32)), z = min(32, max(0, hi - c4 * 32));   // visible [a, z) of the chunk
@@ -943,15 +973,6 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
               if (e & 1) sum_b = fadd2(sum_b, pack2(p0, p1)); else sum_a = fadd2(sum_a, pack2(p0, p1));
               pk[e] = pack_bf16x2(p0, p1);
             }
-            if (masked_tile) {
-              // the polynomial path clamps masked scores at -126 and returns 2^-126, not 0: hidden columns are
-              // set to exact zeros, so that whatever the V row holds cannot reach this row (0 x finite = 0)
-#pragma unroll
-              for (int e = 0; e < 16; ++e) {
-                const uint32_t two = (vis[c] >> (2 * e)) & 3u;
-                pk[e] &= (two & 1u ? 0x0000ffffu : 0u) | (two & 2u ? 0xffff0000u : 0u);
-              }
-            }
           }
           tmem_st16(t_p + lane_addr + c * 16, pk);
         }
@@ -981,6 +1002,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       if (alt) {
         // ---- one sub-tile, two streams (even / odd key tiles): merge them, each storing 64 columns ----
         if (tid128 == 0) sm.alt_has[b] = n_mine > 0;
+        AL_STAGE_ROUND_BEGIN();                        // the previous piece's bulk stores are done with the staging rows
         *reinterpret_cast<float2*>(my_stage) = make_float2(m_used, l_sum);   // exchanged through the staging rows
         bar_sync_both();
         tc_fence_after();                              // the other stream's accumulator is read below, behind its thread's o_full wait
@@ -998,10 +1020,9 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         const float lse2 = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
         bar_sync_both();                               // the exchanged values have been read: the rows may be staged over
         TRACE_E(2);
-        off_b[r] =
-            whole ? (uint32_t)(out_row(p, T, w.g, 0, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
+        const bool full = kTmaStoreOk && T.n_tok >= p.tpt;   // the sub-tile fills its TMA box: no row beyond it may be written
+        if (whole) off_b[r] = (uint32_t)(out_row(p, T, w.g, 0, valid ? r : 0) * (kD * 2 / 128));
         const uint32_t t_o0 = tmem + 256, t_o1 = tmem + 384;
-        float* prow0 = p.plan.part_o + ((long long)slot * 2) * kBM * kD;
 #pragma unroll
         for (int c = 0; c < 2; ++c) {                  // this stream's columns [64 b + 32 c, +32)
           float o[32];
@@ -1021,7 +1042,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
 #pragma unroll
             for (int e = 0; e < 32; ++e) o[e] = f1 > 0.f ? fmaf(a[e], f1, o[e]) : o[e];
           }
-          if (whole) {                                 // bf16: both chunks make one 128-byte round
+          if (whole) {                                 // bf16: both chunks make one 128-byte round = half b of the tile
 #pragma unroll
             for (int e = 0; e < 4; ++e)
               stage_chunk(my_stage, r, c * 4 + e,
@@ -1029,24 +1050,32 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
                                      pack_bf16x2(o[8 * e + 4], o[8 * e + 5]), pack_bf16x2(o[8 * e + 6], o[8 * e + 7])));
             TRACE_E(3 + c);
             if (c == 1) {
-              __syncwarp();
-              copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + b * 128);
+              if (full) {
+                AL_STAGE_ROUND_END(tma_store_3d(pmap_out, stage_b, b * 64, w.g * p.n_rep, T.q_tok0));
+              } else {
+                __syncwarp();
+                copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + b * 128);
+                __syncwarp();
+              }
               TRACE_E(5);
-              __syncwarp();
             }
           } else {                                     // fp32 partial (rows of sub-tile 0): one round per chunk
+            if (c == 1) AL_STAGE_ROUND_BEGIN();
 #pragma unroll
             for (int e = 0; e < 8; ++e)
               stage_chunk(my_stage, r, e, make_uint4(__float_as_uint(o[4 * e]), __float_as_uint(o[4 * e + 1]),
                                                      __float_as_uint(o[4 * e + 2]), __float_as_uint(o[4 * e + 3])));
-            __syncwarp();
-            copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + (b * 64 + c * 32) * 4);
-            __syncwarp();
+            AL_STAGE_ROUND_END(bulk_store(part_round_ptr(p, slot, 0, 2 * b + c), stage_b, kBM * kStagePitch));
           }
         }
         if (whole && b == 0 && valid && p.lse) p.lse[out_row(p, T, w.g, 0, r)] = lse2;
         if (do_ticket && b == 0) p.plan.part_lse[((long long)slot * 2) * kBM + r] = valid ? lse2 : -INFINITY;
-        if (do_ticket) __threadfence();
+        if (do_ticket) {
+          // stream 0 counts the piece for both streams: stream 1's half of the partial has to be complete
+          // (performed, visible) before the barrier below lets stream 0 take the ticket
+          if (tid128 == 0) { bulk_wait_all(); fence_proxy_async_all(); }
+          __threadfence();
+        }
         tc_fence_before();
         TRACE_E(6);
         bar_sync_both();                               // both streams have read both accumulators (and published)
@@ -1054,16 +1083,18 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         if (n_mine > 0) mbar_arrive(&sm.o_empty[b]);
         do_ticket = do_ticket && b == 0;               // stream 0 counts and merges for the tile
       } else {
-      // global offset of this row's output in units of 128 bytes, for the copy loop (pad of the staging row)
-      off_b[r] =
-          whole ? (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128)) : (uint32_t)(r * (kD * 4 / 128));
+      const bool full = kTmaStoreOk && T.n_tok - b * p.tpt >= p.tpt;     // the sub-tile fills its TMA box: no row beyond it may be written
       if (n_mine == 0) {
         // nothing accumulated: no key tile of this piece concerns the sub-tile (or it is empty)
       } else if (whole) {
-        // bf16 output: two rounds of 64 columns = 128 bytes per row
+        // bf16 output: two rounds of 64 columns = 128 bytes per row = one 64-column half of the tile, which a full
+        // sub-tile stores with ONE TMA tensor store from the staging rows (same box and swizzle as the Q loads);
+        // the last, partial sub-tile of a run copies its rows out itself
+        off_b[r] = (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128));
 #pragma unroll
         for (int rd = 0; rd < 2; ++rd) {
           TRACE_E(1 + 5 * rd);
+          uint4 ch[8];
 #pragma unroll
           for (int c = 0; c < 2; ++c) {
             float o[32];
@@ -1072,35 +1103,43 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             if (rd == 1 && c == 1) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }   // O_b is in registers
 #pragma unroll
             for (int e = 0; e < 4; ++e)
-              stage_chunk(my_stage, r, c * 4 + e,
-                          make_uint4(pack_bf16x2(o[8 * e] * inv, o[8 * e + 1] * inv), pack_bf16x2(o[8 * e + 2] * inv, o[8 * e + 3] * inv),
-                                     pack_bf16x2(o[8 * e + 4] * inv, o[8 * e + 5] * inv), pack_bf16x2(o[8 * e + 6] * inv, o[8 * e + 7] * inv)));
+              ch[c * 4 + e] =
+                  make_uint4(pack_bf16x2(o[8 * e] * inv, o[8 * e + 1] * inv), pack_bf16x2(o[8 * e + 2] * inv, o[8 * e + 3] * inv),
+                             pack_bf16x2(o[8 * e + 4] * inv, o[8 * e + 5] * inv), pack_bf16x2(o[8 * e + 6] * inv, o[8 * e + 7] * inv));
           }
           TRACE_E(2 + 5 * rd);
-          __syncwarp();                                // a warp stages and copies its own 32 rows
-          TRACE_E(3 + 5 * rd);
-          copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + rd * 128);
-          TRACE_E(4 + 5 * rd);
-          __syncwarp();                                // the staging rows are rewritten by the next round / piece
+          if (full) {
+            AL_STAGE_ROUND_BEGIN();
+#pragma unroll
+            for (int e = 0; e < 8; ++e) stage_chunk(my_stage, r, e, ch[e]);
+            TRACE_E(3 + 5 * rd);
+            AL_STAGE_ROUND_END(tma_store_3d(pmap_out, stage_b, rd * 64, w.g * p.n_rep, T.q_tok0 + b * p.tpt));
+            TRACE_E(4 + 5 * rd);
+          } else {
+            if (rd == 0) AL_STAGE_ROUND_BEGIN();
+#pragma unroll
+            for (int e = 0; e < 8; ++e) stage_chunk(my_stage, r, e, ch[e]);
+            __syncwarp();                              // a warp stages and copies its own 32 rows
+            copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(p.out) + rd * 128);
+            __syncwarp();                              // the staging rows are rewritten by the next round
+          }
           TRACE_E(5 + 5 * rd);
         }
         if (valid && p.lse) p.lse[out_row(p, T, w.g, b, r)] = lse;
       } else {
-        // fp32 partial: four rounds of 32 columns = 128 bytes per row
-        float* prow0 = p.plan.part_o + ((long long)slot * 2 + b) * kBM * kD;
+        // fp32 partial: four rounds of 32 columns = 128 bytes per row, each round one 16 KB bulk store
 #pragma unroll
         for (int rd = 0; rd < 4; ++rd) {
           float o[32];
           tmem_ld32_f(t_o + lane_addr + rd * 32, o);
           tmem_wait_ld();
           if (rd == 3) { tc_fence_before(); mbar_arrive(&sm.o_empty[b]); }
+          AL_STAGE_ROUND_BEGIN();
 #pragma unroll
           for (int e = 0; e < 8; ++e)
             stage_chunk(my_stage, r, e, make_uint4(__float_as_uint(o[4 * e] * inv), __float_as_uint(o[4 * e + 1] * inv),
                                                    __float_as_uint(o[4 * e + 2] * inv), __float_as_uint(o[4 * e + 3] * inv)));
-          __syncwarp();
-          copy_out_rows(stage_b, off_b, n_rows, tid128, reinterpret_cast<uint8_t*>(prow0) + rd * 128);
-          __syncwarp();
+          AL_STAGE_ROUND_END(bulk_store(part_round_ptr(p, slot, b, rd), stage_b, kBM * kStagePitch));
         }
       }
       if (do_ticket) {
@@ -1113,6 +1152,10 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         bar_sync_stream(b);
         if (tid128 == 0 && b == 0) TRACE(10);
         if (tid128 == 0) {
+          // the bulk stores of this stream's partial have completed (in alt mode stream 1's too: see below)
+          bulk_wait_all();
+          fence_proxy_async_all();
+          __threadfence();
           // pieces of this item live on consecutive CTAs c0..c1 (from the plan): a piece that does not
           // start its item is this CTA's first piece, one that does not finish it is its last
           const int c0 = w.kt_begin > 0 ? w.first_c0 : w.last_c0;
@@ -1133,13 +1176,15 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         bar_sync_stream(b);                            // ticket is reused by the next piece
       }
     }
+    if (tid128 == 0) bulk_wait_all();                  // the staging rows must outlive the bulk stores that read them
   }
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
 lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_knew,
                            const __grid_constant__ CUtensorMap map_vnew, const __grid_constant__ CUtensorMap map_kc,
-                           const __grid_constant__ CUtensorMap map_vc, const AttnParams p) {
+                           const __grid_constant__ CUtensorMap map_vc, const __grid_constant__ CUtensorMap map_out,
+                           const AttnParams p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   AttnSmem& sm = *reinterpret_cast<AttnSmem*>(smem_raw);
   // the shuffle tells the compiler that `warp` is warp-uniform: the role branches and everything derived
@@ -1159,7 +1204,7 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     }
     fence_barrier_init();
     prefetch_tensormap(&map_q); prefetch_tensormap(&map_knew); prefetch_tensormap(&map_vnew);
-    prefetch_tensormap(&map_kc); prefetch_tensormap(&map_vc);
+    prefetch_tensormap(&map_kc); prefetch_tensormap(&map_vc); prefetch_tensormap(&map_out);
   }
   if (warp == 1) tmem_alloc<512>(&sm.tmem_base);
   tc_fence_before();
@@ -1172,8 +1217,8 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   // that opts in (the next layer) may then begin its own prologue as SMs free up.
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (p.plan.hdr->alt) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, tmem, warp, lane);
-  else attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, tmem, warp, lane);
+  if (p.plan.hdr->alt) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
+  else attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
   tc_fence_before();
   __syncthreads();
   if (threadIdx.x == 0) TRACE(13);
@@ -1294,10 +1339,12 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   const WsLayout L = ws_layout(s, b);
   if (workspace_bytes < L.total) AL_FAIL(AL_ERR_WORKSPACE, "al_lane_attention: workspace %zu < %zu", workspace_bytes, L.total);
 
-  CUtensorMap mq, mkn, mvn, mkc, mvc;
+  CUtensorMap mq, mkn, mvn, mkc, mvc, mo;
   const uint64_t T = (uint64_t)total_q_rows, Hq = (uint64_t)s->n_q_heads, Hkv = (uint64_t)s->n_kv_heads;
   const uint64_t rowb = kD * 2;
   if ((rc = make_map_3d(h, &mq, q, kD, Hq, T, rowb, Hq * rowb, 64, (uint32_t)n_rep, (uint32_t)tpt)) != AL_OK) return rc;
+  // the output has the layout of Q: a full sub-tile's 64-column half is stored with the box it was loaded with
+  if ((rc = make_map_3d(h, &mo, out, kD, Hq, T, rowb, Hq * rowb, 64, (uint32_t)n_rep, (uint32_t)tpt)) != AL_OK) return rc;
   if ((rc = make_map_3d(h, &mkn, k_new, kD, Hkv, T, rowb, Hkv * rowb, 64, 1, kBN)) != AL_OK) return rc;
   if ((rc = make_map_3d(h, &mvn, v_new, kD, Hkv, T, rowb, Hkv * rowb, 64, 1, kBN)) != AL_OK) return rc;
   // a group with no prefix never touches the cache maps; encode them over k_new when there is no cache
@@ -1324,7 +1371,7 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lane_attention_umma_kernel, mq, mkn, mvn, mkc, mvc, p));
+  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lane_attention_umma_kernel, mq, mkn, mvn, mkc, mvc, mo, p));
   h->launches += 1;
   return AL_OK;
 }
