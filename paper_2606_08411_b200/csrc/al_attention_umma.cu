@@ -69,6 +69,9 @@ constexpr int kMinPiece = 256 / kBN;       // do not cut the work finer than 256
 #define AL_EPI_COST 4
 #endif
 constexpr int kEpiCost = AL_EPI_COST;      // what the epilogue of an item costs, in 64-key steps, when the step ranges are cut
+constexpr int kPieceCost = 3;              // what a whole piece costs besides its steps (drain, epilogue, restart), in steps: measured 2.8 us
+constexpr int kSplitPieceCost = 6;         // ... and a piece of a split item (fp32 partial, ticket, its share of the merge): measured 5.8 us
+constexpr int kDealMaxTiles = 512;         // item-list plans rank the tiles by counting: n_tiles^2 / 256 smem reads per thread
 constexpr int kSplitCost = 1280 / kBN;     // what splitting an item costs (partial epilogue, ticket, merge by the last CTA), in steps: measured 12-20 us
 
 struct __align__(16) TileRec {             // 64 bytes
@@ -92,7 +95,8 @@ struct __align__(16) CtaRec {              // 96 bytes
 struct PlanHeader {
   int n_tiles, n_items, k_total, n_ctas;
   int alt;           // tiles of one sub-tile are worked on by both streams (chosen with the whole-item mode)
-  int pad[3];
+  int item_lists;    // 1: a CTA's [f_begin, f_end) indexes `order` (whole items dealt to the CTAs); 0: flattened steps
+  int pad[2];
 };
 
 struct Plan {
@@ -101,6 +105,7 @@ struct Plan {
   CtaRec* ctas;
   int* bounds;       // [n_ctas + 1]
   int* counters;     // [n_items][2] tickets per (item, sub-tile), zero between calls (the merging CTA resets its item's)
+  int* order;        // [n_items] item-list plans: item ids (tile * n_kv + kv-head), CTA after CTA
   float* part_o;     // [2 * grid][256][128]  slot 2c: CTA c's first piece, 2c+1: its last piece
   float* part_lse;   // [2 * grid][256]          (rows 128.. belong to sub-tile B)
 };
@@ -168,6 +173,8 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   __shared__ int s_bounds[kMaxCtas + 1];
   __shared__ int s_warp[32];
   __shared__ int s_max_nk;                     // longest item, in steps
+  __shared__ int s_sorted[kDealMaxTiles];      // item-list plans: tile of rank r (longest first)
+  __shared__ int s_makespan;
   const int tid = threadIdx.x;
   // programmatic dependent launch: the attention kernel may start its prologue (barriers, TMEM) now; it
   // waits for this grid's completion before it reads the plan
@@ -246,6 +253,66 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   const bool whole_items = n_tiles > 0 && n_tiles * n_kv_heads <= grid &&
                            s_max_nk <= ceil_div(k_total, n_ctas) + kSplitCost;
   if (whole_items) n_ctas = n_tiles * n_kv_heads;
+  // ---- more items than CTAs: whole items DEALT to the CTAs instead of step ranges, when that is cheaper ----
+  // Cutting the flattened steps into equal ranges leaves (nearly) every CTA with two pieces of split items,
+  // and a split piece is the most expensive thing a CTA does (fp32 partial, ticket, merge: measured 5.8 us
+  // against 1 us per step and 2.8 us per whole piece).  Dealing the items, longest first, forwards and
+  // backwards over the CTAs ("snake") gives every CTA whole items only; the CTAs then differ by at most about
+  // one item, which is compared with the estimated cost of the ranges.
+  const int n_items_all = n_tiles * n_kv_heads;
+  if (!whole_items && n_items_all > grid && n_tiles <= kDealMaxTiles) {
+    if (tid == 0) s_makespan = 0;
+    for (int t = tid; t < n_tiles; t += blockDim.x) {        // rank of tile t among the tiles, longest first
+      const int nk = (s_a[t + 1] - s_a[t]) / n_kv_heads;
+      int rank = 0;
+      for (int u = 0; u < n_tiles; ++u) {
+        const int nku = (s_a[u + 1] - s_a[u]) / n_kv_heads;
+        rank += (nku > nk || (nku == nk && u < t)) ? 1 : 0;
+      }
+      s_sorted[rank] = t;
+    }
+    __syncthreads();
+    // item j of the sorted sequence = (tile s_sorted[j / n_kv], kv-head j % n_kv); round k deals items
+    // [k C, k C + C) to CTAs 0..C-1 (k even) or C-1..0 (k odd)
+    const int C = grid, R = n_items_all / C, rem = n_items_all - R * C;
+    for (int c = tid; c < C; c += blockDim.x) {
+      const int count = R + (((R & 1) ? (C - 1 - c) : c) < rem ? 1 : 0);
+      int load = 0;
+      for (int k = 0; k < count; ++k) {
+        const int j = k * C + ((k & 1) ? C - 1 - c : c);
+        const int t = s_sorted[j / n_kv_heads];
+        load += (s_a[t + 1] - s_a[t]) / n_kv_heads + kPieceCost;
+      }
+      atomicMax(&s_makespan, load);
+    }
+    __syncthreads();
+    const int ranges = ceil_div(k_total + kPieceCost * n_items_all, n_ctas) + 2 * kSplitPieceCost - kPieceCost;
+    if (s_makespan <= ranges) {
+      for (int c = tid; c < C; c += blockDim.x) {
+        const int extra = ((R & 1) ? (C - 1 - c) : c) < rem ? 1 : 0;
+        const int count = R + extra;
+        const int start = c * R + ((R & 1) ? max(0, c - (C - rem)) : min(c, rem));
+        for (int k = 0; k < count; ++k) {
+          const int j = k * C + ((k & 1) ? C - 1 - c : c);
+          plan.order[start + k] = s_sorted[j / n_kv_heads] * n_kv_heads + j % n_kv_heads;
+        }
+        CtaRec Cr;
+        Cr.f_begin = start; Cr.f_end = start + count;
+        Cr.tile0 = s_sorted[c / n_kv_heads];
+        Cr.first_c0 = Cr.first_c1 = Cr.last_c0 = Cr.last_c1 = c;
+        Cr.pad = Cr.tile0 * n_kv_heads + c % n_kv_heads;       // the CTA's first item
+        Cr.first = Cr.tile0 < kPlanTilesInSmem ? s_tiles[Cr.tile0] : plan.tiles[Cr.tile0];   // written by this block above
+        plan.ctas[c] = Cr;
+      }
+      for (int i = tid; i < 2 * n_items_all; i += blockDim.x) plan.counters[i] = 0;
+      if (tid == 0) {
+        plan.hdr->n_tiles = n_tiles; plan.hdr->n_items = n_items_all;
+        plan.hdr->k_total = k_total; plan.hdr->n_ctas = C;
+        plan.hdr->alt = 0; plan.hdr->item_lists = 1;
+      }
+      return;
+    }
+  }
   const bool snap = k_total / n_ctas >= 4;
   for (int c = tid; c <= n_ctas; c += blockDim.x) {
     int f = (int)((long long)c * k_total / n_ctas);
@@ -308,6 +375,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     // with one item per CTA a single-sub-tile item would leave half of the CTA's softmax threads idle;
     // under stream-K the CTAs have long mixed ranges and the merge of the two streams does not pay
     plan.hdr->alt = whole_items ? 1 : 0;
+    plan.hdr->item_lists = 0;
   }
 }
 
@@ -353,34 +421,56 @@ struct AttnParams {
   float scale_log2;
 };
 
-// One CTA's walk over its range of the flattened step sequence: pieces (tile, g, [kt_begin, kt_end)).
+// One CTA's walk over its work: pieces (tile, g, [kt_begin, kt_end)).  Step-range plans: the CTA's range
+// [f, f_end) of the flattened step sequence, items in (tile, kv-head) order, the first and last piece possibly
+// parts of split items.  Item-list plans: whole items order[f .. f_end), in the order they were dealt.
 struct PieceWalk {
   const TileRec* tiles;
+  const int* order;
   int n_kv;
+  bool lists;
   int f, f_end, t, g, kt;
   TileRec T;
   int kt_begin, kt_end;                    // the current piece
   int first_c0, first_c1, last_c0, last_c1;
-  __device__ __forceinline__ PieceWalk(const CtaRec* ctas, const TileRec* tiles_, int n_kv_heads, int cta, bool active)
-      : tiles(tiles_), n_kv(n_kv_heads) {
+  __device__ __forceinline__ PieceWalk(const Plan& plan, int n_kv_heads, int cta, bool active)
+      : tiles(plan.tiles), order(plan.order), n_kv(n_kv_heads) {
     f = f_end = t = g = kt = 0;
+    lists = false;
     first_c0 = first_c1 = last_c0 = last_c1 = cta;
     if (active) {                          // records beyond hdr->n_ctas are not written by the plan
-      const CtaRec* C = ctas + cta;
+      const CtaRec* C = plan.ctas + cta;
+      lists = plan.hdr->item_lists != 0;
       f = C->f_begin; f_end = C->f_end; t = C->tile0;
       first_c0 = C->first_c0; first_c1 = C->first_c1; last_c0 = C->last_c0; last_c1 = C->last_c1;
       if (f < f_end) {
         T = C->first;
-        const int off = f - T.kt_off;
-        g = off / T.n_key_tiles;
-        kt = off - g * T.n_key_tiles;
+        if (lists) {
+          g = C->pad - t * n_kv;           // pad = id of the CTA's first item
+          kt = -1;                         // the first item is already in (t, g, T)
+        } else {
+          const int off = f - T.kt_off;
+          g = off / T.n_key_tiles;
+          kt = off - g * T.n_key_tiles;
+        }
       }
     }
   }
-  // Advances to the next piece; false when the range is exhausted.  After a true return T, g,
+  // Advances to the next piece; false when the work is exhausted.  After a true return T, g,
   // kt_begin, kt_end describe the piece.
   __device__ __forceinline__ bool next() {
     if (f >= f_end) return false;
+    if (lists) {
+      if (kt >= 0) {
+        const int item = order[f];
+        const int tt = item / n_kv;
+        g = item - tt * n_kv;
+        if (tt != t) { t = tt; T = tiles[t]; }
+      }
+      kt_begin = 0; kt_end = kt = T.n_key_tiles;
+      ++f;
+      return true;
+    }
     if (kt == T.n_key_tiles) {             // previous piece ended its item
       kt = 0;
       if (++g == n_kv) { g = 0; T = tiles[++t]; }
@@ -656,7 +746,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
     if (warp == 0 && lane == 0 && active) {
       // ===================== TMA producer of Q and the K tiles =====================
       uint32_t kv_it = 0, piece_it = 0;
-      PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
+      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const TileRec& T = w.T;
         const bool two = T.n_tok > p.tpt;
@@ -685,7 +775,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       // (its own thread: a V stage is freed by P.V, long after the K stage of the same step, and K loads
       // must not queue behind it)
       uint32_t kv_it = 0;
-      PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
+      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const TileRec& T = w.T;
         for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
@@ -725,7 +815,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       uint32_t kv_it = 0, piece_it = 0;
       uint32_t c_qk = 0, c_pv = 0;             // key tiles of this stream whose Q.K^T / P.V has been issued (all pieces)
       uint32_t oe = 0;                         // pieces so far in which the stream had key tiles: o_empty phase
-      PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
+      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
         const bool alt = alt_ok && w.T.n_tok <= p.tpt;     // one sub-tile: both streams work on Q of sub-tile A
@@ -853,7 +943,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
     uint32_t* off_b = sm.stage_off + b * kBM;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
     uint32_t pieces_done = 0;                          // pieces in which it had key tiles: o_full phase
-    PieceWalk w(p.plan.ctas, p.plan.tiles, p.n_kv_heads, blockIdx.x, active);
+    PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
     while (w.next()) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
@@ -1239,7 +1329,7 @@ Bounds bounds_for(const al_attn_shape* s, int n_lanes, int total_q_rows, int n_s
 }
 
 struct WsLayout {
-  size_t hdr, tiles, ctas, bounds, counters, part_lse, part_o, total;
+  size_t hdr, tiles, ctas, bounds, counters, order, part_lse, part_o, total;
 };
 WsLayout ws_layout(const al_attn_shape* s, const Bounds& b) {
   WsLayout L;
@@ -1250,6 +1340,7 @@ WsLayout ws_layout(const al_attn_shape* s, const Bounds& b) {
   L.ctas = take(sizeof(CtaRec) * (size_t)b.grid);
   L.bounds = take(sizeof(int) * (size_t)(b.grid + 1));
   L.counters = take(sizeof(int) * (size_t)b.max_tiles * s->n_kv_heads * 2);
+  L.order = take(sizeof(int) * (size_t)b.max_tiles * s->n_kv_heads);
   L.part_lse = take(sizeof(float) * (size_t)2 * b.grid * 2 * kBM);
   L.part_o = take(sizeof(float) * (size_t)2 * b.grid * 2 * kBM * kD);
   L.total = off;
@@ -1266,6 +1357,7 @@ Plan plan_in(void* workspace, const WsLayout& L) {
   plan.ctas = reinterpret_cast<CtaRec*>(ws + L.ctas);
   plan.bounds = reinterpret_cast<int*>(ws + L.bounds);
   plan.counters = reinterpret_cast<int*>(ws + L.counters);
+  plan.order = reinterpret_cast<int*>(ws + L.order);
   plan.part_lse = reinterpret_cast<float*>(ws + L.part_lse);
   plan.part_o = reinterpret_cast<float*>(ws + L.part_o);
   return plan;
