@@ -84,14 +84,18 @@ struct __align__(16) TileRec {             // 64 bytes
   int kt_off;                 // index of step (g = 0, kt = 0) of this tile in the flattened sequence
   int sub_lk0[2], sub_lk1[2]; // local key rows the lanes of sub-tile A / B can see (lk0 > lk1: none)
 };
-struct __align__(16) CtaRec {              // 96 bytes
-  int f_begin, f_end;         // this CTA's range of the flattened step sequence
+struct __align__(16) CtaRec {              // 112 bytes; the ONE record a CTA reads before it can issue its first loads
+  int f_begin, f_end;         // this CTA's range of the flattened step sequence (item-list plans: of `order`)
   int tile0;                  // tile that contains f_begin
   int first_c0, first_c1;     // CTAs that hold pieces of the item this CTA's FIRST step belongs to
   int last_c0, last_c1;       // same for the item of its LAST step
-  int pad;
+  int pad;                    // item-list plans: id of the CTA's first item
   TileRec first;              // copy of tiles[tile0]: one load instead of two dependent ones at kernel start
+  int flags;                  // kCtaActive | kCtaAlt | kCtaLists (copies of the plan header's switches)
+  int reserved[3];
 };
+constexpr int kCtaActive = 1, kCtaAlt = 2, kCtaLists = 4;
+static_assert(sizeof(CtaRec) == 112, "CtaRec is loaded as seven 16-byte vectors");
 struct PlanHeader {
   int n_tiles, n_items, k_total, n_ctas;
   int alt;           // tiles of one sub-tile are worked on by both streams (chosen with the whole-item mode)
@@ -179,6 +183,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   // programmatic dependent launch: the attention kernel may start its prologue (barriers, TMEM) now; it
   // waits for this grid's completion before it reads the plan
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  TRACE_P(0);
   if (tid == 0) s_max_nk = 0;
 
   // runs
@@ -193,7 +198,9 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     s_a[i] = start;
   }
   __syncthreads();
+  TRACE_P(1);
   const int n_runs = block_exclusive_scan(s_a, n_lanes, s_warp);
+  TRACE_P(2);
   for (int i = tid; i < n_lanes; i += blockDim.x) {
     const bool start = (i + 1 < n_lanes ? s_a[i + 1] : n_runs) != s_a[i];
     if (start) s_run_lane0[s_a[i]] = i;
@@ -206,7 +213,9 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     s_run_tile_base[r] = ceil_div(max(0, s_qe[l1 - 1] - s_qs[l0]), 2 * tpt);
   }
   __syncthreads();
+  TRACE_P(3);
   int n_tiles = block_exclusive_scan(s_run_tile_base, n_runs, s_warp);
+  TRACE_P(4);
   n_tiles = min(n_tiles, min(bounds.max_tiles, kMaxPlanTiles));   // cannot bind when the lanes are disjoint
   // tiles
   for (int t = tid; t < n_tiles; t += blockDim.x) {
@@ -241,7 +250,9 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     atomicMax(&s_max_nk, T.n_key_tiles);
   }
   __syncthreads();
+  TRACE_P(5);
   const int k_total = block_exclusive_scan(s_a, n_tiles, s_warp);
+  TRACE_P(6);
   if (tid == 0) s_a[n_tiles] = k_total;
   for (int t = tid; t < n_tiles; t += blockDim.x) plan.tiles[t].kt_off = s_a[t];
   // per-CTA ranges of the flattened step sequence
@@ -250,8 +261,13 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   // When every item can have a CTA of its own, cutting items only pays if the longest item costs more
   // than the balanced share plus what a split costs (fp32 partials, tickets, merge).
   __syncthreads();
+  // steps per item of tile t, for t < kMaxPlanLanes, in the (now free) tiles-per-run scratch: the loops below
+  // would otherwise divide by n_kv_heads per element
+  int* s_nk = s_run_tile_base;
+  for (int t = tid; t < min(n_tiles, kMaxPlanLanes); t += blockDim.x) s_nk[t] = (s_a[t + 1] - s_a[t]) / n_kv_heads;
   const bool whole_items = n_tiles > 0 && n_tiles * n_kv_heads <= grid &&
                            s_max_nk <= ceil_div(k_total, n_ctas) + kSplitCost;
+  __syncthreads();
   if (whole_items) n_ctas = n_tiles * n_kv_heads;
   // ---- more items than CTAs: whole items DEALT to the CTAs instead of step ranges, when that is cheaper ----
   // Cutting the flattened steps into equal ranges leaves (nearly) every CTA with two pieces of split items,
@@ -259,19 +275,21 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   // against 1 us per step and 2.8 us per whole piece).  Dealing the items, longest first, forwards and
   // backwards over the CTAs ("snake") gives every CTA whole items only; the CTAs then differ by at most about
   // one item, which is compared with the estimated cost of the ranges.
+  TRACE_P(7);
   const int n_items_all = n_tiles * n_kv_heads;
   if (!whole_items && n_items_all > grid && n_tiles <= kDealMaxTiles) {
     if (tid == 0) s_makespan = 0;
     for (int t = tid; t < n_tiles; t += blockDim.x) {        // rank of tile t among the tiles, longest first
-      const int nk = (s_a[t + 1] - s_a[t]) / n_kv_heads;
+      const int nk = s_nk[t];
       int rank = 0;
       for (int u = 0; u < n_tiles; ++u) {
-        const int nku = (s_a[u + 1] - s_a[u]) / n_kv_heads;
+        const int nku = s_nk[u];
         rank += (nku > nk || (nku == nk && u < t)) ? 1 : 0;
       }
       s_sorted[rank] = t;
     }
     __syncthreads();
+    TRACE_P(8);
     // item j of the sorted sequence = (tile s_sorted[j / n_kv], kv-head j % n_kv); round k deals items
     // [k C, k C + C) to CTAs 0..C-1 (k even) or C-1..0 (k odd)
     const int C = grid, R = n_items_all / C, rem = n_items_all - R * C;
@@ -280,12 +298,12 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
       int load = 0;
       for (int k = 0; k < count; ++k) {
         const int j = k * C + ((k & 1) ? C - 1 - c : c);
-        const int t = s_sorted[j / n_kv_heads];
-        load += (s_a[t + 1] - s_a[t]) / n_kv_heads + kPieceCost;
+        load += s_nk[s_sorted[j / n_kv_heads]] + kPieceCost;
       }
       atomicMax(&s_makespan, load);
     }
     __syncthreads();
+    TRACE_P(9);
     const int ranges = ceil_div(k_total + kPieceCost * n_items_all, n_ctas) + 2 * kSplitPieceCost - kPieceCost;
     if (s_makespan <= ranges) {
       for (int c = tid; c < C; c += blockDim.x) {
@@ -301,6 +319,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
         Cr.tile0 = s_sorted[c / n_kv_heads];
         Cr.first_c0 = Cr.first_c1 = Cr.last_c0 = Cr.last_c1 = c;
         Cr.pad = Cr.tile0 * n_kv_heads + c % n_kv_heads;       // the CTA's first item
+        Cr.flags = kCtaActive | kCtaLists; Cr.reserved[0] = Cr.reserved[1] = Cr.reserved[2] = 0;
         Cr.first = Cr.tile0 < kPlanTilesInSmem ? s_tiles[Cr.tile0] : plan.tiles[Cr.tile0];   // written by this block above
         plan.ctas[c] = Cr;
       }
@@ -310,8 +329,39 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
         plan.hdr->k_total = k_total; plan.hdr->n_ctas = C;
         plan.hdr->alt = 0; plan.hdr->item_lists = 1;
       }
+      TRACE_P(10);
       return;
     }
+  }
+  TRACE_P(11);
+  if (whole_items) {                                     // CTA c = item c = (tile c / n_kv, head c % n_kv): no searches
+    for (int c = tid; c <= n_ctas; c += blockDim.x) {
+      const int t = c / n_kv_heads, g = c - t * n_kv_heads;
+      const int f0 = c == n_ctas ? k_total : s_a[t] + g * s_nk[t];
+      plan.bounds[c] = f0;
+      if (c < n_ctas) {
+        CtaRec C;
+        C.f_begin = f0; C.f_end = f0 + s_nk[t];
+        C.tile0 = t;
+        C.first_c0 = C.first_c1 = C.last_c0 = C.last_c1 = c;
+        C.pad = c;
+        C.flags = kCtaActive | kCtaAlt; C.reserved[0] = C.reserved[1] = C.reserved[2] = 0;
+        C.first = t < kPlanTilesInSmem ? s_tiles[t] : plan.tiles[t];   // written by this block above
+        C.first.kt_off = s_a[t];
+        plan.ctas[c] = C;
+      }
+    }
+    for (int c = n_ctas + tid; c < grid; c += blockDim.x) plan.ctas[c].flags = kCtaAlt;   // idle CTAs
+    for (int i = tid; i < 2 * n_items_all; i += blockDim.x) plan.counters[i] = 0;
+    if (tid == 0) {
+      plan.hdr->n_tiles = n_tiles; plan.hdr->n_items = n_items_all;
+      plan.hdr->k_total = k_total; plan.hdr->n_ctas = k_total > 0 ? n_ctas : 0;
+      // with one item per CTA a single-sub-tile item would leave half of the CTA's softmax threads idle: both
+      // streams work on it, taking alternate key tiles
+      plan.hdr->alt = 1; plan.hdr->item_lists = 0;
+    }
+    TRACE_P(12);
+    return;
   }
   const bool snap = k_total / n_ctas >= 4;
   for (int c = tid; c <= n_ctas; c += blockDim.x) {
@@ -350,6 +400,8 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
       C.tile0 = n_tiles ? last_le(s_a, n_tiles, C.f_begin) : 0;
       C.first_c0 = C.first_c1 = C.last_c0 = C.last_c1 = c;
       C.pad = 0;
+      C.flags = (n_tiles && s_bounds[c] < s_bounds[c + 1]) ? kCtaActive : 0;
+      C.reserved[0] = C.reserved[1] = C.reserved[2] = 0;
       if (n_tiles) {
         C.first = C.tile0 < kPlanTilesInSmem ? s_tiles[C.tile0] : plan.tiles[C.tile0];   // written by this block above
         C.first.kt_off = s_a[C.tile0];
@@ -368,6 +420,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
       plan.ctas[c] = C;
     }
   }
+  for (int c = n_ctas + tid; c < grid; c += blockDim.x) plan.ctas[c].flags = 0;            // idle CTAs
   for (int i = tid; i < 2 * n_tiles * n_kv_heads; i += blockDim.x) plan.counters[i] = 0;   // one per (item, sub-tile)
   if (tid == 0) {
     plan.hdr->n_tiles = n_tiles; plan.hdr->n_items = n_tiles * n_kv_heads;
@@ -377,6 +430,7 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     plan.hdr->alt = whole_items ? 1 : 0;
     plan.hdr->item_lists = 0;
   }
+  TRACE_P(12);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -405,6 +459,7 @@ struct AttnSmem {
   uint64_t s_full[2], s_free[2];           // [stream]: S written by Q.K^T / S in the softmax threads' registers
   uint64_t p_full[2][2], pv_done[2][2];    // [stream][P buffer]: P written / the P.V that read it has completed
   uint64_t o_full[2], o_empty[2];          // per piece: accumulator complete / read out
+  CtaRec cta;                              // this CTA's plan record
   uint32_t tmem_base;
   int ticket[2][3];
   int alt_has[2];                          // alt mode: did stream b have key tiles in this piece
@@ -433,14 +488,14 @@ struct PieceWalk {
   TileRec T;
   int kt_begin, kt_end;                    // the current piece
   int first_c0, first_c1, last_c0, last_c1;
-  __device__ __forceinline__ PieceWalk(const Plan& plan, int n_kv_heads, int cta, bool active)
+  // C: the CTA's own record (a copy in shared memory, loaded once in the kernel prologue)
+  __device__ __forceinline__ PieceWalk(const Plan& plan, const CtaRec* C, int n_kv_heads, int cta)
       : tiles(plan.tiles), order(plan.order), n_kv(n_kv_heads) {
     f = f_end = t = g = kt = 0;
     lists = false;
     first_c0 = first_c1 = last_c0 = last_c1 = cta;
-    if (active) {                          // records beyond hdr->n_ctas are not written by the plan
-      const CtaRec* C = plan.ctas + cta;
-      lists = plan.hdr->item_lists != 0;
+    if (C->flags & kCtaActive) {
+      lists = (C->flags & kCtaLists) != 0;
       f = C->f_begin; f_end = C->f_end; t = C->tile0;
       first_c0 = C->first_c0; first_c1 = C->first_c1; last_c0 = C->last_c0; last_c1 = C->last_c1;
       if (f < f_end) {
@@ -737,7 +792,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
                                            const CUtensorMap* pmap_knew, const CUtensorMap* pmap_vnew,
                                            const CUtensorMap* pmap_kc, const CUtensorMap* pmap_vc,
                                            const CUtensorMap* pmap_out, uint32_t tmem, int warp, int lane) {
-  const bool active = (int)blockIdx.x < p.plan.hdr->n_ctas;
+  const bool active = (sm.cta.flags & kCtaActive) != 0;
   constexpr bool alt_ok = kAltOk;
   if (threadIdx.x == 0) TRACE(1);
 
@@ -746,18 +801,11 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
     if (warp == 0 && lane == 0 && active) {
       // ===================== TMA producer of Q and the K tiles =====================
       uint32_t kv_it = 0, piece_it = 0;
-      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+      PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
       while (w.next()) {
         const TileRec& T = w.T;
         const bool two = T.n_tok > p.tpt;
-        mbar_wait_relaxed(&sm.q_empty, (piece_it & 1) ^ 1);
-        mbar_arrive_expect_tx(&sm.q_full, two ? 2 * p.q_box_bytes : p.q_box_bytes);   // a box is tpt*n_rep (<= 128) rows per half
-        for (int b = 0; b < (two ? 2 : 1); ++b) {
-          tma_load_3d(sm.q[b][0], pmap_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
-          tma_load_3d(sm.q[b][1], pmap_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
-        }
-        TRACE(2);
-        for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
+        auto issue_k = [&](int kt) {
           const int sk = kv_it % kStagesK;
           const bool pref = kt < T.n_pref_tiles;
           const int row = pref ? T.kv_base_row + kt * kBN : T.lk0 + (kt - T.n_pref_tiles) * kBN;
@@ -767,6 +815,23 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           mbar_arrive_expect_tx(&sm.k_full[sk], kTileBytes);
           tma_load_3d(sm.k[sk][0], mk, &sm.k_full[sk], 0, c1, c2);
           tma_load_3d(sm.k[sk][1], mk, &sm.k_full[sk], 64, c1, c2);
+          ++kv_it;
+        };
+        int kt = w.kt_begin;
+        // Cold start: all CTAs fill their rings at the same moment (148 x 192 KB: several microseconds of HBM
+        // bandwidth), so what the first Q.K^T needs goes out first -- key tile 0, then Q, then key tile 1 -- and the
+        // rest of the ring (and the V ring, below) only once key tile 0 has landed.
+        if (piece_it == 0) issue_k(kt++);
+        mbar_wait_relaxed(&sm.q_empty, (piece_it & 1) ^ 1);
+        mbar_arrive_expect_tx(&sm.q_full, two ? 2 * p.q_box_bytes : p.q_box_bytes);   // a box is tpt*n_rep (<= 128) rows per half
+        for (int b = 0; b < (two ? 2 : 1); ++b) {
+          tma_load_3d(sm.q[b][0], pmap_q, &sm.q_full, 0, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
+          tma_load_3d(sm.q[b][1], pmap_q, &sm.q_full, 64, w.g * p.n_rep, T.q_tok0 + b * p.tpt);
+        }
+        TRACE(2);
+        for (; kt < w.kt_end; ++kt) {
+          if (piece_it == 0 && kv_it == 2) mbar_wait_relaxed(&sm.k_full[0], 0);
+          issue_k(kt);
         }
         ++piece_it;
       }
@@ -775,7 +840,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       // (its own thread: a V stage is freed by P.V, long after the K stage of the same step, and K loads
       // must not queue behind it)
       uint32_t kv_it = 0;
-      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+      PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
       while (w.next()) {
         const TileRec& T = w.T;
         for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
@@ -784,6 +849,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
           const int row = pref ? T.kv_base_row + kt * kBN : T.lk0 + (kt - T.n_pref_tiles) * kBN;
           const CUtensorMap* mv = pref ? pmap_vc : pmap_vnew;
           const int c1 = pref ? row : w.g, c2 = pref ? w.g : row;
+          if (kv_it == 0) mbar_wait_relaxed(&sm.k_full[0], 0);   // cold start: behind key tile 0 (see the K producer)
           mbar_wait_relaxed(&sm.v_empty[sv], ((kv_it / kStagesV) & 1) ^ 1);
           mbar_arrive_expect_tx(&sm.v_full[sv], kTileBytes);
           tma_load_3d(sm.v[sv][0], mv, &sm.v_full[sv], 0, c1, c2);
@@ -815,7 +881,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       uint32_t kv_it = 0, piece_it = 0;
       uint32_t c_qk = 0, c_pv = 0;             // key tiles of this stream whose Q.K^T / P.V has been issued (all pieces)
       uint32_t oe = 0;                         // pieces so far in which the stream had key tiles: o_empty phase
-      PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+      PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
         const bool alt = alt_ok && w.T.n_tok <= p.tpt;     // one sub-tile: both streams work on Q of sub-tile A
@@ -943,7 +1009,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
     uint32_t* off_b = sm.stage_off + b * kBM;
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
     uint32_t pieces_done = 0;                          // pieces in which it had key tiles: o_full phase
-    PieceWalk w(p.plan, p.n_kv_heads, blockIdx.x, active);
+    PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
     while (w.next()) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
@@ -1297,17 +1363,21 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
     prefetch_tensormap(&map_kc); prefetch_tensormap(&map_vc); prefetch_tensormap(&map_out);
   }
   if (warp == 1) tmem_alloc<512>(&sm.tmem_base);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = sm.tmem_base;
-  // TMEM columns: S of stream b at 64 b; P of stream b, buffer u at 128 + 64 b + 32 u; O of stream b at 256 + 128 b
   // programmatic dependent launch: everything above overlapped the previous kernel in the stream (the
   // plan, or the previous layer); its memory is visible after the wait.  The next launch in the stream
   // that opts in (the next layer) may then begin its own prologue as SMs free up.
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (p.plan.hdr->alt) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
+  // the CTA's plan record: the one global read on the way to the first TMA load, in flight under the TMEM
+  // allocation and the barrier initialisation of the other warps
+  if (warp == 2 && lane < (int)(sizeof(CtaRec) / 16))
+    reinterpret_cast<uint4*>(&sm.cta)[lane] = __ldcg(reinterpret_cast<const uint4*>(p.plan.ctas + blockIdx.x) + lane);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = sm.tmem_base;
+  // TMEM columns: S of stream b at 64 b; P of stream b, buffer u at 128 + 64 b + 32 u; O of stream b at 256 + 128 b
+  if (sm.cta.flags & kCtaAlt) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
   else attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
   tc_fence_before();
   __syncthreads();

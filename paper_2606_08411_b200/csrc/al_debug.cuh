@@ -29,6 +29,12 @@ __device__ unsigned long long g_trace_epi[16];
       g_trace[blockIdx.x * 16 + 0] = clock64();                                                                \
     }                                                                                                          \
   } while (0)
+// plan kernel: clock64 stamps after each phase (thread 0)
+__device__ unsigned long long g_trace_plan[32];
+#define TRACE_P(i) do { if (threadIdx.x == 0) g_trace_plan[i] = clock64(); } while (0)
+extern "C" int al_debug_plan_trace(unsigned long long* host_out) {        // [32]
+  return (int)cudaMemcpyFromSymbol(host_out, g_trace_plan, sizeof(g_trace_plan));
+}
 extern "C" int al_debug_attn_trace(unsigned long long* host_out) {        // [256 * 16]
   return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace));
 }
@@ -48,4 +54,5 @@ extern "C" int al_debug_attn_trace_tile(unsigned long long* host_out) {   // [16
 #define TRACE_E(k) do { } while (0)
 #define TRACE_M(k) do { } while (0)
 #define TRACE_RESET() do { } while (0)
+#define TRACE_P(i) do { } while (0)
 #endif
