@@ -15,8 +15,8 @@ What is timed (DESIGN.md "Measurement"):
             on DISTINCT copies of every streamed buffer (rotation set > 2x L2) so nothing is served
             from L2.  Device time from CUDA events on the launching stream, max over ranks.
   roofline  per-part device time: every part (attention = plan + all layers, refresh, confidence) has
-            its own graph per copy, replayed over the same rotation right after the timed region and
-            timed with CUDA events on the stream.
+            a graph of its own that runs it on every resident copy in turn, replayed right after the
+            timed region and timed with CUDA events on the stream (time / launches in the graph).
   e2e       the same step through the C-ABI host entry al_lane_step_host: every step copies its
             inputs from pinned host memory, runs the kernels and copies the results back.
   cpu_baseline / --impl reference   the CPU oracle (oracle/, fp64, as it stands) on the host cores.
@@ -243,17 +243,19 @@ def measure_resident(h, wl, dev, stream, dist, sampler, steps, warmup, kernel_ev
                 st.run(stream)
             launches_per_step = h.al_launch_count - before
             graphs.append(g)
-            # one graph per part (attention = plan + every layer, refresh, confidence) for the per-part
-            # times: event nodes inside the step graph would cost a few us per step and break the
-            # programmatic-dependent-launch edges between the kernels
-            if kernel_events:
-                pg = {}
-                for name, fn in (("attention", st.attention), ("refresh", st.refresh), ("confidence", st.confidence)):
-                    gp = torch.cuda.CUDAGraph()
-                    with torch.cuda.graph(gp, stream=stream):
-                        fn(stream)
-                    pg[name] = gp
-                part_graphs.append(pg)
+        # Per-part times: ONE graph per part that runs the part on every resident copy in turn (at least 4
+        # launches), so that consecutive launches never share data through L2 and the time between two
+        # launches inside the graph is what a step sees (event nodes inside the step graph would cost a few us
+        # and break the programmatic-dependent-launch edges; one graph replay per launch would add the graph
+        # launch latency, ~2 us, to every sample)
+        if kernel_events:
+            inner = max(n_copies, 4)
+            for name in ("attention", "refresh", "confidence"):
+                gp = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gp, stream=stream):
+                    for i in range(inner):
+                        getattr(copies[i % n_copies], name)(stream)
+                part_graphs.append((name, gp, inner))
     stream.synchronize()
 
     def barrier():
@@ -282,21 +284,20 @@ def measure_resident(h, wl, dev, stream, dist, sampler, steps, warmup, kernel_ev
     # same rotation of copies (so its inputs come from HBM, not L2) and timed with CUDA events on the stream
     part_ms = None
     if kernel_events:
-        reps = max(4 * n_copies, 40)
         part_ms = {}
         sampler.active.set()
-        for name in ("attention", "refresh", "confidence"):
+        for name, gp, inner in part_graphs:
+            reps = max(40 // inner, 8)
             with torch.cuda.stream(stream):
-                for i in range(n_copies):
-                    part_graphs[i % n_copies][name].replay()
+                gp.replay()
                 e0.record(stream)
                 for i in range(reps):
-                    part_graphs[i % n_copies][name].replay()
+                    gp.replay()
                 e1.record(stream)
             barrier()
-            part_ms[name] = e0.elapsed_time(e1) / reps
+            part_ms[name] = e0.elapsed_time(e1) / (reps * inner)
+            part_ms["n_samples"] = reps * inner
         sampler.active.clear()
-        part_ms["n_samples"] = reps
     return dict(step_ms=step_ms, part_ms=part_ms, launches_per_step=launches_per_step, copies=copies,
                 n_copies=n_copies, per_copy=per_copy, barrier=barrier, graphs=graphs, part_graphs=part_graphs)
 
@@ -389,7 +390,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         dom = max(parts, key=lambda k: parts[k]["ms"])
         roofline = {k: parts[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")}
         roofline.update(kernel=dom, peak_source=peaks["source"], avg_launch_ms=parts[dom]["ms"] / parts[dom]["launches"],
-                        timed_with="CUDA events on the stream around replays of the part's own graph over the same rotating copies, right after the timed region")
+                        timed_with="CUDA events on the stream around replays of a graph that runs the part on every resident copy in turn (consecutive launches share nothing through L2), right after the timed region")
     else:
         roofline = None
 
