@@ -138,3 +138,26 @@ def confidence_select(logits, tokens_in, mask_id: int, eos_id: int, threshold: f
                                      ctypes.c_int(1 if force_top1 else 0), _p(conf), _p(argmax),
                                      _p(p2), _p(commit), _p(tokens_out))
     return dict(conf=conf, argmax=argmax, p2=p2, commit=commit, tokens_out=tokens_out)
+
+
+def lane_status(lanes, tokens_in, conf, argmax, mask_id: int, eos_id: int, tau_future: float,
+                delimiters, no_fork_prev, commit, tokens_out):
+    """O-D.  Per-lane integers after the transfer + the lookahead draft rule (Eq.8).  `commit` and
+    `tokens_out` are the select's outputs; copies are returned with the lookahead rows decided by Eq.8.
+    Returns dict(status int32 [n,8] = n_filled, valid_prefix, split_point, n_committed, n_drafts, n_masked, 0, 0;
+    commit u8[N]; tokens_out i32[N])."""
+    lanes = _i32(lanes).reshape(-1, 6)
+    tokens_in = _i32(tokens_in)
+    N = tokens_in.shape[0]
+    conf = np.ascontiguousarray(conf, dtype=np.float64)
+    argmax = _i32(argmax)
+    delimiters, no_fork_prev = _i32(delimiters).reshape(-1), _i32(no_fork_prev).reshape(-1)
+    commit_io = np.ascontiguousarray(commit, dtype=np.uint8).copy()
+    tokens_io = _i32(tokens_out).copy()
+    status = np.zeros((lanes.shape[0], 8), np.int32)
+    _load().oracle_lane_status(_p(lanes), ctypes.c_int(lanes.shape[0]), ctypes.c_int(N), _p(tokens_in), _p(conf),
+                               _p(argmax), ctypes.c_int(mask_id), ctypes.c_int(eos_id), ctypes.c_double(tau_future),
+                               _p(delimiters) if delimiters.size else None, ctypes.c_int(delimiters.size),
+                               _p(no_fork_prev) if no_fork_prev.size else None, ctypes.c_int(no_fork_prev.size),
+                               _p(commit_io), _p(tokens_io), _p(status))
+    return dict(status=status, commit=commit_io, tokens_out=tokens_io)

@@ -6,9 +6,11 @@
  * CUDA path under paper_2606_08411_b200/csrc/ and is written as the plain definitions, in the
  * paper's order, with fp64 arithmetic on the (dtype-rounded) float32 inputs.
  *
- * All three functions are exact definitions (lane batching "does not eliminate
- * token-level computation, but replaces serial lane forwards with grouped GPU execution"), so the
- * oracle is the naive computation.  Pins: tests/test_oracle_pins.py (brute force, closed forms,
+ * The three functions of the lane step (O-A attention, O-B refresh, O-C confidence/select) are exact
+ * definitions (lane batching "does not eliminate token-level computation, but replaces
+ * serial lane forwards with grouped GPU execution"), so the oracle is the naive computation.  O-D (lane
+ * status: Eq.4, 5, 8, 9) is integer bookkeeping written out from the equations.  Pins:
+ * tests/test_oracle_pins*.py (brute force, closed forms, hand-worked examples under tests/golden/,
  * library special cases, invariants).  Nothing here is "parity unpinned".
  *
  * Lane descriptor (int32 x 6 per lane), after PAPER.md L56 Eq.1 / L70 / L168:
@@ -17,7 +19,8 @@
  *   [2] prefix_len   visible cache rows [kv_base_row, kv_base_row+prefix_len) = P + s_l (L70)
  *   [3] q_start      first row of the lane in the packed Q / K_new / V_new / logits
  *   [4] q_len        lane length b_l + w_l (L72 Eq.2)
- *   [5] flags        bit0 = refine lane (EOS suppressed, L80)
+ *   [5] flags        bit0 = refine lane (EOS suppressed, L80); bits 8..23 = lookahead window w_l (Eq.2):
+ *                    the LAST w_l of the lane's q_len rows (only O-D distinguishes them)
  */
 #include <math.h>
 #include <stdint.h>
@@ -195,4 +198,71 @@ void oracle_confidence_select(const float* logits, int n_rows, int vocab, int64_
   }
   for (int i = 0; i < n_rows; ++i) tokens_out[i] = commit[i] ? argmax[i] : tokens_in[i];
   free(suppress);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-D  lane status after the transfer: the per-lane integers the host
+ * scheduler (Alg.1) needs from one iteration, and the lookahead draft rule.
+ *
+ * A lane's rows are u_l = [z_l ; lookahead window] (Eq.2): the first b = q_len - w rows are
+ * the lane state z_l, the last w rows the lookahead window; w = (flags >> 8) & 0xffff.
+ *
+ *  Eq.8 (L108)  lookahead rows:  x_i <- x^_i  if  x_i = [MASK], q_i >= tau_future, x^_i not in E
+ *               (E = {EOS}; the rows are decided here whatever the transfer rule wrote for them)
+ *  Eq.5 (L91)   n_filled    = |{ i < b : z_i != [MASK] }|           (fill ratio = n_filled / b)
+ *  Eq.9 (L113)  valid_prefix v_l = min( { i : z_i = [MASK] or z_i in E } U { b } ),  i 0-based
+ *               (the paper's i - 1 with 1-based i)
+ *  Eq.4 (L86)   split_point p_l = 1 + max{ i : z_i in D_task and ValidBoundary(z_{1:i}) }, i.e.
+ *               with 0-based i the number of tokens up to and including the last valid delimiter;
+ *               0 when there is none.  ValidBoundary (reading C17): a delimiter whose PREVIOUS token is
+ *               in the no-fork set does not count (L195 "numeric-period patterns excluded": a period
+ *               after a digit token); the first token of a lane has no previous token.
+ *  n_committed = rows of z_l committed in this iteration, n_drafts = lookahead rows drafted,
+ *  n_masked = b - n_filled.
+ * All of z is read AFTER the transfer (tokens_io holds tokens_out of the select on entry).
+ * status: int32 [n_lanes][8] = {n_filled, valid_prefix, split_point, n_committed, n_drafts, n_masked, 0, 0}.
+ * -----------------------------------------------------------------------------------------*/
+void oracle_lane_status(const int32_t* lanes, int n_lanes, int n_rows, const int32_t* tokens_in,
+                        const double* conf, const int32_t* argmax, int mask_id, int eos_id,
+                        double tau_future, const int32_t* delimiters, int n_delimiters,
+                        const int32_t* no_fork_prev, int n_no_fork_prev, uint8_t* commit_io,
+                        int32_t* tokens_io, int32_t* status) {
+  for (int l = 0; l < n_lanes; ++l) {
+    const int32_t* lane = lanes + 6 * l;
+    const int q_start = lane[3], q_len = lane[4];
+    int w = (lane[5] >> 8) & 0xffff;
+    if (w > q_len) w = q_len;
+    const int b = q_len - w;
+    int32_t* st = status + 8 * l;
+    for (int k = 0; k < 8; ++k) st[k] = 0;
+    /* Eq.8: the lookahead window */
+    for (int i = b; i < q_len; ++i) {
+      const int row = q_start + i;
+      if (row < 0 || row >= n_rows) continue;
+      const int c = tokens_in[row] == mask_id && conf[row] >= tau_future && argmax[row] != eos_id;
+      commit_io[row] = (uint8_t)c;
+      tokens_io[row] = c ? argmax[row] : tokens_in[row];
+      st[4] += c;
+    }
+    /* the lane state z_l after the transfer */
+    int v = b, p = 0;
+    for (int i = 0; i < b; ++i) {
+      const int row = q_start + i;
+      const int z = tokens_io[row];
+      if (z != mask_id) st[0] += 1;
+      if (commit_io[row]) st[3] += 1;
+      if ((z == mask_id || z == eos_id) && i < v) v = i;
+      int is_delim = 0;
+      for (int d = 0; d < n_delimiters; ++d) is_delim |= (z == delimiters[d]);
+      if (is_delim) {
+        int ok = 1;
+        if (i > 0)
+          for (int d = 0; d < n_no_fork_prev; ++d) ok &= (tokens_io[row - 1] != no_fork_prev[d]);
+        if (ok) p = i + 1;
+      }
+    }
+    st[1] = v;
+    st[2] = p;
+    st[5] = b - st[0];
+  }
 }
