@@ -57,10 +57,13 @@ typedef struct {
   int32_t prefix_len;  /* visible cache rows [kv_base_row, kv_base_row+prefix_len) = P+s_l  */
   int32_t q_start;     /* "lane start": first row of the lane in packed Q/K_new/V_new/O/logits      */
   int32_t q_len;       /* "lane length": b_l + w_l rows of u_l (Eq.2)                         */
-  int32_t flags;       /* bit0: refine lane => EOS suppressed in confidence_select          */
+  int32_t flags;       /* bit0: refine lane => EOS suppressed in confidence_select;
+                          bits 8..23: lookahead window w_l (Eq.2), the LAST w_l of the q_len rows */
 } al_lane_desc;
 
 #define AL_LANE_FLAG_REFINE 1
+#define AL_LANE_LOOKAHEAD(flags) (((flags) >> 8) & 0xffff)
+#define AL_LANE_FLAGS(refine, lookahead) (((refine) ? AL_LANE_FLAG_REFINE : 0) | (((lookahead) & 0xffff) << 8))
 
 typedef struct {
   int32_t n_q_heads;  /* H_q                                                            */
@@ -191,6 +194,36 @@ al_status al_confidence_select(al_handle* handle, const void* logits, int32_t lo
                                int32_t n_lanes, int32_t flags, float* conf_out, int32_t* argmax_out,
                                uint8_t* commit_out, int32_t* tokens_out, void* workspace,
                                size_t workspace_bytes, void* cuda_stream);
+
+/* ---- (d) lane status: what the scheduler reads back from one iteration ------------------------- */
+
+/*
+ * Per lane, AFTER the transfer.  A lane's rows are u_l = [z_l ; lookahead window]
+ * (Eq.2): the first b = q_len - w rows are the lane state z_l, the last w = AL_LANE_LOOKAHEAD(flags)
+ * rows the window.
+ *   lookahead rows (Eq.8): commit_io[i] = tokens_in[i] == mask_id && conf[i] >= tau_future &&
+ *     argmax[i] != eos_id;  tokens_io[i] = commit ? argmax[i] : tokens_in[i]   (this call DECIDES those rows,
+ *     whatever al_confidence_select wrote for them)
+ *   n_filled     |{ i < b : z_i != MASK }|                       (Eq.5: fill ratio = n_filled / b)
+ *   valid_prefix v_l = first 0-based i with z_i == MASK or z_i == eos_id, else b          (Eq.9)
+ *   split_point  p_l = 1 + the last 0-based i < b with z_i in delimiter_ids and ValidBoundary, else 0
+ *                (Eq.4).  ValidBoundary (reading C17): the delimiter's previous token (i > 0) is not
+ *                in no_fork_prev_ids -- the "numeric-period patterns excluded" of P:L195
+ *   n_committed  rows of z_l with commit_io set;  n_drafts  lookahead rows drafted;  n_masked = b - n_filled
+ * z is read from tokens_io (on entry the tokens_out of al_confidence_select; must not alias tokens_in).
+ * One small launch, no synchronisation; status_out_dev[n_lanes] is what the host copies back.
+ */
+typedef struct {
+  int32_t n_filled, valid_prefix, split_point, n_committed, n_drafts, n_masked, reserved[2];
+} al_lane_status_rec;
+
+al_status al_lane_status(al_handle* handle, const al_lane_desc* lanes_dev, int32_t n_lanes, int32_t n_rows,
+                         const int32_t* tokens_in_dev, const float* conf_dev, const int32_t* argmax_dev,
+                         int32_t mask_id, int32_t eos_id, float tau_future,
+                         const int32_t* delimiter_ids_dev, int32_t n_delimiters,
+                         const int32_t* no_fork_prev_ids_dev, int32_t n_no_fork_prev,
+                         uint8_t* commit_io_dev, int32_t* tokens_io_dev,
+                         al_lane_status_rec* status_out_dev, void* cuda_stream);
 
 /* ---- whole step from HOST buffers (end-to-end entry) ------------------------------------------ */
 

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_PKG, "libasynclane.so")
 EXPORTS = [
     "al_create", "al_destroy", "al_last_error", "al_version", "al_sm_count",
     "al_lane_attention_workspace_bytes", "al_lane_attention", "al_lane_plan", "al_lane_attention_planned",
-    "al_kv_refresh",
+    "al_kv_refresh", "al_lane_status",
     "al_confidence_select_workspace_bytes", "al_confidence_select", "al_validate_lanes", "al_validate_refresh",
     "al_selftest_umma", "al_lane_step_host", "al_lane_step_host_arena_bytes", "al_lane_step_host_traffic",
     "al_launch_count",
@@ -87,6 +87,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.al_confidence_select_workspace_bytes.restype = sz
     lib.al_confidence_select.argtypes = [vp, vp, i32, i32, i32, i64, vp, i32, i32, f32, vp, i32, i32,
                                          vp, vp, vp, vp, vp, sz, vp]
+    lib.al_lane_status.argtypes = [vp, vp, i32, i32, vp, vp, vp, i32, i32, f32, vp, i32, vp, i32, vp, vp, vp, vp]
     lib.al_validate_lanes.argtypes = [vp, shp, vp, i32, i32]
     lib.al_validate_refresh.argtypes = [vp, shp, vp, i32, i32]
     lib.al_selftest_umma.argtypes = [vp, vp, vp, vp, f32, vp, vp, vp]
@@ -235,6 +236,16 @@ class Handle:
 
     def al_validate_lanes(self, shape, lanes_dev, n_lanes, total_q_rows) -> None:
         _check(self._lib.al_validate_lanes(self._h, ctypes.byref(shape), _ptr(lanes_dev), n_lanes, total_q_rows))
+
+    def al_lane_status(self, lanes_dev, n_lanes, n_rows, tokens_in, conf, argmax, mask_id, eos_id, tau_future,
+                       delimiter_ids, no_fork_prev_ids, commit_io, tokens_io, status_out, stream=None) -> None:
+        """status_out: int32 CUDA tensor [n_lanes, 8] (al_lane_status_rec)."""
+        nd = 0 if delimiter_ids is None else int(delimiter_ids.numel())
+        nn = 0 if no_fork_prev_ids is None else int(no_fork_prev_ids.numel())
+        _check(self._lib.al_lane_status(self._h, _ptr(lanes_dev), n_lanes, n_rows, _ptr(tokens_in), _ptr(conf),
+                                        _ptr(argmax), mask_id, eos_id, tau_future, _ptr(delimiter_ids), nd,
+                                        _ptr(no_fork_prev_ids), nn, _ptr(commit_io), _ptr(tokens_io),
+                                        _ptr(status_out), _stream_ptr(stream)))
 
     def al_validate_refresh(self, shape, pos_dev, n_pos, kv_base_row=0) -> None:
         _check(self._lib.al_validate_refresh(self._h, ctypes.byref(shape), _ptr(pos_dev), n_pos, kv_base_row))
