@@ -225,6 +225,86 @@ al_status al_lane_status(al_handle* handle, const al_lane_desc* lanes_dev, int32
                          uint8_t* commit_io_dev, int32_t* tokens_io_dev,
                          al_lane_status_rec* status_out_dev, void* cuda_stream);
 
+/* ---- (e) host scheduler: Algorithm 1 driving the calls above ---------------------------------- */
+
+/*
+ * AsyncLane active-lane decoding (Alg.1) of ONE sequence, as host control flow around the
+ * device calls: per iteration the active lanes A_t (Eq.10) are packed into lane descriptors,
+ * the model is called once for all of them (Eq.11), al_confidence_select applies the transfer rule
+ * (refine lanes suppress EOS; one token per lane is forced so that a lane's budget is finite, reading
+ * C4), al_lane_status returns the per-lane integers, and the host applies the fork operator (Eq.6),
+ * completion / successor spawning with cascading termination (Eq.9, Alg.1 lines 10-17) and the
+ * periodic compact refresh (Eq.12).  COLLECTDFS reconstructs the output.
+ * Readings (C18-C21): a lane forks when 0 < p_l < b_l, n_filled / b_l >= rho_min, t_l >= t_min
+ * and it still holds a MASK; the refine child covers [s, s + p) with a fresh clock, the continuation starts
+ * at s + p with min(B, L - (s + p)) tokens; a lane is completed when it holds no MASK or after max_lane_steps
+ * steps; a completed unforked generate lane spawns a successor at s + v_l unless v_l = 0 or s + v_l >= L;
+ * generate lanes get a lookahead window of min(W, L - (s + b)) rows; all lanes of the sequence share the
+ * cache rows (group 0, kv_base_row 0) and see prefix_len = P + s of them (reading C1).
+ * The model is a callback: it receives the iteration's lanes (host copies), each lane's local step, the
+ * packed input rows (device) with their global positions, and writes fp32 logits [n_rows][vocab] (device)
+ * on the given stream.  al_stub_model_fn is a table-driven stand-in for tests and benchmarks (there are no
+ * weights here): logits[row][v] = base[pos][v] + gain * (step + 1) * (v == target[pos]).
+ * This entry allocates its own device and pinned buffers, synchronises once per iteration (the scheduler
+ * reads 32 bytes per lane and the transferred tokens back) and frees everything before it returns.
+ */
+typedef struct {
+  int32_t prompt_len, gen_len, block_size, lookahead;      /* P, L, B, W                                  */
+  int32_t vocab, mask_id, eos_id;
+  float tau, tau_future, rho_min;                          /* transfer / draft thresholds, Eq.5 fill ratio */
+  int32_t t_min, max_lane_steps, max_iterations;           /* Eq.5 t_min; denoising budget per lane; total */
+  int32_t refresh_period, refresh_margin;                  /* iterations between refreshes (0: never); m   */
+  const int32_t* delimiter_ids;    int32_t n_delimiters;   /* HOST arrays: D_task                         */
+  const int32_t* no_fork_prev_ids; int32_t n_no_fork_prev; /*              ValidBoundary exclusion        */
+} al_sched_config;
+
+typedef struct {             /* one node of the lane tree T_lane (host) */
+  int32_t role;              /* 0 generate, 1 refine                                                       */
+  int32_t start, len, steps; /* s_l, b_l, t_l                                                              */
+  int32_t parent, ref_child, gen_child, successor;   /* node indices, -1 = none                           */
+  int32_t state;             /* 0 active, 1 completed, 2 forked                                            */
+  int32_t valid_prefix, split_point, n_masked;       /* as of the lane's last update                      */
+} al_sched_lane;
+
+typedef struct {
+  int32_t iterations, model_calls, lane_forwards, forks, successors, refreshes, stopped_frontiers;
+  int32_t rows_forwarded, tokens_committed, tokens_drafted, refreshed_rows_last, reserved;
+} al_sched_stats;
+
+typedef int (*al_model_fn)(void* user, const al_lane_desc* lanes_host, const int32_t* lane_steps_host,
+                           int32_t n_lanes, int32_t n_rows, const int32_t* row_pos_dev,
+                           const int32_t* tokens_dev, float* logits_dev, void* cuda_stream);
+
+typedef struct {             /* user data of al_stub_model_fn; the tables live in DEVICE memory */
+  const float* base_dev;     /* [gen_len][vocab]                                                           */
+  const int32_t* target_dev; /* [gen_len]                                                                  */
+  float gain;
+  int32_t vocab;
+} al_stub_model;
+int al_stub_model_fn(void* user, const al_lane_desc* lanes_host, const int32_t* lane_steps_host,
+                     int32_t n_lanes, int32_t n_rows, const int32_t* row_pos_dev, const int32_t* tokens_dev,
+                     float* logits_dev, void* cuda_stream);
+
+typedef struct {             /* optional device state the scheduler drives besides the logits (may be NULL) */
+  al_attn_shape shape;       /* cache_rows >= P + L                                                        */
+  void* k_cache; void* v_cache;            /* [H_kv][cache_rows][d]: refreshed rows are written here      */
+  const void* k_src; const void* v_src;    /* [P + L][H_kv][d]: recomputed prefix states (Eq.12 source)   */
+  const void* q; const void* k_new; const void* v_new;   /* [max_rows][H][d] lane inputs of the stub layer */
+  void* out;                               /* [max_rows][H_q][d]; NULL q => no attention is run           */
+  int32_t max_rows;
+} al_sched_device_state;
+
+/*
+ * prompt_host [P]; x_host [P + L] receives the final global token state; output_host [L] the collected
+ * sequence (n_output tokens); tree_out [max_tree] the lane tree (n_tree nodes; node 0 is the root).
+ * Returns AL_ERR_UNSUPPORTED when the tree outgrows max_tree, AL_ERR_CUDA when the model callback fails.
+ */
+al_status al_scheduler_run(al_handle* handle, const al_sched_config* config, al_model_fn model,
+                           void* model_user, const al_sched_device_state* device_state_or_null,
+                           const int32_t* prompt_host, int32_t* x_host, int32_t* output_host,
+                           int32_t* n_output, al_sched_lane* tree_out, int32_t max_tree, int32_t* n_tree,
+                           al_sched_stats* stats_out, void* cuda_stream);
+
 /* ---- whole step from HOST buffers (end-to-end entry) ------------------------------------------ */
 
 /*

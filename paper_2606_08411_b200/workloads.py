@@ -315,3 +315,31 @@ CONFIGS = {
     "cfg4": cfg4_long_llada,
     "cfg5": cfg5_throughput_batch,
 }
+
+
+def scheduler_case(seed: int, prompt_len: int = 24, gen_len: int = 160, block_size: int = 32, lookahead: int = 8,
+                   vocab: int = 64, eos_frac: float = 0.8) -> Dict[str, object]:
+    """Inputs of one scheduler run (Alg.1) with the table-driven stub model (there are no
+    weights): a target "text" of sentences over token ids 20.., delimiter id 7 every 6..20 tokens (a third of
+    them after the digit id 5: the numeric-period exclusion of L195), EOS (id 2) from eos_frac of the generation
+    length on; `base` [gen_len][vocab] float32 logits in eighths (exactly representable), the target token's base
+    logit in [-1, 3] so that positions reach the threshold after different numbers of steps while the target is
+    the row maximum from the first step.  Data only: no arithmetic of the method."""
+    rng = np.random.default_rng(seed)
+    mask_id, eos_id, delim, digit = vocab - 1, 2, 7, 5
+    target = rng.integers(20, vocab - 4, size=gen_len).astype(np.int32)
+    i = int(rng.integers(6, 21))
+    while i < gen_len:
+        target[i] = delim
+        if i > 0 and rng.random() < 0.33:
+            target[i - 1] = digit
+        i += int(rng.integers(6, 21))
+    eos_at = int(eos_frac * gen_len)
+    target[eos_at:] = eos_id                               # a finished sequence is padded with EOS
+    base = (rng.integers(-24, -7, size=(gen_len, vocab)) / 8.0).astype(np.float32)        # others in [-3, -1]
+    base[np.arange(gen_len), target] = (rng.integers(-8, 25, size=gen_len) / 8.0).astype(np.float32)   # [-1, 3]
+    prompt = rng.integers(20, vocab - 4, size=prompt_len).astype(np.int32)
+    cfg = dict(prompt_len=prompt_len, gen_len=gen_len, block_size=block_size, lookahead=lookahead, vocab=vocab,
+               mask_id=mask_id, eos_id=eos_id, tau=0.9, tau_future=0.95, rho_min=0.5, t_min=2, max_lane_steps=24,
+               max_iterations=400, refresh_period=4, refresh_margin=8, delimiter_ids=[delim], no_fork_prev_ids=[digit])
+    return dict(cfg=cfg, base=base, target=target, gain=0.75, prompt=prompt, eos_at=eos_at)
