@@ -242,8 +242,9 @@ al_status al_lane_status(al_handle* handle, const al_lane_desc* lanes_dev, int32
  * generate lanes get a lookahead window of min(W, L - (s + b)) rows; all lanes of the sequence share the
  * cache rows (group 0, kv_base_row 0) and see prefix_len = P + s of them (reading C1).
  * The model is a callback: it receives the iteration's lanes (host copies), each lane's local step, the
- * packed input rows (device) with their global positions, and writes fp32 logits [n_rows][vocab] (device)
- * on the given stream.  al_stub_model_fn is a table-driven stand-in for tests and benchmarks (there are no
+ * packed input rows tokens_dev [n_rows] (device), row_pos_dev [2][n_rows] (device: the rows' positions in
+ * generation coordinates, then the rows' lane-local steps), and writes fp32 logits [n_rows][vocab] (device)
+ * on the given stream; it returns 0 on success.  al_stub_model_fn is a table-driven stand-in for tests and benchmarks (there are no
  * weights here): logits[row][v] = base[pos][v] + gain * (step + 1) * (v == target[pos]).
  * This entry allocates its own device and pinned buffers, synchronises once per iteration (the scheduler
  * reads 32 bytes per lane and the transferred tokens back) and frees everything before it returns.

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_PKG, "libasynclane.so")
 EXPORTS = [
     "al_create", "al_destroy", "al_last_error", "al_version", "al_sm_count",
     "al_lane_attention_workspace_bytes", "al_lane_attention", "al_lane_plan", "al_lane_attention_planned",
-    "al_kv_refresh", "al_lane_status",
+    "al_kv_refresh", "al_lane_status", "al_scheduler_run", "al_stub_model_fn",
     "al_confidence_select_workspace_bytes", "al_confidence_select", "al_validate_lanes", "al_validate_refresh",
     "al_selftest_umma", "al_lane_step_host", "al_lane_step_host_arena_bytes", "al_lane_step_host_traffic",
     "al_launch_count",
@@ -54,6 +54,43 @@ class al_host_step(ctypes.Structure):
                 ("commit", ctypes.c_void_p), ("tokens_out", ctypes.c_void_p),
                 ("n_layers", ctypes.c_int32), ("reserved", ctypes.c_int32), ("cache_layer_stride", ctypes.c_int64)]
 
+
+class al_sched_config(ctypes.Structure):
+    """Mirror of al_sched_config (include/asynclane.h): Algorithm 1's parameters; the id lists are HOST arrays."""
+    _fields_ = [("prompt_len", ctypes.c_int32), ("gen_len", ctypes.c_int32), ("block_size", ctypes.c_int32),
+                ("lookahead", ctypes.c_int32), ("vocab", ctypes.c_int32), ("mask_id", ctypes.c_int32),
+                ("eos_id", ctypes.c_int32), ("tau", ctypes.c_float), ("tau_future", ctypes.c_float),
+                ("rho_min", ctypes.c_float), ("t_min", ctypes.c_int32), ("max_lane_steps", ctypes.c_int32),
+                ("max_iterations", ctypes.c_int32), ("refresh_period", ctypes.c_int32),
+                ("refresh_margin", ctypes.c_int32), ("delimiter_ids", ctypes.c_void_p), ("n_delimiters", ctypes.c_int32),
+                ("no_fork_prev_ids", ctypes.c_void_p), ("n_no_fork_prev", ctypes.c_int32)]
+
+
+class al_sched_lane(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("role", "start", "len", "steps", "parent", "ref_child", "gen_child",
+                                              "successor", "state", "valid_prefix", "split_point", "n_masked")]
+
+
+class al_sched_stats(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("iterations", "model_calls", "lane_forwards", "forks", "successors",
+                                              "refreshes", "stopped_frontiers", "rows_forwarded", "tokens_committed",
+                                              "tokens_drafted", "refreshed_rows_last", "reserved")]
+
+
+class al_stub_model(ctypes.Structure):
+    _fields_ = [("base_dev", ctypes.c_void_p), ("target_dev", ctypes.c_void_p), ("gain", ctypes.c_float),
+                ("vocab", ctypes.c_int32)]
+
+
+class al_sched_device_state(ctypes.Structure):
+    _fields_ = [("shape", al_attn_shape), ("k_cache", ctypes.c_void_p), ("v_cache", ctypes.c_void_p),
+                ("k_src", ctypes.c_void_p), ("v_src", ctypes.c_void_p), ("q", ctypes.c_void_p),
+                ("k_new", ctypes.c_void_p), ("v_new", ctypes.c_void_p), ("out", ctypes.c_void_p),
+                ("max_rows", ctypes.c_int32)]
+
+
+AL_MODEL_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
+                               ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p)
 
 _lib: Optional[ctypes.CDLL] = None
 
@@ -88,6 +125,9 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.al_confidence_select.argtypes = [vp, vp, i32, i32, i32, i64, vp, i32, i32, f32, vp, i32, i32,
                                          vp, vp, vp, vp, vp, sz, vp]
     lib.al_lane_status.argtypes = [vp, vp, i32, i32, vp, vp, vp, i32, i32, f32, vp, i32, vp, i32, vp, vp, vp, vp]
+    lib.al_scheduler_run.argtypes = [vp, ctypes.POINTER(al_sched_config), vp, vp, ctypes.POINTER(al_sched_device_state),
+                                     vp, vp, vp, ctypes.POINTER(i32), ctypes.POINTER(al_sched_lane), i32,
+                                     ctypes.POINTER(i32), ctypes.POINTER(al_sched_stats), vp]
     lib.al_validate_lanes.argtypes = [vp, shp, vp, i32, i32]
     lib.al_validate_refresh.argtypes = [vp, shp, vp, i32, i32]
     lib.al_selftest_umma.argtypes = [vp, vp, vp, vp, f32, vp, vp, vp]
@@ -104,7 +144,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         fn = getattr(lib, name)
         if name not in ("al_last_error", "al_version", "al_sm_count", "al_lane_attention_workspace_bytes",
                         "al_confidence_select_workspace_bytes", "al_lane_step_host_arena_bytes",
-                        "al_lane_step_host_traffic", "al_launch_count"):
+                        "al_lane_step_host_traffic", "al_launch_count", "al_stub_model_fn"):
             fn.restype = ctypes.c_int
     _lib = lib
     return lib
@@ -246,6 +286,19 @@ class Handle:
                                         _ptr(argmax), mask_id, eos_id, tau_future, _ptr(delimiter_ids), nd,
                                         _ptr(no_fork_prev_ids), nn, _ptr(commit_io), _ptr(tokens_io),
                                         _ptr(status_out), _stream_ptr(stream)))
+
+    def al_scheduler_run(self, config: al_sched_config, model_fn, model_user, device_state, prompt_host, x_host,
+                         output_host, tree, stream=None):
+        """model_fn: a C function pointer (the library's al_stub_model_fn, or an AL_MODEL_FN wrapping a Python
+        callable); model_user: ctypes pointer/int passed through; prompt/x/output: int32 numpy arrays (host);
+        tree: ctypes array of al_sched_lane.  Returns (n_output, n_tree, al_sched_stats)."""
+        n_out, n_tree, stats = ctypes.c_int32(0), ctypes.c_int32(0), al_sched_stats()
+        ds = None if device_state is None else ctypes.byref(device_state)
+        _check(self._lib.al_scheduler_run(self._h, ctypes.byref(config), ctypes.cast(model_fn, ctypes.c_void_p),
+                                          model_user, ds, prompt_host.ctypes.data, x_host.ctypes.data,
+                                          output_host.ctypes.data, ctypes.byref(n_out), tree, len(tree),
+                                          ctypes.byref(n_tree), ctypes.byref(stats), _stream_ptr(stream)))
+        return int(n_out.value), int(n_tree.value), stats
 
     def al_validate_refresh(self, shape, pos_dev, n_pos, kv_base_row=0) -> None:
         _check(self._lib.al_validate_refresh(self._h, ctypes.byref(shape), _ptr(pos_dev), n_pos, kv_base_row))
