@@ -161,3 +161,23 @@ def lane_status(lanes, tokens_in, conf, argmax, mask_id: int, eos_id: int, tau_f
                                _p(no_fork_prev) if no_fork_prev.size else None, ctypes.c_int(no_fork_prev.size),
                                _p(commit_io), _p(tokens_io), _p(status))
     return dict(status=status, commit=commit_io, tokens_out=tokens_io)
+
+
+def refresh_forward(q, k_new, v_new, k_cache, v_cache, lanes, scale: Optional[float] = None):
+    """O-E.  Attention of every lane over [its prefix ; its own rows] (O-A), then the lanes' K_new/V_new rows
+    written into the caches behind their prefixes, IN PLACE on k_cache / v_cache (float32 [Hkv,cache_rows,d]).
+    Returns (out fp64 [T,Hq,d], lse fp64 [T,Hq])."""
+    q, k_new, v_new = map(_f32, (q, k_new, v_new))
+    assert k_cache.dtype == np.float32 and v_cache.dtype == np.float32
+    assert k_cache.flags["C_CONTIGUOUS"] and v_cache.flags["C_CONTIGUOUS"]
+    lanes = _i32(lanes).reshape(-1, 6)
+    T, Hq, d = q.shape
+    Hkv, cache_rows = k_cache.shape[0], k_cache.shape[1]
+    if scale is None:
+        scale = 1.0 / np.sqrt(float(d))
+    out = np.zeros((T, Hq, d), dtype=np.float64)
+    lse = np.zeros((T, Hq), dtype=np.float64)
+    _load().oracle_refresh_forward(_p(q), _p(k_new), _p(v_new), _p(k_cache), _p(v_cache), _p(lanes),
+                                   ctypes.c_int(lanes.shape[0]), ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d),
+                                   ctypes.c_int64(cache_rows), ctypes.c_double(scale), _p(out), _p(lse))
+    return out, lse

@@ -266,3 +266,31 @@ void oracle_lane_status(const int32_t* lanes, int n_lanes, int n_rows, const int
     st[5] = b - st[0];
   }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * O-E  refresh forward (Eq.12): the prefix states of a range are
+ * RECOMPUTED -- bidirectional attention of the range's rows over [older prefix ; the range itself]
+ * (Eq.2-3 with the range as the "lane") -- and the recomputed K/V rows are written into the cache right
+ * behind that older prefix:
+ *     out, lse        = O-A on the same arguments (the cache is read BEFORE it is written)
+ *     cache[g][kv_base_row + prefix_len + i][:] = k_new[q_start + i][g][:]   for i in [0, q_len)   (K and V)
+ * Eq.12's own case is prefix_len = 0, q_len = L_refresh: dense self-attention over the refreshed range whose
+ * states replace cache rows [0, L_refresh).  The same call with prefix_len > 0 is the "finalize the valid
+ * prefix" append of Alg.1 line 16.  Caches are float32 here (values already rounded to the I/O dtype).
+ * -----------------------------------------------------------------------------------------*/
+void oracle_refresh_forward(const float* q, const float* k_new, const float* v_new, float* k_cache, float* v_cache,
+                            const int32_t* lanes, int n_lanes, int n_q_heads, int n_kv_heads, int head_dim,
+                            int64_t cache_rows, double scale, double* out, double* lse) {
+  oracle_lane_attention(q, k_new, v_new, k_cache, v_cache, lanes, n_lanes, n_q_heads, n_kv_heads, head_dim, cache_rows,
+                        scale, out, lse);
+  for (int l = 0; l < n_lanes; ++l) {
+    const int32_t* lane = lanes + 6 * l;
+    for (int i = 0; i < lane[4]; ++i)
+      for (int g = 0; g < n_kv_heads; ++g) {
+        const int64_t dst = ((int64_t)g * cache_rows + lane[1] + lane[2] + i) * head_dim;
+        const int64_t src = ((int64_t)(lane[3] + i) * n_kv_heads + g) * head_dim;
+        memcpy(k_cache + dst, k_new + src, sizeof(float) * (size_t)head_dim);
+        memcpy(v_cache + dst, v_new + src, sizeof(float) * (size_t)head_dim);
+      }
+  }
+}
