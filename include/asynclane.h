@@ -169,6 +169,23 @@ al_status al_kv_refresh(al_handle* handle, const al_attn_shape* shape, void* k_c
                         int32_t kv_base_row, int32_t n_layers, int64_t layer_stride_cache,
                         int64_t layer_stride_src, void* cuda_stream);
 
+/*
+ * Refresh forward (Eq.12): the prefix states of a range are recomputed and
+ * replace the cached ones.  Each descriptor is one RANGE: its q_len rows (q, k_new, v_new: the recomputed
+ * activations of this layer) attend bidirectionally to [the older prefix the range keeps: cache rows
+ * kv_base_row + [0, prefix_len) ; the range itself] exactly as in al_lane_attention, and then
+ *   k_cache[g][kv_base_row + prefix_len + i][:] = k_new[q_start + i][g][:]      (same for V), i in [0, q_len)
+ * Eq.12's own case is prefix_len = 0, q_len = L_refresh (dense self-attention over the refreshed range); with
+ * prefix_len > 0 the same call appends a finalized valid prefix (Alg.1 line 16).  The attention reads the
+ * cache BEFORE these rows are written (stream order); kv_base_row + prefix_len + q_len <= cache_rows.
+ * Arguments, limits and workspace as al_lane_attention (max_prefix_len >= every prefix_len).
+ */
+al_status al_refresh_forward(al_handle* handle, const al_attn_shape* shape, const void* q,
+                             const void* k_new, const void* v_new, void* k_cache, void* v_cache,
+                             const al_lane_desc* lanes_dev, int32_t n_lanes, int32_t total_q_rows,
+                             int32_t max_prefix_len, void* out, float* lse_or_null, void* workspace,
+                             size_t workspace_bytes, void* cuda_stream);
+
 /* ---- (c) confidence / argmax / threshold select ----------------------------------------------- */
 
 #define AL_SELECT_FORCE_TOP1 1

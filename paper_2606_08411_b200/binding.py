@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_PKG, "libasynclane.so")
 EXPORTS = [
     "al_create", "al_destroy", "al_last_error", "al_version", "al_sm_count",
     "al_lane_attention_workspace_bytes", "al_lane_attention", "al_lane_plan", "al_lane_attention_planned",
-    "al_kv_refresh", "al_lane_status", "al_scheduler_run", "al_stub_model_fn",
+    "al_kv_refresh", "al_refresh_forward", "al_lane_status", "al_scheduler_run", "al_stub_model_fn",
     "al_confidence_select_workspace_bytes", "al_confidence_select", "al_validate_lanes", "al_validate_refresh",
     "al_selftest_umma", "al_lane_step_host", "al_lane_step_host_arena_bytes", "al_lane_step_host_traffic",
     "al_launch_count",
@@ -118,6 +118,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.al_lane_attention_workspace_bytes.restype = sz
     lib.al_lane_attention.argtypes = [vp, shp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, sz, vp]
     lib.al_lane_attention_planned.argtypes = lib.al_lane_attention.argtypes
+    lib.al_refresh_forward.argtypes = lib.al_lane_attention.argtypes
     lib.al_lane_plan.argtypes = [vp, shp, vp, i32, i32, i32, vp, sz, vp]
     lib.al_kv_refresh.argtypes = [vp, shp, vp, vp, vp, vp, vp, i32, i32, i32, i64, i64, vp]
     lib.al_confidence_select_workspace_bytes.argtypes = [i32, i32]
@@ -223,6 +224,14 @@ class Handle:
                                            _ptr(k_cache), _ptr(v_cache), _ptr(lanes_dev), n_lanes, total_q_rows,
                                            max_prefix_len, _ptr(out), _ptr(lse), _ptr(workspace), ws_bytes,
                                            _stream_ptr(stream)))
+
+    def al_refresh_forward(self, shape, q, k_new, v_new, k_cache, v_cache, lanes_dev, n_lanes, total_q_rows,
+                           max_prefix_len, out, lse=None, workspace=None, stream=None) -> None:
+        ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+        _check(self._lib.al_refresh_forward(self._h, ctypes.byref(shape), _ptr(q), _ptr(k_new), _ptr(v_new),
+                                            _ptr(k_cache), _ptr(v_cache), _ptr(lanes_dev), n_lanes, total_q_rows,
+                                            max_prefix_len, _ptr(out), _ptr(lse), _ptr(workspace), ws_bytes,
+                                            _stream_ptr(stream)))
 
     def al_lane_plan(self, shape, lanes_dev, n_lanes, total_q_rows, max_prefix_len, workspace, stream=None) -> None:
         ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()

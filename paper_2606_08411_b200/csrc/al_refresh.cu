@@ -65,7 +65,67 @@ kv_refresh_kernel(int4* __restrict__ k_cache, int4* __restrict__ v_cache,
   }
 }
 
+// K2b kv_append_kernel (al_refresh_forward): cache[g][kv_base_row + prefix_len + i][:] = src[q_start + i][g][:] for every
+// lane, K and V, as 16-byte vectors.  blockIdx.y = lane; the blocks of a lane stride over its q_len * H_kv * vecs items.
+__global__ void __launch_bounds__(kThreads)
+kv_append_kernel(int4* __restrict__ k_cache, int4* __restrict__ v_cache, const int4* __restrict__ k_src,
+                 const int4* __restrict__ v_src, const al_lane_desc* __restrict__ lanes, int n_kv_heads,
+                 long long cache_rows, int vecs_per_row) {
+  // programmatic dependent launch: behind the attention that still reads the cache rows written here
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const al_lane_desc L = lanes[blockIdx.y];
+  const long long items = (long long)L.q_len * n_kv_heads * vecs_per_row;
+  const long long dst_row0 = (long long)L.kv_base_row + L.prefix_len;
+  for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < items; i += (long long)gridDim.x * kThreads) {
+    const int c = (int)(i % vecs_per_row);
+    const long long rg = i / vecs_per_row;
+    const int g = (int)(rg % n_kv_heads);
+    const long long r = rg / n_kv_heads;
+    const long long s = ((long long)(L.q_start + r) * n_kv_heads + g) * vecs_per_row + c;
+    const long long d = ((long long)g * cache_rows + dst_row0 + r) * vecs_per_row + c;
+    k_cache[d] = ld_stream(k_src + s);
+    v_cache[d] = ld_stream(v_src + s);
+  }
+}
+
 }  // namespace
+
+// al_refresh_forward: the refresh forward of Eq.12 -- the lane-batched attention
+// of the given ranges over [their older prefix ; themselves] on the tcgen05 path, then their K/V rows written into the
+// cache behind that prefix.  The attention reads the cache before the append writes it (stream order).
+extern "C" al_status al_refresh_forward(al_handle* h, const al_attn_shape* s, const void* q, const void* k_new,
+                                        const void* v_new, void* k_cache, void* v_cache, const al_lane_desc* lanes,
+                                        int32_t n_lanes, int32_t total_q_rows, int32_t max_prefix_len, void* out,
+                                        float* lse, void* workspace, size_t workspace_bytes, void* stream) {
+  const char* who = "al_refresh_forward";
+  al_status st = al_lane_attention_impl(4, who, h, s, q, k_new, v_new, k_cache, v_cache, lanes, n_lanes, total_q_rows,
+                                        max_prefix_len, out, lse, workspace, workspace_bytes, stream);
+  if (st != AL_OK) return st;
+  if (n_lanes == 0 || total_q_rows == 0) return AL_OK;
+  if (!k_cache || !v_cache || s->cache_rows <= 0) AL_FAIL(AL_ERR_INVALID_ARG, "%s: no cache to write", who);
+  const long long row_bytes = (long long)s->head_dim * al_esize(s->dtype);
+  if (row_bytes % 16 != 0) AL_FAIL(AL_ERR_UNSUPPORTED, "%s: head_dim*esize = %lld not a multiple of 16", who, row_bytes);
+  st = al_lane_attention_impl(3, who, h, s, q, k_new, v_new, k_cache, v_cache, lanes, n_lanes, total_q_rows, max_prefix_len,
+                              out, lse, workspace, workspace_bytes, stream);
+  if (st != AL_OK) return st;
+  const int vpr = (int)(row_bytes / 16);
+  long long bx = ((long long)total_q_rows * s->n_kv_heads * vpr + kThreads * 4 - 1) / (kThreads * 4);
+  bx = bx < 1 ? 1 : (bx > 32 ? 32 : bx);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)bx, (unsigned)n_lanes);
+  cfg.blockDim = dim3(kThreads);
+  cfg.stream = static_cast<cudaStream_t>(stream);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.wait in the kernel
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, kv_append_kernel, (int4*)k_cache, (int4*)v_cache, (const int4*)k_new,
+                                (const int4*)v_new, lanes, (int)s->n_kv_heads, (long long)s->cache_rows, vpr));
+  h->launches++;
+  return AL_OK;
+}
 
 al_status al_kv_refresh_check(const char* who, const al_handle* h, const al_attn_shape* s, const void* k_cache,
                               const void* v_cache, const void* k_src, const void* v_src, const int32_t* pos_dev,
