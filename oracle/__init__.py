@@ -181,3 +181,24 @@ def refresh_forward(q, k_new, v_new, k_cache, v_cache, lanes, scale: Optional[fl
                                    ctypes.c_int(lanes.shape[0]), ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d),
                                    ctypes.c_int64(cache_rows), ctypes.c_double(scale), _p(out), _p(lse))
     return out, lse
+
+
+def lm_head_confidence(hidden, weight, tokens_in, mask_id: int, eos_id: int, threshold: float, lanes=None,
+                       force_top1: bool = False):
+    """O-F.  hidden [N,K], weight [V,K] (float32 values already rounded to the I/O dtype); logits = hidden @ weight.T
+    in fp64, consumed by the rule of O-C.  Returns the same dict as confidence_select."""
+    hidden, weight = _f32(hidden), _f32(weight)
+    N, K = hidden.shape
+    V = weight.shape[0]
+    assert weight.shape == (V, K)
+    tokens_in = _i32(tokens_in)
+    lanes_arr = None if lanes is None else _i32(lanes).reshape(-1, 6)
+    conf, p2 = np.zeros(N, np.float64), np.zeros(N, np.float64)
+    argmax, commit, tokens_out = np.zeros(N, np.int32), np.zeros(N, np.uint8), np.zeros(N, np.int32)
+    _load().oracle_lm_head_confidence(_p(hidden), _p(weight), ctypes.c_int(N), ctypes.c_int(V), ctypes.c_int(K),
+                                      _p(tokens_in), ctypes.c_int(mask_id), ctypes.c_int(eos_id),
+                                      ctypes.c_double(threshold), _p(lanes_arr),
+                                      ctypes.c_int(0 if lanes_arr is None else lanes_arr.shape[0]),
+                                      ctypes.c_int(1 if force_top1 else 0), _p(conf), _p(argmax), _p(p2), _p(commit),
+                                      _p(tokens_out))
+    return dict(conf=conf, argmax=argmax, p2=p2, commit=commit, tokens_out=tokens_out)

@@ -294,3 +294,75 @@ void oracle_refresh_forward(const float* q, const float* k_new, const float* v_n
       }
   }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * O-F  LM head fused with the transfer rule (the step upstream of PAPER.md L78:
+ * "the first b_l logits of o_l are used to update the current lane"): the logits of row i are
+ *     o_iv = sum_k hidden[i][k] * weight[v][k]            (weight stored [V][K] as a linear layer keeps it)
+ * and are consumed by exactly the rule of O-C (first argmax, q = 1 / sum_v exp(o_v - max), EOS = -inf on
+ * refine-lane rows, commit iff MASK and q >= tau, optional force-top1) WITHOUT ever being stored as an
+ * [N][V] array by the product.  Here they are formed in fp64, one row at a time, and fed through the same
+ * steps in the same order as O-C.
+ * -----------------------------------------------------------------------------------------*/
+void oracle_lm_head_confidence(const float* hidden, const float* weight, int n_rows, int vocab, int hidden_dim,
+                               const int32_t* tokens_in, int mask_id, int eos_id, double threshold,
+                               const int32_t* lanes, int n_lanes, int flags, double* conf, int32_t* argmax,
+                               double* p2, uint8_t* commit, int32_t* tokens_out) {
+  uint8_t* suppress = (uint8_t*)calloc((size_t)(n_rows > 0 ? n_rows : 1), 1);
+  if (lanes && eos_id >= 0)
+    for (int l = 0; l < n_lanes; ++l)
+      if (lanes[6 * l + 5] & 1)
+        for (int i = 0; i < lanes[6 * l + 4]; ++i) {
+          const int row = lanes[6 * l + 3] + i;
+          if (row >= 0 && row < n_rows) suppress[row] = 1;
+        }
+#pragma omp parallel
+  {
+    double* x = (double*)malloc(sizeof(double) * (size_t)vocab);
+#pragma omp for schedule(dynamic, 1)
+    for (int i = 0; i < n_rows; ++i) {
+      const float* h = hidden + (int64_t)i * hidden_dim;
+      for (int v = 0; v < vocab; ++v) {
+        const float* w = weight + (int64_t)v * hidden_dim;
+        double acc = 0.0;
+        for (int k = 0; k < hidden_dim; ++k) acc += (double)h[k] * (double)w[k];
+        x[v] = acc;
+      }
+      if (suppress[i]) x[eos_id] = -INFINITY;
+      int a = -1;
+      double m = -INFINITY;
+      for (int v = 0; v < vocab; ++v)
+        if (a < 0 || x[v] > m) { m = x[v]; a = v; }        /* strict > keeps the first maximiser */
+      double Z = 0.0, second = -INFINITY;
+      for (int v = 0; v < vocab; ++v) {
+        Z += exp(x[v] - m);
+        if (v != a && x[v] > second) second = x[v];
+      }
+      conf[i] = 1.0 / Z;
+      argmax[i] = a;
+      if (p2) p2[i] = (vocab > 1) ? exp(second - m) / Z : 0.0;
+      commit[i] = (uint8_t)(tokens_in[i] == mask_id && conf[i] >= threshold);
+    }
+    free(x);
+  }
+  if (flags & 1) {                                        /* force-top1 per lane, as in O-C */
+    const int32_t whole[6] = {0, 0, 0, 0, n_rows, 0};
+    const int nl = lanes ? n_lanes : 1;
+    for (int l = 0; l < nl; ++l) {
+      const int32_t* lane = lanes ? lanes + 6 * l : whole;
+      int any_masked = 0, any_commit = 0, best = -1;
+      for (int i = 0; i < lane[4]; ++i) {
+        const int row = lane[3] + i;
+        if (row < 0 || row >= n_rows) continue;
+        if (tokens_in[row] == mask_id) {
+          any_masked = 1;
+          if (best < 0 || conf[row] > conf[best]) best = row;
+        }
+        if (commit[row]) any_commit = 1;
+      }
+      if (any_masked && !any_commit) commit[best] = 1;
+    }
+  }
+  for (int i = 0; i < n_rows; ++i) tokens_out[i] = commit[i] ? argmax[i] : tokens_in[i];
+  free(suppress);
+}
