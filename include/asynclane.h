@@ -212,6 +212,25 @@ al_status al_confidence_select(al_handle* handle, const void* logits, int32_t lo
                                uint8_t* commit_out, int32_t* tokens_out, void* workspace,
                                size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * LM head fused with the transfer rule (the step upstream of P:L78): the logits
+ *   o[i][v] = sum_k hidden[i][k] * weight[v][k]          hidden [n_rows][hidden_dim], weight [vocab][hidden_dim],
+ * both bf16 row-major (the layout a linear layer keeps), fp32 accumulation on the tensor cores, are consumed
+ * tile by tile by the recurrence of al_confidence_select and never stored: outputs, EOS suppression on refine
+ * lanes, commit rule and AL_SELECT_FORCE_TOP1 are exactly those of al_confidence_select (argmax = first
+ * maximiser of the fp32 logits).  hidden_dim must be a multiple of 8; any n_rows, vocab.  The workspace
+ * (al_lm_head_confidence_workspace_bytes) holds one (m, s, idx) per row and vocabulary chunk; no zeroing needed.
+ * With few rows (<= 512) the call streams the weights once at HBM rate; with many it is bound by the tensor
+ * cores' operand traffic through L2 (single-CTA 128 x 256 tiles) -- see DESIGN.md K5.
+ */
+size_t al_lm_head_confidence_workspace_bytes(int32_t n_rows, int32_t vocab);
+al_status al_lm_head_confidence(al_handle* handle, const void* hidden_bf16, const void* weight_bf16,
+                                int32_t n_rows, int32_t vocab, int32_t hidden_dim,
+                                const int32_t* tokens_in_dev, int32_t mask_id, int32_t eos_id, float threshold,
+                                const al_lane_desc* lanes_dev_or_null, int32_t n_lanes, int32_t flags,
+                                float* conf_out, int32_t* argmax_out, uint8_t* commit_out, int32_t* tokens_out,
+                                void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---- (d) lane status: what the scheduler reads back from one iteration ------------------------- */
 
 /*

@@ -395,6 +395,16 @@ cudaError_t launch_select(int k, int n_rows, cudaStream_t cs, const T* logits, i
 
 // The cluster/DSMEM merge keeps every partial on chip: no HBM workspace is needed.  The entry point stays in
 // the ABI (callers size their arenas through it) and returns 0; al_confidence_select accepts workspace == NULL.
+al_status al_launch_force_top1(al_handle* h, const al_lane_desc* lanes, int n_lanes, int n_rows, int mask_id,
+                               const float* conf, const int32_t* argmax, uint8_t* commit, int32_t* tokens_out,
+                               cudaStream_t cs) {
+  force_top1_kernel<<<(n_lanes + kWarps - 1) / kWarps, kThreads, 0, cs>>>(lanes, n_lanes, n_rows, mask_id, conf, argmax,
+                                                                         commit, tokens_out);
+  AL_CUDA_OK(cudaGetLastError());
+  h->launches++;
+  return AL_OK;
+}
+
 extern "C" size_t al_confidence_select_workspace_bytes(int32_t n_rows, int32_t vocab) {
   (void)n_rows; (void)vocab;
   return 0;

@@ -1,0 +1,106 @@
+"""GPU parity of al_lm_head_confidence against oracle.lm_head_confidence: conf within 2e-3,
+argmax / commit / tokens bit-exact wherever the top-2 probability gap exceeds 1e-3 and |conf - tau| > 4e-3
+(BASELINE north_star; the logits are fp32-accumulated on the GPU, fp64 in the oracle)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from paper_2606_08411_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def handle():
+    from paper_2606_08411_b200 import binding
+    h = binding.Handle(0)
+    yield h
+    h.close()
+
+
+def run_case(handle, N, V, K, seed, lanes=None, eos=-1, force=False, peaked=0.5, tau=0.9):
+    from paper_2606_08411_b200 import binding as B
+    from paper_2606_08411_b200.step import to_device
+    rng = np.random.default_rng(seed)
+    hidden = W.round_to_bf16(rng.standard_normal((N, K)).astype(np.float32))
+    weight = W.round_to_bf16((rng.standard_normal((V, K)) / np.sqrt(K)).astype(np.float32))      # logits ~ N(0, 1)
+    # peaked rows: the hidden state points along one token's weight row, so that token's logit dominates
+    hot = rng.integers(0, V, size=N)
+    pk = rng.random(N) < peaked
+    scale = 14.0 / np.maximum((weight[hot] ** 2).sum(1), 1e-6)
+    hidden[pk] = W.round_to_bf16((weight[hot] * scale[:, None])[pk].astype(np.float32))
+    tokens = np.where(rng.random(N) < 0.6, V - 1, 3).astype(np.int32)
+    dev = torch.device("cuda:0")
+    th, tw = to_device(hidden, "bf16", dev), to_device(weight, "bf16", dev)
+    conf = torch.zeros(N, device=dev); am = torch.zeros(N, dtype=torch.int32, device=dev)
+    cm = torch.zeros(N, dtype=torch.uint8, device=dev); to = torch.zeros(N, dtype=torch.int32, device=dev)
+    ws = torch.full((handle.al_lm_head_confidence_workspace_bytes(N, V),), 0xFF, dtype=torch.uint8, device=dev)
+    ln = None if lanes is None else torch.from_numpy(np.asarray(lanes, np.int32)).to(dev)
+    handle.al_lm_head_confidence(th, tw, N, V, K, torch.from_numpy(tokens).to(dev), V - 1, eos, tau, ln,
+                                 0 if lanes is None else len(lanes), B.AL_SELECT_FORCE_TOP1 if force else 0, conf, am, cm,
+                                 to, ws)
+    torch.cuda.synchronize()
+    ref = oracle.lm_head_confidence(hidden, weight, tokens, V - 1, eos, tau, lanes, force)
+    c = conf.cpu().numpy()
+    assert np.abs(c - ref["conf"]).max() <= 2e-3, np.abs(c - ref["conf"]).max()
+    gap_ok = (ref["conf"] - ref["p2"]) > 1e-3
+    tau_ok = np.abs(ref["conf"] - tau) > 4e-3
+    assert np.array_equal(am.cpu().numpy()[gap_ok], ref["argmax"][gap_ok])
+    sel = gap_ok & tau_ok
+    if not force:
+        assert np.array_equal(cm.cpu().numpy()[sel], ref["commit"][sel])
+        assert np.array_equal(to.cpu().numpy()[sel], ref["tokens_out"][sel])
+    else:
+        assert np.array_equal(cm.cpu().numpy(), ref["commit"]) and np.array_equal(to.cpu().numpy(), ref["tokens_out"])
+    # rows the gap rule exempts (flat rows: every probability ~ 1 / V) must still pick a token whose logit is the
+    # maximum up to the fp32 accumulation error
+    x = hidden.astype(np.float64) @ weight.astype(np.float64).T
+    if lanes is not None and eos >= 0:
+        for l in lanes:
+            if l[5] & 1:
+                x[l[3]:l[3] + l[4], eos] = -np.inf
+    got = x[np.arange(N), am.cpu().numpy()]
+    assert (got >= x.max(1) - 2e-3).all()
+    assert N < 16 or ((gap_ok.mean() >= 0.8 * peaked) and (ref["commit"].sum() > 0 or peaked == 0))
+    return ref
+
+
+def test_small_rows_ragged_everything(handle):
+    """BN = 128 path: 37 rows (one partial row tile), vocabulary and hidden size that are multiples of nothing useful"""
+    run_case(handle, 37, 5003, 200, seed=1)
+    run_case(handle, 1, 1000, 64, seed=2)
+    run_case(handle, 130, 3000, 72, seed=3)                 # two row tiles, K tail of 8
+
+
+def test_llada_shaped_few_rows(handle):
+    """the paper's operating point: one lane of 32 rows over the full LLaDA-shaped head (126464 x 4096 weights, 1 GB)"""
+    lanes = [[0, 0, 0, 0, 16, 1], [0, 0, 0, 16, 16, 0]]
+    run_case(handle, 32, W.LLADA_VOCAB, 4096, seed=4, lanes=lanes, eos=126081)
+
+
+def test_many_rows_bn256_path_with_lanes_eos_and_force_top1(handle):
+    N = 700                                                  # 6 row tiles -> 256-wide vocabulary tiles
+    lanes = [[0, 0, 0, 0, 300, 1], [0, 0, 0, 300, 400, 0]]
+    ref = run_case(handle, N, 20000, 512, seed=5, lanes=lanes, eos=77)
+    run_case(handle, N, 20000, 512, seed=6, lanes=lanes, eos=77, force=True, peaked=0.0, tau=0.999)
+
+
+def test_eos_suppression_changes_the_argmax_only_on_refine_rows(handle):
+    from paper_2606_08411_b200.step import to_device
+    V, K, N = 512, 64, 4
+    w = np.zeros((V, K), np.float32); w[np.arange(K), np.arange(K)] = 8.0          # token k <-> direction e_k
+    h = np.zeros((N, K), np.float32); h[:, 5] = 1.0; h[:, 9] = 0.5                 # logits: token 5 -> 8, token 9 -> 4
+    lanes = np.array([[0, 0, 0, 0, 2, 1], [0, 0, 0, 2, 2, 0]], np.int32)
+    dev = torch.device("cuda:0")
+    conf = torch.zeros(N, device=dev); am = torch.zeros(N, dtype=torch.int32, device=dev)
+    cm = torch.zeros(N, dtype=torch.uint8, device=dev); to = torch.zeros(N, dtype=torch.int32, device=dev)
+    ws = torch.empty(handle.al_lm_head_confidence_workspace_bytes(N, V), dtype=torch.uint8, device=dev)
+    handle.al_lm_head_confidence(to_device(h, "bf16", dev), to_device(w, "bf16", dev), N, V, K,
+                                 torch.full((N,), 511, dtype=torch.int32, device=dev), 511, 5, 0.5,
+                                 torch.from_numpy(lanes).to(dev), 2, 0, conf, am, cm, to, ws)
+    torch.cuda.synchronize()
+    assert am.cpu().tolist() == [9, 9, 5, 5]
+    ref = oracle.lm_head_confidence(h, w, np.full(N, 511, np.int32), 511, 5, 0.5, lanes)
+    assert np.abs(conf.cpu().numpy() - ref["conf"]).max() <= 2e-3 and np.array_equal(cm.cpu().numpy(), ref["commit"])
