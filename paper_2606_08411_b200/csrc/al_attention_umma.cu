@@ -446,6 +446,11 @@ constexpr bool kTmaStoreOk = false;        // debug knob: every bf16 sub-tile is
 #else
 constexpr bool kTmaStoreOk = true;
 #endif
+#ifdef AL_NO_VZERO
+#define AL_VZERO_ON 0
+#else
+#define AL_VZERO_ON 1
+#endif
 constexpr int kStagePitch = 128;           // 128 data bytes per staged row; 16-byte chunk c of row r sits at chunk c ^ (r & 7)
 
 struct AttnSmem {
@@ -925,7 +930,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
             /* rows beyond the group's longest prefix: unwritten or recycled memory).  P is exactly 0 there, */ \
             /* but 0 x NaN/Inf would still poison every row of the tile, so they are zeroed in shared memory */ \
             /* before the MMA reads them (both issuers may do it: same zeros).                               */ \
-            if (valid_ & 15) {                                                                                 \
+            if (AL_VZERO_ON && (valid_ & 15)) {                                                                 \
               const int nz_ = ksteps_ * 16 - valid_;                 /* 1..15 key rows of 128 bytes per half */ \
               for (int j_ = lane; j_ < nz_ * 16; j_ += 32) {                                                   \
                 const int row_ = valid_ + (j_ >> 4), hc_ = j_ & 15;  /* half = hc_ >> 3, 16-byte chunk hc_ & 7 */ \
