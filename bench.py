@@ -302,6 +302,94 @@ def measure_resident(h, wl, dev, stream, dist, sampler, steps, warmup, kernel_ev
                 n_copies=n_copies, per_copy=per_copy, barrier=barrier, graphs=graphs, part_graphs=part_graphs)
 
 
+def measure_next_rows(h, dev, stream, peaks):
+    """SURVEY 8(f) rows, each timed on its own (CUDA events on the stream, inputs resident): the fused LM head at the
+    LLaDA-layer and batch-16 shapes (next to the library route it replaces: cuBLAS GEMM + al_confidence_select on
+    materialised bf16 logits), al_lane_status on the batch-16 lanes, the Eq.12 refresh forward of one Dream-shaped
+    sequence, and Algorithm 1 end to end with the table-driven stub model."""
+    import numpy as np
+    import torch
+    from paper_2606_08411_b200 import binding as B, workloads as W
+    from paper_2606_08411_b200.scheduler import run_with_stub_model
+
+    def timed(fn, n):
+        with torch.cuda.stream(stream):
+            fn(); fn()
+            stream.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(n):
+                fn()
+            e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n * 1e3
+
+    out = {}
+    gen = torch.Generator(device=dev).manual_seed(1)
+    rnd = lambda *sh: torch.randn(*sh, device=dev, generator=gen)
+    for name, N, V, K in (("llada_layer_128x126464x4096", 128, W.LLADA_VOCAB, 4096),
+                          ("batch16_3264x152064x3584", 3264, W.DREAM_VOCAB, 3584)):
+        hid = rnd(N, K).bfloat16()
+        wts = [(rnd(V, K) / K ** 0.5).bfloat16() for _ in range(2)]         # two copies: 2 x 1 GB > L2
+        tok = torch.zeros(N, dtype=torch.int32, device=dev)
+        conf = torch.zeros(N, device=dev); am = torch.zeros(N, dtype=torch.int32, device=dev)
+        cm = torch.zeros(N, dtype=torch.uint8, device=dev); to = torch.zeros(N, dtype=torch.int32, device=dev)
+        ws = torch.empty(h.al_lm_head_confidence_workspace_bytes(N, V), dtype=torch.uint8, device=dev)
+        logits = torch.empty(N, V, device=dev, dtype=torch.bfloat16)
+        i = [0]
+
+        def fused():
+            i[0] += 1
+            h.al_lm_head_confidence(hid, wts[i[0] & 1], N, V, K, tok, 7, -1, 0.9, None, 0, 0, conf, am, cm, to, ws, stream)
+
+        def library():
+            i[0] += 1
+            torch.matmul(hid, wts[i[0] & 1].t(), out=logits)
+            h.al_confidence_select(logits, N, V, V, tok, 7, -1, 0.9, None, 0, 0, conf, am, cm, to, None, stream)
+
+        tf, tl = timed(fused, 10), timed(library, 10)
+        flops = 2.0 * N * V * K
+        out["lm_head_fused_" + name] = {"us": tf, "tflops": flops / tf / 1e6, "frac_of_bf16_peak": flops / tf / 1e6 / peaks["tensor"],
+                                        "weight_gbs": V * K * 2 / tf / 1e3, "frac_of_hbm_peak": V * K * 2 / tf / 1e3 / peaks["hbm"],
+                                        "library_route_us": tl, "library_route": "torch.matmul (cuBLAS) -> bf16 logits -> al_confidence_select"}
+        del wts, logits, hid
+        torch.cuda.empty_cache()
+    # lane status on the batch-16 lanes (102 lanes, 3264 rows)
+    wl_lanes = W.make_lanes(W.cfg5_lane_tree(np.random.default_rng(W.SEED_BASE + 5), 16, 1280))
+    n_l, n_r = len(wl_lanes), int(wl_lanes[:, W.LANE_Q_LEN].sum())
+    lanes_d = torch.from_numpy(wl_lanes).to(dev)
+    ti = torch.full((n_r,), 7, dtype=torch.int32, device=dev); cf = torch.rand(n_r, device=dev, generator=gen)
+    am = torch.randint(0, 100, (n_r,), dtype=torch.int32, device=dev)
+    cm = torch.zeros(n_r, dtype=torch.uint8, device=dev); to = ti.clone() + 1
+    stt = torch.zeros((n_l, 8), dtype=torch.int32, device=dev)
+    dl = torch.tensor([13, 30], dtype=torch.int32, device=dev)
+    out["lane_status_batch16"] = {"us": timed(lambda: h.al_lane_status(lanes_d, n_l, n_r, ti, cf, am, 7, 2, 0.9, dl, None, cm, to, stt, stream), 50),
+                                  "lanes": n_l, "rows": n_r}
+    # refresh forward (Eq.12) of one Dream-shaped sequence: L_refresh = 1024, 28q / 4kv heads, d = 128
+    Lr, Hq, Hkv, d = 1024, 28, 4, 128
+    shape = B.Handle.make_shape(Hq, Hkv, d, B.AL_BF16, Lr + 64)
+    q, k, v = rnd(Lr, Hq, d).bfloat16(), rnd(Lr, Hkv, d).bfloat16(), rnd(Lr, Hkv, d).bfloat16()
+    kc, vc = rnd(Hkv, Lr + 64, d).bfloat16(), rnd(Hkv, Lr + 64, d).bfloat16()
+    o = torch.zeros_like(q)
+    ln = torch.tensor([[0, 0, 0, 0, Lr, 0]], dtype=torch.int32, device=dev)
+    wsa = torch.empty(h.al_lane_attention_workspace_bytes(shape, 1, Lr, 0), dtype=torch.uint8, device=dev)
+    t_rf = timed(lambda: h.al_refresh_forward(shape, q, k, v, kc, vc, ln, 1, Lr, 0, o, None, wsa, stream), 30)
+    fl = 4.0 * Hq * d * Lr * Lr
+    out["refresh_forward_dream_1024"] = {"us": t_rf, "tflops": fl / t_rf / 1e6, "frac_of_bf16_peak": fl / t_rf / 1e6 / peaks["tensor"]}
+    # Algorithm 1 with the stub model (whole decode of 192 tokens, one synchronisation per iteration)
+    case = W.scheduler_case(37, gen_len=192)
+    t0 = time.perf_counter()
+    reps = 5
+    for _ in range(reps):
+        r = run_with_stub_model(h, case["cfg"], case["base"], case["target"], case["gain"], case["prompt"])
+    dt = (time.perf_counter() - t0) / reps
+    out["scheduler_stub_model_192"] = {"ms_per_decode": dt * 1e3, "iterations": r["stats"]["iterations"],
+                                       "us_per_iteration": dt * 1e6 / max(1, r["stats"]["iterations"]),
+                                       "decoded_tokens": int(len(r["output"])), "forks": r["stats"]["forks"],
+                                       "note": "stub model: measures the scheduler's per-iteration overhead (H2D, 4 kernels, D2H, sync), not a model"}
+    return out
+
+
 def run_ours(args, rank: int, local_rank: int, world: int):
     import gc
     import torch
@@ -339,6 +427,12 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             del m, wl_x
             gc.collect()
             torch.cuda.empty_cache()
+
+    next_rows = None
+    if args.next_rows and world == 1:
+        next_rows = measure_next_rows(h, dev, stream, peaks)
+        gc.collect()
+        torch.cuda.empty_cache()
 
     wl = W.CONFIGS[args.workload]()
     acc = accounting.summary(wl)
@@ -419,7 +513,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                        "confidence + D2H per step)",
                 "gpu_launches_per_step": e2e_launches},
         "gpu_launches": launches_per_step * args.steps,
-        "roofline": roofline, "parts": parts, "workloads": extra, "cpu_baseline": cpu,
+        "roofline": roofline, "parts": parts, "workloads": extra, "next_rows": next_rows, "cpu_baseline": cpu,
         "algorithmic": acc, "peaks": peaks,
     }
     print(json.dumps(line), flush=True)
@@ -442,6 +536,8 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-events", dest="kernel_events", action="store_false")
+    ap.add_argument("--no-next-rows", dest="next_rows", action="store_false",
+                    help="skip the SURVEY 8(f) rows (fused LM head, lane status, refresh forward, scheduler) reported under `next_rows`")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     rank = int(os.environ.get("RANK", "0"))
