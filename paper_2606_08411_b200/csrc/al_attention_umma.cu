@@ -179,12 +179,13 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   __shared__ int s_max_nk;                     // longest item, in steps
   __shared__ int s_sorted[kDealMaxTiles];      // item-list plans: tile of rank r (longest first)
   __shared__ int s_makespan;
+  __shared__ int s_tiles2;                     // tiles of the launch if every tile takes two sub-tiles
   const int tid = threadIdx.x;
   // programmatic dependent launch: the attention kernel may start its prologue (barriers, TMEM) now; it
   // waits for this grid's completion before it reads the plan
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   TRACE_P(0);
-  if (tid == 0) s_max_nk = 0;
+  if (tid == 0) { s_max_nk = 0; s_tiles2 = 0; }
 
   // runs
   for (int i = tid; i < n_lanes; i += blockDim.x) {
@@ -207,10 +208,19 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
   }
   if (tid == 0) s_run_lane0[n_runs] = n_lanes;
   __syncthreads();
-  // tiles per run
+  // tiles per run: two sub-tiles of tpt tokens per tile (they share every prefix K/V tile staged in shared memory).
+  // Few tiles (twice as many items would still leave every item a CTA of its own): ONE sub-tile per tile, so that
+  // both softmax streams of a CTA work on the same sub-tile's key tiles alternately (alt mode) and an item takes
+  // half as many steps -- latency, not L2 traffic, is what such a launch pays for (cfg3: 32 items on 148 SMs).
   for (int r = tid; r < n_runs; r += blockDim.x) {
     const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
-    s_run_tile_base[r] = ceil_div(max(0, s_qe[l1 - 1] - s_qs[l0]), 2 * tpt);
+    atomicAdd(&s_tiles2, ceil_div(max(0, s_qe[l1 - 1] - s_qs[l0]), 2 * tpt));
+  }
+  __syncthreads();
+  const int tile_tok = (s_tiles2 > 0 && 4 * s_tiles2 * n_kv_heads <= min(bounds.grid, kMaxCtas)) ? tpt : 2 * tpt;
+  for (int r = tid; r < n_runs; r += blockDim.x) {
+    const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
+    s_run_tile_base[r] = ceil_div(max(0, s_qe[l1 - 1] - s_qs[l0]), tile_tok);
   }
   __syncthreads();
   TRACE_P(3);
@@ -222,8 +232,8 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
     const int r = last_le(s_run_tile_base, n_runs, t);
     const int l0 = s_run_lane0[r], l1 = s_run_lane0[r + 1];
     TileRec T;
-    T.q_tok0 = s_qs[l0] + (t - s_run_tile_base[r]) * 2 * tpt;
-    T.n_tok = min(2 * tpt, s_qe[l1 - 1] - T.q_tok0);
+    T.q_tok0 = s_qs[l0] + (t - s_run_tile_base[r]) * tile_tok;
+    T.n_tok = min(tile_tok, s_qe[l1 - 1] - T.q_tok0);
     T.kv_base_row = s_kb[l0];
     T.kv_len_max = 0; T.kv_len_min = 0x7fffffff; T.lk0 = 0x7fffffff; T.lk1 = 0;
     T.sub_lk0[0] = T.sub_lk0[1] = 0x7fffffff; T.sub_lk1[0] = T.sub_lk1[1] = 0;
@@ -1398,7 +1408,8 @@ Bounds bounds_for(const al_attn_shape* s, int n_lanes, int total_q_rows, int n_s
   const int n_rep = s->n_q_heads / s->n_kv_heads;
   const int tpt = kBM / n_rep;
   Bounds b;
-  b.max_tiles = ceil_div(total_q_rows, 2 * tpt) + n_lanes;
+  b.max_tiles = ceil_div(total_q_rows, 2 * tpt) + n_lanes;   // (one-sub-tile plans have at most grid / (2 n_kv) tiles)
+  if (b.max_tiles < kMaxCtas) b.max_tiles = kMaxCtas;
   b.grid = n_sms < kMaxCtas ? n_sms : kMaxCtas;
   return b;
 }
