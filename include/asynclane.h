@@ -177,7 +177,8 @@ al_status al_kv_refresh(al_handle* handle, const al_attn_shape* shape, void* k_c
  *   k_cache[g][kv_base_row + prefix_len + i][:] = k_new[q_start + i][g][:]      (same for V), i in [0, q_len)
  * Eq.12's own case is prefix_len = 0, q_len = L_refresh (dense self-attention over the refreshed range); with
  * prefix_len > 0 the same call appends a finalized valid prefix (Alg.1 line 16).  The attention reads the
- * cache BEFORE these rows are written (stream order); kv_base_row + prefix_len + q_len <= cache_rows.
+ * cache BEFORE these rows are written (stream order); kv_base_row + prefix_len + q_len <= cache_rows, and
+ * the ranges of one call must write disjoint cache rows (two ranges appending to the same rows race).
  * Arguments, limits and workspace as al_lane_attention (max_prefix_len >= every prefix_len).
  */
 al_status al_refresh_forward(al_handle* handle, const al_attn_shape* shape, const void* q,

@@ -104,3 +104,53 @@ def test_eos_suppression_changes_the_argmax_only_on_refine_rows(handle):
     assert am.cpu().tolist() == [9, 9, 5, 5]
     ref = oracle.lm_head_confidence(h, w, np.full(N, 511, np.int32), 511, 5, 0.5, lanes)
     assert np.abs(conf.cpu().numpy() - ref["conf"]).max() <= 2e-3 and np.array_equal(cm.cpu().numpy(), ref["commit"])
+
+
+def test_new_calls_are_graph_capturable_and_replay_bit_identically(handle):
+    """al_lm_head_confidence, al_lane_status and al_refresh_forward only enqueue on the given stream: captured into
+    one CUDA graph and replayed, they reproduce the eager results bit for bit."""
+    from paper_2606_08411_b200 import binding as B
+    from paper_2606_08411_b200.step import to_device
+    rng = np.random.default_rng(9)
+    dev = torch.device("cuda:0")
+    N, V, K = 96, 4096, 256
+    hid = to_device(W.round_to_bf16(rng.standard_normal((N, K)).astype(np.float32)), "bf16", dev)
+    wt = to_device(W.round_to_bf16((rng.standard_normal((V, K)) / 16).astype(np.float32)), "bf16", dev)
+    lanes = torch.tensor([[0, 0, 40, 0, 48, (8 << 8)], [1, 128, 40, 48, 48, 1]], dtype=torch.int32, device=dev)
+    tok = torch.full((N,), V - 1, dtype=torch.int32, device=dev)
+    conf = torch.zeros(N, device=dev); am = torch.zeros(N, dtype=torch.int32, device=dev)
+    cm = torch.zeros(N, dtype=torch.uint8, device=dev); to = torch.zeros(N, dtype=torch.int32, device=dev)
+    ws = torch.empty(handle.al_lm_head_confidence_workspace_bytes(N, V), dtype=torch.uint8, device=dev)
+    status = torch.zeros((2, 8), dtype=torch.int32, device=dev)
+    delims = torch.tensor([5, 6], dtype=torch.int32, device=dev)
+    Hq, Hkv, d = 4, 2, 128
+    shape = B.Handle.make_shape(Hq, Hkv, d, B.AL_BF16, 256)
+    q = torch.randn(N, Hq, d, device=dev).bfloat16(); k = torch.randn(N, Hkv, d, device=dev).bfloat16()
+    v = torch.randn(N, Hkv, d, device=dev).bfloat16()
+    kc = torch.randn(Hkv, 256, d, device=dev).bfloat16(); vc = torch.randn(Hkv, 256, d, device=dev).bfloat16()
+    kc0, vc0 = kc.clone(), vc.clone()
+    out = torch.zeros_like(q)
+    wsa = torch.empty(handle.al_lane_attention_workspace_bytes(shape, 2, N, 40), dtype=torch.uint8, device=dev)
+
+    def step(s):
+        handle.al_lm_head_confidence(hid, wt, N, V, K, tok, V - 1, 3, 0.5, lanes, 2, 0, conf, am, cm, to, ws, s)
+        handle.al_lane_status(lanes, 2, N, tok, conf, am, V - 1, 3, 0.4, delims, None, cm, to, status, s)
+        handle.al_refresh_forward(shape, q, k, v, kc, vc, lanes, 2, N, 40, out, None, wsa, s)
+
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        step(s)
+    s.synchronize()
+    eager = [t.clone() for t in (conf, am, cm, to, status, out, kc, vc)]
+    kc.copy_(kc0); vc.copy_(vc0)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            step(s)
+    for t in (conf, am, cm, to, status, out):
+        t.zero_()
+    kc.copy_(kc0); vc.copy_(vc0)
+    g.replay(); torch.cuda.synchronize()
+    for a, b in zip(eager, (conf, am, cm, to, status, out, kc, vc)):
+        assert torch.equal(a, b)
