@@ -313,6 +313,7 @@ def measure_next_rows(h, dev, stream, peaks):
     from paper_2606_08411_b200.scheduler import run_with_stub_model
 
     def timed(fn, n):
+        torch.cuda.synchronize()                 # the inputs were made on the default stream: nothing else may be running
         with torch.cuda.stream(stream):
             fn(); fn()
             stream.synchronize()

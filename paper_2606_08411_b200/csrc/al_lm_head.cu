@@ -15,6 +15,10 @@
 //     running at the same time share weight tiles through L2; a unit leaves one (m, s, idx) per row in the workspace
 //     and lm_head_select_kernel merges a row's chunks in vocabulary order (first maximiser wins) and applies the
 //     commit rule.  BN = 128 for few rows (the weight stream is HBM-bound and small tiles balance the SMs), 256 else.
+//     Few rows, kCluster = 2: every CTA would re-read the same hidden tile for each of its vocabulary tiles (L2 -> SM
+//     traffic twice the weight stream), so the two CTAs of a cluster take alternate vocabulary tiles of one unit and
+//     each loads HALF of the hidden tile with TMA multicast into both; a stage is reused once BOTH issuers'
+//     tcgen05.commit (multicast to both CTAs' barriers) have released it.
 #include <cuda_bf16.h>
 
 #include "al_internal.h"
@@ -45,6 +49,7 @@ template <int BN> struct LmSmem {
 struct LmParams {
   int n_rows, vocab, hidden_dim;
   int m_tiles, n_tiles, n_chunks;          // unit u = chunk * m_tiles + m_tile; chunk j = vocabulary tiles [j n_tiles / n_chunks, ...)
+                                           // (cluster of 2: a unit is a PAIR of chunks 2j, 2j+1 taking alternate tiles of the pair's range)
   int eos_id, n_lanes;
   const al_lane_desc* lanes;
   float4* parts;                           // [n_chunks][m_tiles * 128]  (m, s, idx bits, unused)
@@ -56,16 +61,44 @@ __device__ __forceinline__ float ex2f(float x) {
   return y;
 }
 
-template <int BN>
+// The vocabulary tiles [t0, t0 + step * count) one CTA takes of unit u: the whole chunk (no cluster), or every second
+// tile of the pair's range starting at its rank (cluster of 2; the range is rounded up to an even number of tiles --
+// tiles beyond the vocabulary are loaded as zeros and masked in the epilogue -- so that both ranks run equally long).
+template <int kCluster>
+__device__ __forceinline__ void unit_tiles(const LmParams& p, int u, int rank, int& chunk, int& mt, int& t0, int& count, int& step,
+                                           int& t_end) {
+  const int group = u / p.m_tiles;                         // chunk (no cluster) or pair of chunks
+  mt = u - group * p.m_tiles;
+  if (kCluster == 1) {
+    chunk = group;
+    t0 = (int)((long long)group * p.n_tiles / p.n_chunks);
+    t_end = (int)((long long)(group + 1) * p.n_tiles / p.n_chunks);
+    count = t_end - t0;
+    step = 1;
+  } else {
+    const int n_pairs = p.n_chunks / 2;
+    const int a = (int)((long long)group * p.n_tiles / n_pairs), b = (int)((long long)(group + 1) * p.n_tiles / n_pairs);
+    chunk = 2 * group + rank;
+    t0 = a + rank;
+    count = (b - a + 1) / 2;
+    step = 2;
+    t_end = b;                                             // rank 1's last tile of an odd range is the next unit's: masked
+  }
+}
+
+template <int BN, int kCluster>
 __global__ void __launch_bounds__(kThreads, 1)
 lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, const LmParams p) {
   using C = Cfg<BN>;
+  const int rank = kCluster > 1 ? (int)cluster_ctarank() : 0;
+  const int cta = kCluster > 1 ? (int)blockIdx.x / kCluster : (int)blockIdx.x;      // cluster (or CTA) index
+  const int n_ctas = (int)gridDim.x / kCluster;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   LmSmem<BN>& sm = *reinterpret_cast<LmSmem<BN>*>(smem_raw);
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) __trap();
-    for (int s = 0; s < C::kStages; ++s) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], 1); }
+    for (int s = 0; s < C::kStages; ++s) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kCluster); }
     for (int a = 0; a < 2; ++a) { mbar_init(&sm.acc_full[a], 1); mbar_init(&sm.acc_empty[a], 128); }
     fence_barrier_init();
     prefetch_tensormap(&map_a); prefetch_tensormap(&map_b);
@@ -75,24 +108,30 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   tc_fence_before();
   __syncthreads();
+  if (kCluster > 1) cluster_sync_all();                    // the peer's barriers are initialised before anything arrives on them
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   const int k_steps = (p.hidden_dim + kBK - 1) / kBK;
-  const int n_units = p.m_tiles * p.n_chunks;
+  const int n_units = p.m_tiles * (p.n_chunks / kCluster);
 
   if (warp == 0 && lane == 0) {
     // ===================== TMA producer =====================
     uint32_t it = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const int chunk = u / p.m_tiles, mt = u - chunk * p.m_tiles;
-      const int nt0 = (int)((long long)chunk * p.n_tiles / p.n_chunks), nt1 = (int)((long long)(chunk + 1) * p.n_tiles / p.n_chunks);
-      for (int nt = nt0; nt < nt1; ++nt)
+    for (int u = cta; u < n_units; u += n_ctas) {
+      int chunk, mt, t0, count, step, t_end;
+      unit_tiles<kCluster>(p, u, rank, chunk, mt, t0, count, step, t_end);
+      for (int j = 0; j < count; ++j)
         for (int kb = 0; kb < k_steps; ++kb, ++it) {
           const int s = it % C::kStages;
-          mbar_wait_relaxed(&sm.empty[s], ((it / C::kStages) & 1) ^ 1);
+          mbar_wait_relaxed(&sm.empty[s], ((it / C::kStages) & 1) ^ 1);      // released by every CTA of the cluster
           mbar_arrive_expect_tx(&sm.full[s], C::kABytes + C::kBBytes);
-          tma_load_2d(sm.a[s], &map_a, &sm.full[s], kb * kBK, mt * kBM);
-          tma_load_2d(sm.b[s], &map_b, &sm.full[s], kb * kBK, nt * BN);
+          if (kCluster == 1) {
+            tma_load_2d(sm.a[s], &map_a, &sm.full[s], kb * kBK, mt * kBM);
+          } else {                                                           // my half of the hidden tile, into both CTAs
+            tma_load_2d_multicast(sm.a[s] + rank * (C::kABytes / 2), &map_a, &sm.full[s], kb * kBK,
+                                  mt * kBM + rank * (kBM / 2), (uint16_t)0x3);
+          }
+          tma_load_2d(sm.b[s], &map_b, &sm.full[s], kb * kBK, (t0 + j * step) * BN);
         }
     }
   } else if (warp == 1) {
@@ -102,10 +141,10 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
     const uint64_t da0 = make_desc_sw128(smem_u32(sm.a[0]), 16, 1024);
     const uint64_t db0 = make_desc_sw128(smem_u32(sm.b[0]), 16, 1024);
     uint32_t it = 0, tile = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const int chunk = u / p.m_tiles;
-      const int nt0 = (int)((long long)chunk * p.n_tiles / p.n_chunks), nt1 = (int)((long long)(chunk + 1) * p.n_tiles / p.n_chunks);
-      for (int nt = nt0; nt < nt1; ++nt, ++tile) {
+    for (int u = cta; u < n_units; u += n_ctas) {
+      int chunk, mt, t0, count, step, t_end;
+      unit_tiles<kCluster>(p, u, rank, chunk, mt, t0, count, step, t_end);
+      for (int j = 0; j < count; ++j, ++tile) {
         const uint32_t acc = tile & 1;
         mbar_wait(&sm.acc_empty[acc], ((tile >> 1) & 1) ^ 1);            // the epilogue has read this accumulator
         tc_fence_after();
@@ -118,7 +157,10 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
 #pragma unroll
           for (int k = 0; k < kBK / 16; ++k)
             if (leader) mma_ss(d, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (kb | k) ? 1u : 0u);
-          if (leader) mma_commit(&sm.empty[s]);
+          if (leader) {
+            if (kCluster == 1) mma_commit(&sm.empty[s]);
+            else mma_commit_multicast(&sm.empty[s], (uint16_t)0x3);      // the stage holds a half the peer loaded: both release it
+          }
         }
         if (leader) mma_commit(&sm.acc_full[acc]);
       }
@@ -129,9 +171,9 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
     const int r = quad * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
     uint32_t tile = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const int chunk = u / p.m_tiles, mt = u - chunk * p.m_tiles;
-      const int nt0 = (int)((long long)chunk * p.n_tiles / p.n_chunks), nt1 = (int)((long long)(chunk + 1) * p.n_tiles / p.n_chunks);
+    for (int u = cta; u < n_units; u += n_ctas) {
+      int chunk, mt, t0, count, step, t_end;
+      unit_tiles<kCluster>(p, u, rank, chunk, mt, t0, count, step, t_end);
       const int row = mt * kBM + r;
       int sup = -1;                                        // EOS suppressed on rows of refine lanes
       if (p.eos_id >= 0 && p.lanes)
@@ -141,7 +183,8 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
         }
       float m = -INFINITY, s = 0.f;
       int idx = kNoIdx;
-      for (int nt = nt0; nt < nt1; ++nt, ++tile) {
+      for (int j = 0; j < count; ++j, ++tile) {
+        const int nt = t0 + j * step;
         const uint32_t acc = tile & 1;
         mbar_wait(&sm.acc_full[acc], (tile >> 1) & 1);
         tc_fence_after();
@@ -155,7 +198,7 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
 #pragma unroll
           for (int e = 0; e < 32; ++e) {
             const int v = v0 + e;
-            x[e] = (v < p.vocab && v != sup) ? __uint_as_float(raw[e]) : -INFINITY;   // vocabulary tail, EOS
+            x[e] = (v < p.vocab && v != sup && nt < t_end) ? __uint_as_float(raw[e]) : -INFINITY;   // vocabulary tail, EOS, padding tile
           }
           float cm = x[0];
 #pragma unroll
@@ -185,6 +228,7 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
   }
   tc_fence_before();
   __syncthreads();
+  if (kCluster > 1) cluster_sync_all();                    // no CTA leaves while its peer may still write into it
   if (warp == 1) { __syncwarp(); tmem_dealloc<512>(tmem); }
 }
 
@@ -202,11 +246,13 @@ lm_head_select_kernel(const float4* __restrict__ parts, int n_chunks, int rows_p
   int idx = kNoIdx;
   for (int j = 0; j < n_chunks; ++j) {
     const float4 q = parts[(long long)j * rows_padded + row];
+    const int qi = __float_as_int(q.z);
     if (q.x > m) {
       s = s * ex2f((m - q.x) * kLog2e) + q.y;
-      m = q.x; idx = __float_as_int(q.z);
+      m = q.x; idx = qi;
     } else if (q.x > -INFINITY) {
       s += q.y * ex2f((q.x - m) * kLog2e);
+      if (q.x == m && qi < idx) idx = qi;                 // the chunks of a cluster pair interleave: lowest index wins
     }
   }
   const float conf = 1.0f / s;
@@ -219,50 +265,58 @@ lm_head_select_kernel(const float4* __restrict__ parts, int n_chunks, int rows_p
 }
 
 struct LmPlan {
-  int bn, m_tiles, n_tiles, n_chunks;
+  int bn, cluster, m_tiles, n_tiles, n_chunks;
   size_t ws_bytes;
 };
 LmPlan lm_plan(int n_rows, int vocab, int sm_count) {
   LmPlan L;
   L.m_tiles = (n_rows + kBM - 1) / kBM;
-  // few rows: the weight stream is HBM-bound and what matters is equal bytes per SM -> small vocabulary tiles
+  // few rows: the weight stream is HBM-bound and what matters is equal bytes per SM -> small vocabulary tiles, and the
+  // hidden tile shared by the two CTAs of a cluster (TMA multicast)
   L.bn = L.m_tiles <= 4 ? 128 : 256;
+  L.cluster = L.m_tiles <= 4 ? 2 : 1;
   L.n_tiles = (vocab + L.bn - 1) / L.bn;
-  // chunks: units = chunks * m_tiles should fill whole waves of the SMs (a last wave of a few units would leave the
-  // others idle for a whole unit) while a unit keeps at least 4 vocabulary tiles; the coarsest plan within 2 % of
-  // the best fill wins (fewer partials, longer register-resident runs)
-  const int max_chunks = L.n_tiles >= 4 ? L.n_tiles / 4 : 1;
-  auto fill_of = [&](int ch) {
-    const long long units = (long long)ch * L.m_tiles;
-    const long long waves = (units + sm_count - 1) / sm_count;
-    return (double)units / (double)(waves * sm_count);
+  const int slots = sm_count / L.cluster;                  // CTAs, or clusters, that run at the same time
+  // groups (chunks, or pairs of chunks): units = groups * m_tiles should fill whole waves of the slots (a last wave of
+  // a few units would leave the others idle for a whole unit) while a CTA keeps at least 4 vocabulary tiles per unit;
+  // the coarsest plan within 2 % of the best fill wins (fewer partials, longer register-resident runs)
+  const int max_groups = L.n_tiles >= 4 * L.cluster ? L.n_tiles / (4 * L.cluster) : 1;
+  auto fill_of = [&](int g) {
+    const long long units = (long long)g * L.m_tiles;
+    const long long waves = (units + slots - 1) / slots;
+    return (double)units / (double)(waves * slots);
   };
   double best = 0.0;
-  for (int ch = 1; ch <= max_chunks; ++ch) best = fill_of(ch) > best ? fill_of(ch) : best;
-  long long chunks = 1;
-  for (int ch = 1; ch <= max_chunks; ++ch)
-    if (fill_of(ch) >= best - 0.02) { chunks = ch; break; }
-  L.n_chunks = (int)chunks;
+  for (int g = 1; g <= max_groups; ++g) best = fill_of(g) > best ? fill_of(g) : best;
+  long long groups = 1;
+  for (int g = 1; g <= max_groups; ++g)
+    if (fill_of(g) >= best - 0.02) { groups = g; break; }
+  L.n_chunks = (int)groups * L.cluster;
   L.ws_bytes = (size_t)L.n_chunks * L.m_tiles * kBM * sizeof(float4);
   return L;
 }
 
-template <int BN>
+template <int BN, int kCluster>
 al_status launch_lm_head(const al_handle* h, const CUtensorMap& ma, const CUtensorMap& mb, const LmParams& p, int n_units,
                          cudaStream_t cs) {
   const size_t smem = sizeof(LmSmem<BN>);
-  AL_CUDA_OK(cudaFuncSetAttribute(lm_head_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  AL_CUDA_OK(cudaFuncSetAttribute(lm_head_kernel<BN, kCluster>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int slots = h->sm_count / kCluster;
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3((unsigned)(n_units < h->sm_count ? n_units : h->sm_count));
+  cfg.gridDim = dim3((unsigned)((n_units < slots ? n_units : slots) * kCluster));
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = cs;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = kCluster;
+  attr[1].val.clusterDim.y = 1;
+  attr[1].val.clusterDim.z = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lm_head_kernel<BN>, ma, mb, p));
+  cfg.numAttrs = kCluster > 1 ? 2 : 1;
+  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lm_head_kernel<BN, kCluster>, ma, mb, p));
   return AL_OK;
 }
 
@@ -307,7 +361,8 @@ extern "C" al_status al_lm_head_confidence(al_handle* h, const void* hidden, con
   if (!workspace || !al_aligned16(workspace) || workspace_bytes < L.ws_bytes)
     AL_FAIL(AL_ERR_WORKSPACE, "%s: workspace %zu < %zu (or unaligned)", who, workspace_bytes, L.ws_bytes);
   CUtensorMap ma, mb;
-  if ((st = al_make_map_2d(h, &ma, hidden, (uint64_t)n_rows, (uint64_t)hidden_dim, kBM)) != AL_OK) return st;
+  // (a cluster of 2 loads the hidden tile as two 64-row halves, one per CTA, multicast to both)
+  if ((st = al_make_map_2d(h, &ma, hidden, (uint64_t)n_rows, (uint64_t)hidden_dim, (uint32_t)(kBM / L.cluster))) != AL_OK) return st;
   if ((st = al_make_map_2d(h, &mb, weight, (uint64_t)vocab, (uint64_t)hidden_dim, (uint32_t)L.bn)) != AL_OK) return st;
   LmParams p;
   p.n_rows = n_rows; p.vocab = vocab; p.hidden_dim = hidden_dim;
@@ -315,8 +370,8 @@ extern "C" al_status al_lm_head_confidence(al_handle* h, const void* hidden, con
   p.eos_id = eos_id; p.n_lanes = n_lanes; p.lanes = n_lanes > 0 ? lanes : nullptr;
   p.parts = static_cast<float4*>(workspace);
   cudaStream_t cs = static_cast<cudaStream_t>(stream);
-  const int n_units = L.m_tiles * L.n_chunks;
-  st = L.bn == 128 ? launch_lm_head<128>(h, ma, mb, p, n_units, cs) : launch_lm_head<256>(h, ma, mb, p, n_units, cs);
+  const int n_units = L.m_tiles * (L.n_chunks / L.cluster);
+  st = L.cluster == 2 ? launch_lm_head<128, 2>(h, ma, mb, p, n_units, cs) : launch_lm_head<256, 1>(h, ma, mb, p, n_units, cs);
   if (st != AL_OK) return st;
   h->launches++;
   cudaLaunchConfig_t cfg{};
