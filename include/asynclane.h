@@ -136,7 +136,14 @@ al_status al_lane_attention(al_handle* handle, const al_attn_shape* shape, const
  * model once per group (Eq.11) and every layer of that call sees the same lanes.
  *   al_lane_plan               builds the decomposition from lanes_dev into `workspace` (one small launch)
  *   al_lane_attention_planned  runs the attention of one layer from a workspace al_lane_plan filled
- *                              with the SAME shape, lanes_dev contents, n_lanes and total_q_rows
+ *                              with the SAME shape, lanes_dev contents, n_lanes, total_q_rows and
+ *                              max_prefix_len
+ * Small calls need no plan launch at all: with at most 32 lanes, (ceil(total_q_rows / floor(128 / n_rep)) +
+ * n_lanes - 1) * H_kv <= SMs and ceil(max_prefix_len / 64) + ceil(total_q_rows / 64) <= 24, every CTA of the
+ * attention kernel derives its own work from lanes_dev in its prologue (the same decomposition the plan
+ * launch would write); al_lane_plan then enqueues nothing and leaves the workspace untouched.  The rule
+ * depends on the host-side bounds only, which is why the planned call must be given the same ones.  (A
+ * handle created while the environment holds ASYNCLANE_SELF_PLAN=0 always launches the plan.)
  * al_lane_attention == al_lane_plan followed by al_lane_attention_planned.  The planned call leaves
  * the plan intact, so it may be repeated (other layers, other q/k/v/cache/out pointers) on the same
  * stream.  For shapes the tensor-core path does not cover (fp32, head_dim != 128) there is no plan:

@@ -1,6 +1,7 @@
 // Handle life cycle, error reporting, descriptor validation and the attention dispatch of
 // libasynclane (C ABI in include/asynclane.h).
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -45,6 +46,8 @@ extern "C" al_status al_create(al_handle** out, int device) {
   h->cc_minor = p.minor;
   h->smem_optin = p.sharedMemPerBlockOptin;
   h->encode_tiled = reinterpret_cast<decltype(h->encode_tiled)>(fn);
+  const char* sp = getenv("ASYNCLANE_SELF_PLAN");   // "0": small attention calls use the plan kernel too (tests compare the two)
+  h->self_plan = !(sp && sp[0] == '0');
   *out = h;
   return AL_OK;
 }
@@ -121,7 +124,7 @@ al_status al_lane_attention_impl(int mode, const char* who, al_handle* h, const 
       AL_FAIL(AL_ERR_WORKSPACE, "%s: workspace %zu < %zu", who, workspace_bytes, need);
     if ((st = al_attention_umma_check(h, s, n_lanes, total_q_rows)) != AL_OK) return st;
     if (mode & 1) {
-      st = al_launch_plan_umma(h, s, lanes, n_lanes, total_q_rows, workspace, workspace_bytes, cs);
+      st = al_launch_plan_umma(h, s, lanes, n_lanes, total_q_rows, max_prefix_len, workspace, workspace_bytes, cs);
       if (st != AL_OK) return st;
     }
     if (mode & 2)

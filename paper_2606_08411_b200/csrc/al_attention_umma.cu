@@ -489,6 +489,7 @@ struct AttnParams {
   int n_q_heads, n_kv_heads, n_rep, tpt;
   uint32_t q_box_bytes;                    // bytes of ONE sub-tile's Q box (both halves)
   float scale_log2;
+  int n_lanes;
 };
 
 // One CTA's walk over its work: pieces (tile, g, [kt_begin, kt_end)).  Step-range plans: the CTA's range
@@ -1351,6 +1352,94 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// self-planned launches: no plan kernel in front of the attention
+// ---------------------------------------------------------------------------------------------
+// Small calls (at most 32 lanes; by the host's bounds every item has a CTA of its own and no item is long
+// enough for the plan kernel to cut it -- self_plan_ok below) take the whole-item plan whatever the descriptors hold,
+// and CTA c = item (tile c / n_kv, kv-head c % n_kv) needs nothing but its own tile.  One warp derives it
+// from the lane descriptors in the prologue, one lane per thread: the arithmetic of lane_plan_kernel's
+// whole-item branch (runs -> tiles per run -> the tile's lanes) with ballots and warp reductions in place
+// of the block scans.  It costs the one global read the record load would cost, and the 5-6 us plan launch
+// that such a call cannot hide behind anything goes away.
+__device__ __noinline__ void self_plan_record(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv, int tpt,
+                                              int grid, int cta, CtaRec* out) {
+  const unsigned full = 0xffffffffu;
+  const int i = threadIdx.x & 31;
+  const bool has = i < n_lanes;
+  int grp = 0, kb = 0, pl = 0, qs = 0, ql = 0;
+  if (has) {
+    const int2* d = reinterpret_cast<const int2*>(lanes + i);
+    const int2 a = __ldcg(d), b = __ldcg(d + 1), c = __ldcg(d + 2);
+    grp = a.x; kb = a.y; pl = b.x; qs = b.y; ql = c.x;
+  }
+  const int qe = qs + ql;
+  const int p_grp = __shfl_up_sync(full, grp, 1), p_kb = __shfl_up_sync(full, kb, 1), p_qe = __shfl_up_sync(full, qe, 1);
+  const bool start = has && (i == 0 || !(p_grp == grp && p_kb == kb && p_qe == qs));
+  const unsigned starts = __ballot_sync(full, start);
+  // the run of lane i: [l0, l1) = [last start at or below i, next start above i)
+  const unsigned upto = (2u << i) - 1u;
+  const int l0 = has ? 31 - __clz(starts & upto) : 0;
+  const unsigned above = starts & ~upto;
+  const int l1 = has ? (above ? __ffs(above) - 1 : n_lanes) : 1;
+  const int run_q1 = __shfl_sync(full, qe, l1 - 1);
+  const int span = start ? max(0, run_q1 - qs) : 0;
+  (void)l0;
+  const int tiles2 = __reduce_add_sync(full, start ? ceil_div(span, 2 * tpt) : 0);
+  const int tile_tok = (tiles2 > 0 && 4 * tiles2 * n_kv <= grid) ? tpt : 2 * tpt;   // as lane_plan_kernel
+  const int my_tiles = start ? ceil_div(span, tile_tok) : 0;
+  int incl = my_tiles;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const int y = __shfl_up_sync(full, incl, off);
+    if (i >= off) incl += y;
+  }
+  const int base = incl - my_tiles, n_tiles = __shfl_sync(full, incl, 31);
+  const int t = cta / n_kv, g = cta - t * n_kv;
+  CtaRec C{};
+  C.first_c0 = C.first_c1 = C.last_c0 = C.last_c1 = cta;
+  C.pad = cta;
+  C.flags = kCtaAlt;                                         // idle unless the CTA has a tile
+  if (t < n_tiles) {                                         // warp-uniform
+    const unsigned owner = __ballot_sync(full, start && base <= t && t < base + my_tiles);
+    const int o = __ffs(owner) - 1;                          // first lane of the run that holds tile t
+    const int r_l1 = __shfl_sync(full, l1, o), r_base = __shfl_sync(full, base, o);
+    const int r_q0 = __shfl_sync(full, qs, o), r_q1 = __shfl_sync(full, run_q1, o), r_kb = __shfl_sync(full, kb, o);
+    TileRec T;
+    T.q_tok0 = r_q0 + (t - r_base) * tile_tok;
+    T.n_tok = min(tile_tok, r_q1 - T.q_tok0);
+    T.kv_base_row = r_kb;
+    const int end = T.q_tok0 + T.n_tok;
+    const bool in_run = has && i >= o && i < r_l1;
+    const int lf = 31 - __clz(__ballot_sync(full, in_run && qs <= T.q_tok0));   // lane that holds the tile's first token
+    const bool member = in_run && i >= lf && qs < end;
+    T.lane_first = lf; T.lane_count = __popc(__ballot_sync(full, member));
+    T.kv_len_max = __reduce_max_sync(full, member ? pl : 0);
+    T.kv_len_min = __reduce_min_sync(full, member ? pl : 0x7fffffff);
+    T.lk0 = __reduce_min_sync(full, member ? qs : 0x7fffffff);
+    T.lk1 = __reduce_max_sync(full, member ? qe : 0);
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const int t0 = T.q_tok0 + b * tpt, t1 = min(t0 + tpt, end);
+      const bool hit = member && qs < t1 && qe > t0;
+      T.sub_lk0[b] = __reduce_min_sync(full, hit ? qs : 0x7fffffff);
+      T.sub_lk1[b] = __reduce_max_sync(full, hit ? qe : 0);
+    }
+    T.n_pref_tiles = ceil_div(T.kv_len_max, kBN);
+    T.n_key_tiles = T.n_pref_tiles + ceil_div(T.lk1 - T.lk0, kBN);
+    T.kt_off = 0;                                            // the CTA's steps are counted from its own tile
+    C.f_begin = g * T.n_key_tiles; C.f_end = C.f_begin + T.n_key_tiles;
+    C.tile0 = t;
+    C.flags = kCtaActive | kCtaAlt;
+    C.first = T;
+  }
+  if (i == 0) *out = C;
+}
+
+// kSelfPlan: the launch has no plan (self_plan_record); such CTAs always hold one whole item, so only the
+// whole-item instance of the roles is compiled in.  Two kernels rather than a switch in one: the plan-reading
+// instance keeps the code it had (its schedule is sensitive to anything added around it).
+template <bool kSelfPlan>
 __global__ void __launch_bounds__(kThreads, 1)
 lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_knew,
                            const __grid_constant__ CUtensorMap map_vnew, const __grid_constant__ CUtensorMap map_kc,
@@ -1385,15 +1474,19 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   // the CTA's plan record: the one global read on the way to the first TMA load, in flight under the TMEM
   // allocation and the barrier initialisation of the other warps
-  if (warp == 2 && lane < (int)(sizeof(CtaRec) / 16))
-    reinterpret_cast<uint4*>(&sm.cta)[lane] = __ldcg(reinterpret_cast<const uint4*>(p.plan.ctas + blockIdx.x) + lane);
+  if constexpr (kSelfPlan) {
+    if (warp == 2) self_plan_record(p.lanes, p.n_lanes, p.n_kv_heads, p.tpt, (int)gridDim.x, (int)blockIdx.x, &sm.cta);
+  } else {
+    if (warp == 2 && lane < (int)(sizeof(CtaRec) / 16))
+      reinterpret_cast<uint4*>(&sm.cta)[lane] = __ldcg(reinterpret_cast<const uint4*>(p.plan.ctas + blockIdx.x) + lane);
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   // TMEM columns: S of stream b at 64 b; P of stream b, buffer u at 128 + 64 b + 32 u; O of stream b at 256 + 128 b
-  if (sm.cta.flags & kCtaAlt) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
-  else attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
+  if (kSelfPlan || (sm.cta.flags & kCtaAlt)) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
+  else if constexpr (!kSelfPlan) attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
   tc_fence_before();
   __syncthreads();
   if (threadIdx.x == 0) TRACE(13);
@@ -1412,6 +1505,22 @@ Bounds bounds_for(const al_attn_shape* s, int n_lanes, int total_q_rows, int n_s
   if (b.max_tiles < kMaxCtas) b.max_tiles = kMaxCtas;
   b.grid = n_sms < kMaxCtas ? n_sms : kMaxCtas;
   return b;
+}
+
+// Calls whose plan every CTA can derive for itself (self_plan_record): one lane per thread of a warp; every
+// item a CTA of its own even if every lane were a run of its own and every tile took one sub-tile; and no
+// item longer than kSelfPlanMaxSteps key tiles, for which lane_plan_kernel takes the whole-item plan whatever
+// the descriptors hold (s_max_nk <= kMinPiece + kSplitCost) -- so the self-planned record IS the plan kernel's.
+// Decided from the host's bounds alone: al_lane_plan and al_lane_attention_planned, given the same bounds,
+// agree without talking to each other.
+constexpr int kSelfPlanMaxSteps = kMinPiece + kSplitCost;
+bool self_plan_ok(const al_handle* h, const al_attn_shape* s, int n_lanes, int total_q_rows, int max_prefix_len,
+                  const Bounds& b) {
+  if (!h->self_plan || n_lanes > 32) return false;
+  const int tpt = kBM / (s->n_q_heads / s->n_kv_heads);
+  const long long tiles = (long long)ceil_div(total_q_rows, tpt) + n_lanes - 1;
+  if (tiles * s->n_kv_heads > b.grid) return false;
+  return ceil_div(max_prefix_len, kBN) + ceil_div(total_q_rows, kBN) <= kSelfPlanMaxSteps;
 }
 
 struct WsLayout {
@@ -1490,7 +1599,8 @@ size_t al_attention_umma_workspace_bytes(const al_handle* h, const al_attn_shape
 }
 
 al_status al_launch_plan_umma(const al_handle* h, const al_attn_shape* s, const al_lane_desc* lanes, int n_lanes,
-                              int total_q_rows, void* workspace, size_t workspace_bytes, cudaStream_t st) {
+                              int total_q_rows, int max_prefix_len, void* workspace, size_t workspace_bytes,
+                              cudaStream_t st) {
   const int n_rep = s->n_q_heads / s->n_kv_heads;
   const int tpt = kBM / n_rep;
   const Bounds b = bounds_for(s, n_lanes, total_q_rows, h->sm_count);
@@ -1498,6 +1608,7 @@ al_status al_launch_plan_umma(const al_handle* h, const al_attn_shape* s, const 
   if (rc != AL_OK) return rc;
   const WsLayout L = ws_layout(s, b);
   if (workspace_bytes < L.total) AL_FAIL(AL_ERR_WORKSPACE, "al_lane_plan: workspace %zu < %zu", workspace_bytes, L.total);
+  if (self_plan_ok(h, s, n_lanes, total_q_rows, max_prefix_len, b)) return AL_OK;   // the attention CTAs plan for themselves
   lane_plan_kernel<<<1, kPlanThreads, 0, st>>>(lanes, n_lanes, s->n_kv_heads, tpt, b, plan_in(workspace, L));
   AL_CUDA_OK(cudaGetLastError());
   h->launches += 1;
@@ -1508,7 +1619,6 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
                                    const void* k_new, const void* v_new, const void* k_cache, const void* v_cache,
                                    const al_lane_desc* lanes, int n_lanes, int total_q_rows, int max_prefix_len,
                                    void* out, float* lse, void* workspace, size_t workspace_bytes, cudaStream_t st) {
-  (void)max_prefix_len;
   const int n_rep = s->n_q_heads / s->n_kv_heads;
   const int tpt = kBM / n_rep;
   const Bounds b = bounds_for(s, n_lanes, total_q_rows, h->sm_count);
@@ -1536,9 +1646,12 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   p.lanes = lanes; p.plan = plan_in(workspace, L); p.out = static_cast<__nv_bfloat16*>(out); p.lse = lse;
   p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_rep = n_rep; p.tpt = tpt;
   p.scale_log2 = scale * kLog2e;
+  p.n_lanes = n_lanes;
+  const bool self_plan = self_plan_ok(h, s, n_lanes, total_q_rows, max_prefix_len, b);
   p.q_box_bytes = (uint32_t)(2 * tpt * n_rep * 64 * 2);
   const size_t smem = sizeof(AttnSmem);
-  AL_CUDA_OK(cudaFuncSetAttribute(lane_attention_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  AL_CUDA_OK(cudaFuncSetAttribute(lane_attention_umma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  AL_CUDA_OK(cudaFuncSetAttribute(lane_attention_umma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3((unsigned)b.grid);
   cfg.blockDim = dim3(kThreads);
@@ -1549,7 +1662,8 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lane_attention_umma_kernel, mq, mkn, mvn, mkc, mvc, mo, p));
+  if (self_plan) AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lane_attention_umma_kernel<true>, mq, mkn, mvn, mkc, mvc, mo, p));
+  else AL_CUDA_OK(cudaLaunchKernelEx(&cfg, lane_attention_umma_kernel<false>, mq, mkn, mvn, mkc, mvc, mo, p));
   h->launches += 1;
   return AL_OK;
 }

@@ -16,6 +16,7 @@ struct al_handle {
   int cc_major, cc_minor;
   size_t smem_optin;
   mutable std::atomic<uint64_t> launches{0};   // kernels enqueued through this handle
+  bool self_plan = true;   // small attention calls plan inside the attention kernel (ASYNCLANE_SELF_PLAN=0 at al_create: always the plan kernel)
   // cuTensorMapEncodeTiled resolved through the runtime (no -lcuda at link time)
   CUresult (*encode_tiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                            const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
@@ -60,8 +61,8 @@ al_status al_launch_attention_umma(const al_handle* h, const al_attn_shape* s, f
                                    int max_prefix_len, void* out, float* lse, void* workspace,
                                    size_t workspace_bytes, cudaStream_t st);
 al_status al_launch_plan_umma(const al_handle* h, const al_attn_shape* s, const al_lane_desc* lanes,
-                              int n_lanes, int total_q_rows, void* workspace, size_t workspace_bytes,
-                              cudaStream_t st);
+                              int n_lanes, int total_q_rows, int max_prefix_len, void* workspace,
+                              size_t workspace_bytes, cudaStream_t st);
 bool al_attention_umma_supported(const al_attn_shape* s);
 // limits of the tensor-core path's plan (lanes, query tiles); AL_OK when the call fits
 al_status al_attention_umma_check(const al_handle* h, const al_attn_shape* s, int n_lanes, int total_q_rows);
