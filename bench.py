@@ -215,6 +215,8 @@ def part_rooflines(wl, acc, part_ms, step_ms, peaks, traffic):
                                unit="GB/s", ms=tc * 1e3, launches=1)
     for k, p in parts.items():
         p["frac"] = p["achieved"] / p["peak"]
+        if p["bound"] == "hbm" and p["frac"] > 1.0:      # the measured peak is a COPY (read + write); a read-only stream can pass it
+            p["note"] = "read-only stream above the measured copy bandwidth (read+write figure)"
         p["traffic"] = traffic.get(k)
         p["share_of_step"] = p["ms"] / step_ms
     return parts
@@ -423,7 +425,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                 "step_us": m["step_ms"] * 1e3, "query_tok_per_s": acc_x["query_tokens"] / (m["step_ms"] * 1e-3),
                 "steps": min(args.steps, args.extra_steps), "layers": wl_x.n_layers, "query_rows": wl_x.total_q_rows,
                 "copies": m["n_copies"], "gpu_launches_per_step": m["launches_per_step"],
-                "parts": {k: {kk: p[kk] for kk in ("bound", "ms", "achieved", "peak", "unit", "frac", "traffic")}
+                "parts": {k: {kk: p[kk] for kk in ("bound", "ms", "achieved", "peak", "unit", "frac", "traffic", "note") if kk in p}
                           for k, p in parts_x.items()}}
             del m, wl_x
             gc.collect()
@@ -483,7 +485,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     if part_ms:
         parts = part_rooflines(wl, acc, part_ms, step_ms, peaks, load_traffic(wl.name))
         dom = max(parts, key=lambda k: parts[k]["ms"])
-        roofline = {k: parts[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")}
+        roofline = {k: parts[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "note") if k in parts[dom]}
         roofline.update(kernel=dom, peak_source=peaks["source"], avg_launch_ms=parts[dom]["ms"] / parts[dom]["launches"],
                         timed_with="CUDA events on the stream around replays of a graph that runs the part on every resident copy in turn (consecutive launches share nothing through L2), right after the timed region")
     else:

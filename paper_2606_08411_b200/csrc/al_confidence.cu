@@ -6,8 +6,13 @@
 //     148 SMs) owns one row; CTA c streams the c-th contiguous chunk of the row.  A warp folds 2 KB
 //     items (4 x 16-byte streaming loads per lane; two items in registers, the loads of the next one
 //     issued before the current one is reduced) in two register passes:
-//       pass A  packed bf16x2 max over the lane's 64 values -> warp max through one REDUX
-//       pass B  sum += ex2(x*log2e - m*log2e): unpack, FFMA, MUFU.EX2, FADD per element
+//       pass A  packed bf16x2 max over the lane's 32 values -> warp max through one REDUX
+//       pass B  sum += ex2(x*log2e - m*log2e): unpack, then per PAIR of elements one packed FFMA2, two
+//               MUFU.EX2 and one packed FADD2 -- and for two pairs of every eight a degree-4 polynomial on
+//               the FMA pipes instead of the MUFU (exp2_poly_pair).  At the HBM rate one ex2 per element
+//               keeps the SM's 16-per-clock MUFU 75 % busy and the issue slots 70 %: the stream is bound by
+//               all three at once, which is why instructions per element were counted (full items load
+//               unpredicated, the EOS test is one warp-uniform compare per item).
 //     keeping a warp-uniform running max m (rescaling the sum only when an item raises it) and the
 //     first index attaining it.  Warps merge through shared memory, the CTAs of a cluster merge in
 //     the leader's shared memory over DSMEM, and the leader applies the commit rule: no partials in
@@ -29,6 +34,13 @@ constexpr int kItemVecs = 32 * kWarpVecs;    // 128 vectors = 2 KB per item; a w
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kMaxCluster = 8;
+// Of every eight element pairs, those whose exponential runs on the FMA pipes (exp2_poly_pair) instead of the
+// MUFU: one ex2 per element keeps the SM's 16-per-clock MUFU 75 % busy at the HBM rate, and below one wave of
+// CTAs it is the busiest SM's MUFU, not HBM, that bounds the launch.
+#ifndef AL_CONF_POLY_MASK
+#define AL_CONF_POLY_MASK 0x88
+#endif
+constexpr uint32_t kPolyPairs = AL_CONF_POLY_MASK;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr int kNoIdx = 0x7fffffff;
 
@@ -49,6 +61,44 @@ __device__ __forceinline__ float ex2(float x) {           // x <= 0 here (or -in
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+// 2^x for a pair on the FMA pipes, x <= 0 (or -inf): x = n + f, n = rint(x) read from the low mantissa bits of
+// x + 1.5 * 2^23, f in [-0.5, 0.5]; 2^f by a degree-4 polynomial (relative error 2.7e-6 evaluated in fp32, mean
+// 4e-8; the MUFU's ex2.approx is about 2e-7), 2^n by adding n to the exponent field.  Clamped at -126: padding
+// and suppressed elements are -inf and contribute 2^-126 instead of 0, far below the rounding of a sum >= 1.
+__device__ __forceinline__ void exp2_poly_pair(uint64_t x2, float& p0, float& p1) {
+  float x0, x1;
+  unpack2(x2, x0, x1);
+  x2 = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+  const uint64_t r2 = fadd2(x2, pack2(12582912.f, 12582912.f));
+  const uint64_t f2 = ffma2(fadd2(r2, pack2(-12582912.f, -12582912.f)), pack2(-1.f, -1.f), x2);
+  uint64_t q2 = ffma2(pack2(0.009570101276f, 0.009570101276f), f2, pack2(0.05591785908f, 0.05591785908f));
+  q2 = ffma2(q2, f2, pack2(0.2402474433f, 0.2402474433f));
+  q2 = ffma2(q2, f2, pack2(0.6931217909f, 0.6931217909f));
+  q2 = ffma2(q2, f2, pack2(0.9999992847f, 0.9999992847f));
+  float q0, q1, r0, r1;
+  unpack2(q2, q0, q1);
+  unpack2(r2, r0, r1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(r0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(r1) << 23));
 }
 // order-preserving float <-> int map, so that one integer REDUX gives the warp max of floats
 __device__ __forceinline__ int f2ord(float f) {
@@ -145,20 +195,23 @@ __device__ __forceinline__ void fold_scalar(float x, int e, float& m, float& s, 
 
 template <typename T>
 __device__ __forceinline__ void load_item(int4 (&v)[kWarpVecs], const T* __restrict__ row, int vi0, int v_end) {
-  constexpr int E = Vec<T>::kElems;
-  const int pad = (int)Vec<T>::kAccInit;
+  const int4* src = reinterpret_cast<const int4*>(row) + vi0;
+  if (vi0 - (int)(threadIdx.x & 31) + kItemVecs <= v_end) {          // warp-uniform: the whole item is in range
 #pragma unroll
-  for (int j = 0; j < kWarpVecs; ++j) {
-    const int vi = vi0 + j * 32;
-    v[j] = vi < v_end ? ld_stream(row + (long long)vi * E) : make_int4(pad, pad, pad, pad);
+    for (int j = 0; j < kWarpVecs; ++j) v[j] = ld_stream(src + j * 32);
+  } else {
+    const int pad = (int)Vec<T>::kAccInit;
+#pragma unroll
+    for (int j = 0; j < kWarpVecs; ++j)
+      v[j] = vi0 + j * 32 < v_end ? ld_stream(src + j * 32) : make_int4(pad, pad, pad, pad);
   }
 }
 // EOS suppression (refine rows only): element `sup` of the row becomes -inf in the item held in registers
 template <typename T>
 __device__ __forceinline__ void suppress_in_item(int4 (&v)[kWarpVecs], int vi0, int sup) {
   constexpr int E = Vec<T>::kElems;
-  if (sup >= 0) {
-    const int sv = sup / E;
+  const int sv = sup / E;                                    // sup = -1: sv = 0 and the guard below fails
+  if (sup >= 0 && (unsigned)(sv - (vi0 - (int)(threadIdx.x & 31))) < (unsigned)kItemVecs) {   // warp-uniform: this item holds it
 #pragma unroll
     for (int j = 0; j < kWarpVecs; ++j)
       if (vi0 + j * 32 == sv) Vec<T>::set_neg_inf(v[j], sup - sv * E);
@@ -190,18 +243,31 @@ __device__ __forceinline__ void fold_item(const int4 (&v)[kWarpVecs], int vi0, f
     }
     idx = __reduce_min_sync(0xffffffffu, cand);
   }
+  // packed fp32x2 FMA / ADD (sm_100): one issue slot per PAIR for the scaling and for the sum -- the stream is
+  // bound by instruction issue before it is bound by HBM when fewer than four CTAs are resident per SM.  Each
+  // half is the IEEE fma / add of the scalar form, the even elements in the low half, the odd ones in the high.
   const float mb = (m == -INFINITY) ? 0.f : m * kLog2e;
-  float s0 = 0.f, s1 = 0.f;
+  const uint64_t l2 = pack2(kLog2e, kLog2e), nmb2 = pack2(-mb, -mb);
+  uint64_t sum2 = pack2(0.f, 0.f);
 #pragma unroll
   for (int j = 0; j < kWarpVecs; ++j) {
     float x[E];
     Vec<T>::unpack(v[j], x);
 #pragma unroll
     for (int e = 0; e < E; e += 2) {
-      s0 += ex2(fmaf(x[e], kLog2e, -mb));
-      s1 += ex2(fmaf(x[e + 1], kLog2e, -mb));
+      const uint64_t t2 = ffma2(pack2(x[e], x[e + 1]), l2, nmb2);
+      float a, b;
+      if ((kPolyPairs >> ((j * (E / 2) + e / 2) & 7)) & 1u) {
+        exp2_poly_pair(t2, a, b);
+      } else {
+        unpack2(t2, a, b);
+        a = ex2(a); b = ex2(b);
+      }
+      sum2 = fadd2(sum2, pack2(a, b));
     }
   }
+  float s0, s1;
+  unpack2(sum2, s0, s1);
   s += s0 + s1;
 }
 
