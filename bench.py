@@ -109,6 +109,9 @@ class ClockSampler(threading.Thread):
                     pass
             time.sleep(self.period)
 
+    def reset(self):
+        self.samples, self.reason_bits, self.power = [], 0, []
+
     def summary(self):
         if not self.ok or not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unsampled"], "samples": 0}
@@ -300,8 +303,23 @@ def measure_resident(h, wl, dev, stream, dist, sampler, steps, warmup, kernel_ev
             part_ms[name] = e0.elapsed_time(e1) / (reps * inner)
             part_ms["n_samples"] = reps * inner
         sampler.active.clear()
+    # warm-L2 step (cold and warm reported separately): the same graph replayed on ONE copy, for
+    # workloads whose streamed bytes fit the L2 at all -- not the headline, which always rotates the copies
+    warm_ms = None
+    if kernel_events and per_copy <= L2_BYTES:
+        n_warm = max(20, min(steps, 200))
+        with torch.cuda.stream(stream):
+            for _ in range(5):
+                graphs[0].replay()
+            e0.record(stream)
+            for _ in range(n_warm):
+                graphs[0].replay()
+            e1.record(stream)
+        barrier()
+        warm_ms = e0.elapsed_time(e1) / n_warm
     return dict(step_ms=step_ms, part_ms=part_ms, launches_per_step=launches_per_step, copies=copies,
-                n_copies=n_copies, per_copy=per_copy, barrier=barrier, graphs=graphs, part_graphs=part_graphs)
+                n_copies=n_copies, per_copy=per_copy, barrier=barrier, graphs=graphs, part_graphs=part_graphs,
+                warm_ms=warm_ms)
 
 
 def measure_next_rows(h, dev, stream, peaks):
@@ -413,30 +431,6 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     sampler = ClockSampler(local_rank)
     sampler.start()
 
-    # ---- the other single-GPU configs first (extra key `workloads`; fewer steps), then the headline one ----
-    extra = {}
-    if args.extra_workloads and world == 1:
-        for name in [w for w in args.extra_workloads.split(",") if w and w != args.workload]:
-            wl_x = W.CONFIGS[name]()
-            acc_x = accounting.summary(wl_x)
-            m = measure_resident(h, wl_x, dev, stream, None, sampler, min(args.steps, args.extra_steps), args.warmup)
-            parts_x = part_rooflines(wl_x, acc_x, m["part_ms"], m["step_ms"], peaks, load_traffic(wl_x.name))
-            extra[wl_x.name] = {
-                "step_us": m["step_ms"] * 1e3, "query_tok_per_s": acc_x["query_tokens"] / (m["step_ms"] * 1e-3),
-                "steps": min(args.steps, args.extra_steps), "layers": wl_x.n_layers, "query_rows": wl_x.total_q_rows,
-                "copies": m["n_copies"], "gpu_launches_per_step": m["launches_per_step"],
-                "parts": {k: {kk: p[kk] for kk in ("bound", "ms", "achieved", "peak", "unit", "frac", "traffic", "note") if kk in p}
-                          for k, p in parts_x.items()}}
-            del m, wl_x
-            gc.collect()
-            torch.cuda.empty_cache()
-
-    next_rows = None
-    if args.next_rows and world == 1:
-        next_rows = measure_next_rows(h, dev, stream, peaks)
-        gc.collect()
-        torch.cuda.empty_cache()
-
     wl = W.CONFIGS[args.workload]()
     acc = accounting.summary(wl)
     m = measure_resident(h, wl, dev, stream, dist, sampler, args.steps, args.warmup, args.kernel_events)
@@ -472,13 +466,48 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     e2e_ms = max(e0.elapsed_time(e1) / e2e_steps, wall_ms)       # host-visible completion time
     e2e_ms = max_over_ranks(e2e_ms, dist, dev)
     e2e_tokens = wl.total_q_rows                                  # all layers of the workload per host step
-    sampler.stop_flag.set()
-    sampler.join(timeout=2)
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
+
+    # ---- the headline is measured FIRST, on a GPU that has done nothing yet (the fused LM head of `next_rows` draws
+    # ~600 W and leaves this pool's B200s power-capped for a while); `clocks` is the sampler's view of the headline's
+    # timed regions, `clocks_rest` that of everything measured afterwards
+    clocks_headline = sampler.summary()
+    sampler.reset()
+    del hstep
+    gc.collect()
+    torch.cuda.empty_cache()
+    # ---- then the other single-GPU configs (extra key `workloads`; fewer steps) and the 8(f) rows ----
+    extra = {}
+    if args.extra_workloads and world == 1:
+        for name in [w for w in args.extra_workloads.split(",") if w and w != args.workload]:
+            wl_x = W.CONFIGS[name]()
+            acc_x = accounting.summary(wl_x)
+            mx = measure_resident(h, wl_x, dev, stream, None, sampler, min(args.steps, args.extra_steps), args.warmup)
+            parts_x = part_rooflines(wl_x, acc_x, mx["part_ms"], mx["step_ms"], peaks, load_traffic(wl_x.name))
+            extra[wl_x.name] = {
+                "step_us": mx["step_ms"] * 1e3, "query_tok_per_s": acc_x["query_tokens"] / (mx["step_ms"] * 1e-3),
+                "steps": min(args.steps, args.extra_steps), "layers": wl_x.n_layers, "query_rows": wl_x.total_q_rows,
+                "copies": mx["n_copies"], "gpu_launches_per_step": mx["launches_per_step"],
+                "warm_l2_step_us": mx["warm_ms"] * 1e3 if mx["warm_ms"] else None,     # one copy replayed (fits the L2); step_us is the cold figure
+                "parts": {k: {kk: p[kk] for kk in ("bound", "ms", "achieved", "peak", "unit", "frac", "traffic", "note") if kk in p}
+                          for k, p in parts_x.items()}}
+            del mx, wl_x
+            gc.collect()
+            torch.cuda.empty_cache()
+
+    next_rows = None
+    if args.next_rows and world == 1:
+        next_rows = measure_next_rows(h, dev, stream, peaks)
+        gc.collect()
+        torch.cuda.empty_cache()
+
+    clocks_rest = sampler.summary()
+    sampler.stop_flag.set()
+    sampler.join(timeout=2)
 
     # ---- roofline of every part; `roofline` = the part with the largest share of the step ------
     parts = {}
@@ -509,7 +538,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                              if first.logits.numel() * first.logits.element_size() <= first.OVERLAP_MAX_LOGITS_BYTES
                              else "plan -> attention per layer -> refresh -> confidence/select")
                             + "; the parts are also timed alone on graphs of their own"},
-        "clocks": sampler.summary(),
+        "clocks": clocks_headline, "clocks_rest": clocks_rest,
         "e2e": {"value": whole_job_value(e2e_tokens, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps, "layers": wl.n_layers,
                 "api": "al_lane_step_host (pinned host buffers; H2D + plan + attention per layer + refresh + "
@@ -527,7 +556,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--steps", type=int, default=300)   # 71 ms at cfg5: past ~0.25 s of back-to-back steps this pool's B200s report sw_power_cap
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
