@@ -1325,21 +1325,24 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       if (tid128 == 0 && b == 0) TRACE(7);
       // o_full[b] completes once per piece in which the stream had key tiles (a per-P.V parity wait
       // could alias here: with Q.K^T two tiles ahead, two P.V may still be in flight)
-      if (n_mine > 0) { mbar_wait(&sm.o_full[b], pieces_done & 1); tc_fence_after(); ++pieces_done; }
-      if (tid128 == 0 && b == 0) TRACE(8);
-      TRACE_E(0);
+      // what does not need the accumulator is worked out while the last P.V drains
       const float inv = l_sum > 0.f ? 1.0f / l_sum : 0.f;
       const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
       const bool whole = w.whole();
       const int slot = 2 * (int)blockIdx.x + (w.kt_begin == 0 ? 1 : 0);
       bool do_ticket = !whole && n_rows > 0;           // a piece of a split item: publish, count, maybe merge
+      if (!alt && whole && n_mine > 0) off_b[r] = (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128));
+      if (!alt && n_mine > 0) { mbar_wait(&sm.o_full[b], pieces_done & 1); tc_fence_after(); ++pieces_done; }
+      if (tid128 == 0 && b == 0) TRACE(8);
+      TRACE_E(0);
       if (alt) {
         // ---- one sub-tile, two streams (even / odd key tiles): merge them, each storing 64 columns ----
+        // (the streams exchange their running maxima and row sums and work out the merge weights while their
+        // last P.V drain; each waits for its own accumulator just before the second barrier)
         if (tid128 == 0) sm.alt_has[b] = n_mine > 0;
         AL_STAGE_ROUND_BEGIN();                        // the previous piece's bulk stores are done with the staging rows
         *reinterpret_cast<float2*>(my_stage) = make_float2(m_used, l_sum);   // exchanged through the staging rows
         bar_sync_both();
-        tc_fence_after();                              // the other stream's accumulator is read below, behind its thread's o_full wait
         TRACE_E(1);
         const float2 oth = *reinterpret_cast<const float2*>(sm.stage + ((b ^ 1) * kBM + r) * kStagePitch);
         const bool has0 = sm.alt_has[0] != 0, has1 = sm.alt_has[1] != 0;
@@ -1352,7 +1355,9 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         const float rL = L > 0.f ? 1.0f / L : 0.f;
         const float f0 = w0 * rL, f1 = w1 * rL;
         const float lse2 = L > 0.f ? (M * p.scale_log2 + log2f(L)) / kLog2e : -INFINITY;
-        bar_sync_both();                               // the exchanged values have been read: the rows may be staged over
+        if (n_mine > 0) { mbar_wait(&sm.o_full[b], pieces_done & 1); ++pieces_done; }
+        bar_sync_both();                               // the exchanged values have been read (the rows may be staged over) and both accumulators are complete
+        tc_fence_after();                              // the other stream's accumulator is read below, behind its thread's o_full wait
         TRACE_E(2);
         const bool full = kTmaStoreOk && T.n_tok >= p.tpt;   // the sub-tile fills its TMA box: no row beyond it may be written
         if (whole) off_b[r] = (uint32_t)(out_row(p, T, w.g, 0, valid ? r : 0) * (kD * 2 / 128));
@@ -1423,8 +1428,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       } else if (whole) {
         // bf16 output: two rounds of 64 columns = 128 bytes per row = one 64-column half of the tile, which a full
         // sub-tile stores with ONE TMA tensor store from the staging rows (same box and swizzle as the Q loads);
-        // the last, partial sub-tile of a run copies its rows out itself
-        off_b[r] = (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128));
+        // the last, partial sub-tile of a run copies its rows out itself (off_b: set before the o_full wait)
 #pragma unroll
         for (int rd = 0; rd < 2; ++rd) {
           TRACE_E(1 + 5 * rd);
