@@ -355,9 +355,12 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
         C.tile0 = t;
         C.first_c0 = C.first_c1 = C.last_c0 = C.last_c1 = c;
         C.pad = c;
-        C.flags = kCtaActive | kCtaAlt; C.reserved[0] = C.reserved[1] = C.reserved[2] = 0;
+        C.reserved[0] = C.reserved[1] = C.reserved[2] = 0;
         C.first = t < kPlanTilesInSmem ? s_tiles[t] : plan.tiles[t];   // written by this block above
         C.first.kt_off = s_a[t];
+        // a whole item of ONE sub-tile is worked on by both streams (alt instance of the roles); one of two
+        // sub-tiles runs in the other instance, a stream per sub-tile
+        C.flags = kCtaActive | (C.first.n_tok <= tpt ? kCtaAlt : 0);
         plan.ctas[c] = C;
       }
     }
@@ -567,7 +570,7 @@ struct StreamSteps {
   int par;                                 // alt mode: it takes the steps with (i & 1) == par; else -1
   __device__ __forceinline__ StreamSteps(const TileRec& T, int tpt, int b, int kt_begin, bool alt_ok) {
     pref = 0; lo = 0; n_loc = 0; par = -1;
-    if (alt_ok && T.n_tok <= tpt) {        // a tile of one sub-tile: the two streams take alternate key tiles of it
+    if (alt_ok) {                          // a tile of one sub-tile (the CTA's record says so: kCtaAlt): the two streams take alternate key tiles of it
       par = (kt_begin ^ b) & 1;
     } else if (b * tpt < T.n_tok) {
       const int s0 = b ? T.sub_lk0[1] : T.sub_lk0[0], s1 = b ? T.sub_lk1[1] : T.sub_lk1[0];
@@ -805,9 +808,12 @@ __device__ __forceinline__ float* part_round_ptr(const AttnParams& p, int slot, 
     if (tid128 == 0) { issue_stmt; bulk_commit(); }                                                            \
   } while (0)
 
-// The role code of the kernel, compiled twice: with and without the "alt" mode (one sub-tile worked on
-// by both streams).  The plan chooses per launch; keeping the alt code out of the other instance keeps
-// its hot loops as lean as they were (measured: 8 us of 108 at cfg5).
+// The role code of the kernel, compiled twice: FOR the "alt" mode (kAltOk: the CTA holds one whole item of one
+// sub-tile, worked on by both streams -- `alt` is a compile-time constant) and without it (everything else:
+// step ranges, item lists, whole items of two sub-tiles).  The plan (or self_plan_record) chooses per CTA.
+// Keeping each mode's code out of the other instance is worth a lot: the general instance got 8 us of 108 at
+// cfg5 in round 1, and making the alt instance alt-ONLY (it used to test the tile at run time) took cfg4 from
+// 616 to 585 us per 32 layers and the cfg3 kernel from 18.4 to 16.7 us.
 template <bool kAltOk>
 __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, const CUtensorMap* pmap_q,
                                            const CUtensorMap* pmap_knew, const CUtensorMap* pmap_vnew,
@@ -905,7 +911,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
-        const bool alt = alt_ok && w.T.n_tok <= p.tpt;     // one sub-tile: both streams work on Q of sub-tile A
+        const bool alt = alt_ok;     // one sub-tile: both streams work on Q of sub-tile A
         const StreamSteps mine(w.T, p.tpt, b, w.kt_begin, alt_ok);
         const uint64_t dq0 = alt ? dq_a0 : dq_own0, dq1 = alt ? dq_a1 : dq_own1;
         mbar_wait(&sm.q_full, piece_it & 1);
@@ -1045,7 +1051,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
       while (w.next()) {
         const int n = w.kt_end - w.kt_begin;
-        const bool alt = alt_ok && w.T.n_tok <= p.tpt;     // one sub-tile: both streams work on Q of sub-tile A
+        const bool alt = alt_ok;     // one sub-tile: both streams work on Q of sub-tile A
         const StreamSteps mine0(w.T, p.tpt, 0, w.kt_begin, alt_ok), mine1(w.T, p.tpt, 1, w.kt_begin, alt_ok);
         const uint64_t dq10 = alt ? dq_a0 : dq_b0, dq11 = alt ? dq_a1 : dq_b1;
         mbar_wait(&sm.q_full, piece_it & 1);
@@ -1187,7 +1193,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
     while (w.next()) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
-      const bool alt = alt_ok && T.n_tok <= p.tpt;     // one sub-tile: this stream takes every other key tile of it
+      const bool alt = alt_ok;     // one sub-tile: this stream takes every other key tile of it
       const int sb = alt ? 0 : b;                      // sub-tile whose rows this stream holds
       const StreamSteps mine(T, p.tpt, b, w.kt_begin, alt_ok);
       const int n_rows = sub_rows(p, T, sb);
@@ -1596,15 +1602,15 @@ __device__ __noinline__ void self_plan_record(const al_lane_desc* __restrict__ l
     T.kt_off = 0;                                            // the CTA's steps are counted from its own tile
     C.f_begin = g * T.n_key_tiles; C.f_end = C.f_begin + T.n_key_tiles;
     C.tile0 = t;
-    C.flags = kCtaActive | kCtaAlt;
+    C.flags = kCtaActive | (T.n_tok <= tpt ? kCtaAlt : 0);     // one sub-tile: both streams work on it (alt instance)
     C.first = T;
   }
   if (i == 0) *out = C;
 }
 
-// kSelfPlan: the launch has no plan (self_plan_record); such CTAs always hold one whole item, so only the
-// whole-item instance of the roles is compiled in.  Two kernels rather than a switch in one: the plan-reading
-// instance keeps the code it had (its schedule is sensitive to anything added around it).
+// kSelfPlan: the launch has no plan (self_plan_record).  Two kernels rather than a switch in one: the
+// plan-reading kernel keeps the prologue it had (its schedule is sensitive to anything added around it), and
+// each kernel lays out first the instance of the roles its launches use most.
 template <bool kSelfPlan>
 __global__ void __launch_bounds__(kThreads, 1)
 lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_knew,
@@ -1651,12 +1657,16 @@ lane_attention_umma_kernel(const __grid_constant__ CUtensorMap map_q, const __gr
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   // TMEM columns: S of stream b at 64 b; P of stream b, buffer u at 128 + 64 b + 32 u; O of stream b at 256 + 128 b
+  // Two instances of the roles: one for CTAs whose (single, whole) item has ONE sub-tile, which both streams
+  // work on (kCtaAlt in the CTA's record; `alt` is a compile-time constant there), one for everything else.  The
+  // instance laid out FIRST runs measurably faster inside a step (cfg5 plan + attention 67.5 us with the
+  // general instance first, 71.5 us with it second; cfg4 620 us against 634 us per 32 layers the other way
+  // round): the plan-reading kernel gives the throughput configuration the first place, the self-planned one
+  // (small calls: one sub-tile as a rule) the alt instance.
   if constexpr (kSelfPlan) {
-    attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
+    if (sm.cta.flags & kCtaAlt) attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
+    else attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
   } else {
-    // The instance laid out FIRST runs measurably faster inside a step (cfg5 plan + attention 67.5 us with the
-    // step-range instance first, 71.5 us with it second; cfg4 620 us against 634 us per 32 layers the other way
-    // round): the throughput configuration gets the first place.
     if (!(sm.cta.flags & kCtaAlt)) attn_roles<false>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
     else attn_roles<true>(sm, p, &map_q, &map_knew, &map_vnew, &map_kc, &map_vc, &map_out, tmem, warp, lane);
   }
