@@ -1334,7 +1334,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       // what does not need the accumulator is worked out while the last P.V drains
       const float inv = l_sum > 0.f ? 1.0f / l_sum : 0.f;
       const float lse = l_sum > 0.f ? (m_used * p.scale_log2 + log2f(l_sum)) / kLog2e : -INFINITY;
-      const bool whole = w.whole();
+      const bool whole = alt_ok || w.whole();          // an alt CTA holds ONE whole item: no partials, tickets or merges in that instance
       const int slot = 2 * (int)blockIdx.x + (w.kt_begin == 0 ? 1 : 0);
       bool do_ticket = !whole && n_rows > 0;           // a piece of a split item: publish, count, maybe merge
       if (!alt && whole && n_mine > 0) off_b[r] = (uint32_t)(out_row(p, T, w.g, b, valid ? r : 0) * (kD * 2 / 128));
