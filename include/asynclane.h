@@ -239,6 +239,27 @@ al_status al_lm_head_confidence(al_handle* handle, const void* hidden_bf16, cons
                                 float* conf_out, int32_t* argmax_out, uint8_t* commit_out, int32_t* tokens_out,
                                 void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * The same call for callers that cannot allocate device memory (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): it takes no workspace -- the partials live in a device array of
+ * AL_LM_HEAD_STATIC_SCRATCH_BYTES (1 MiB) that is part of the library image, so every GPU that loads the library
+ * holds it until exit -- and calls no cudaMalloc / cudaFree or allocating library routine.  Arguments, results and
+ * errors as al_lm_head_confidence; additionally AL_ERR_UNSUPPORTED, before anything is enqueued, when the shape
+ * needs more scratch than the array holds (16 bytes x 128 x ceil(n_rows / 128) x vocabulary chunks, the chunks
+ * chosen from the SM count: 128 x 126464 takes 0.3 MB, 3264 x 152064 0.9 MB, 8192 x 152064 2 MB -- too many).
+ * ALL calls on a device share the one array: calls that may overlap on the GPU (different streams, or graphs
+ * replayed concurrently) race on it and must be serialised by the caller; calls on one stream are ordered.
+ * The array keeps the last call's contents; nothing in it has to be cleared (every slot read is written first).
+ */
+#define AL_LM_HEAD_STATIC_SCRATCH_BYTES (1 << 20)
+size_t al_lm_head_confidence_static_max_bytes(void);
+al_status al_lm_head_confidence_static(al_handle* handle, const void* hidden_bf16, const void* weight_bf16,
+                                       int32_t n_rows, int32_t vocab, int32_t hidden_dim,
+                                       const int32_t* tokens_in_dev, int32_t mask_id, int32_t eos_id, float threshold,
+                                       const al_lane_desc* lanes_dev_or_null, int32_t n_lanes, int32_t flags,
+                                       float* conf_out, int32_t* argmax_out, uint8_t* commit_out, int32_t* tokens_out,
+                                       void* cuda_stream);
+
 /* ---- (d) lane status: what the scheduler reads back from one iteration ------------------------- */
 
 /*

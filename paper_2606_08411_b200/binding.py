@@ -23,7 +23,8 @@ EXPORTS = [
     "al_lane_attention_workspace_bytes", "al_lane_attention", "al_lane_plan", "al_lane_attention_planned",
     "al_kv_refresh", "al_refresh_forward", "al_lane_status", "al_scheduler_run", "al_stub_model_fn",
     "al_confidence_select_workspace_bytes", "al_confidence_select", "al_lm_head_confidence_workspace_bytes",
-    "al_lm_head_confidence", "al_validate_lanes", "al_validate_refresh",
+    "al_lm_head_confidence", "al_lm_head_confidence_static_max_bytes", "al_lm_head_confidence_static",
+    "al_validate_lanes", "al_validate_refresh",
     "al_selftest_umma", "al_lane_step_host", "al_lane_step_host_arena_bytes", "al_lane_step_host_traffic",
     "al_launch_count",
 ]
@@ -130,6 +131,10 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.al_lm_head_confidence_workspace_bytes.restype = sz
     lib.al_lm_head_confidence.argtypes = [vp, vp, vp, i32, i32, i32, vp, i32, i32, f32, vp, i32, i32, vp, vp, vp, vp, vp,
                                           sz, vp]
+    lib.al_lm_head_confidence_static_max_bytes.argtypes = []
+    lib.al_lm_head_confidence_static_max_bytes.restype = sz
+    lib.al_lm_head_confidence_static.argtypes = [vp, vp, vp, i32, i32, i32, vp, i32, i32, f32, vp, i32, i32, vp, vp, vp, vp,
+                                                 vp]
     lib.al_lane_status.argtypes = [vp, vp, i32, i32, vp, vp, vp, i32, i32, f32, vp, i32, vp, i32, vp, vp, vp, vp]
     lib.al_scheduler_run.argtypes = [vp, ctypes.POINTER(al_sched_config), vp, vp, ctypes.POINTER(al_sched_device_state),
                                      vp, vp, vp, ctypes.POINTER(i32), ctypes.POINTER(al_sched_lane), i32,
@@ -150,7 +155,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         fn = getattr(lib, name)
         if name not in ("al_last_error", "al_version", "al_sm_count", "al_lane_attention_workspace_bytes",
                         "al_confidence_select_workspace_bytes", "al_lane_step_host_arena_bytes",
-                        "al_lm_head_confidence_workspace_bytes",
+                        "al_lm_head_confidence_workspace_bytes", "al_lm_head_confidence_static_max_bytes",
                         "al_lane_step_host_traffic", "al_launch_count", "al_stub_model_fn"):
             fn.restype = ctypes.c_int
     _lib = lib
@@ -303,6 +308,18 @@ class Handle:
                                                _ptr(tokens_in), mask_id, eos_id, threshold, _ptr(lanes_dev), n_lanes,
                                                flags, _ptr(conf_out), _ptr(argmax_out), _ptr(commit_out),
                                                _ptr(tokens_out), _ptr(workspace), ws_bytes, _stream_ptr(stream)))
+
+    def al_lm_head_confidence_static_max_bytes(self) -> int:
+        return int(self._lib.al_lm_head_confidence_static_max_bytes())
+
+    def al_lm_head_confidence_static(self, hidden, weight, n_rows, vocab, hidden_dim, tokens_in, mask_id, eos_id,
+                                     threshold, lanes_dev, n_lanes, flags, conf_out, argmax_out, commit_out, tokens_out,
+                                     stream=None) -> None:
+        """al_lm_head_confidence without a workspace: the partials live in the library's static device array."""
+        _check(self._lib.al_lm_head_confidence_static(self._h, _ptr(hidden), _ptr(weight), n_rows, vocab, hidden_dim,
+                                                      _ptr(tokens_in), mask_id, eos_id, threshold, _ptr(lanes_dev),
+                                                      n_lanes, flags, _ptr(conf_out), _ptr(argmax_out),
+                                                      _ptr(commit_out), _ptr(tokens_out), _stream_ptr(stream)))
 
     def al_lane_status(self, lanes_dev, n_lanes, n_rows, tokens_in, conf, argmax, mask_id, eos_id, tau_future,
                        delimiter_ids, no_fork_prev_ids, commit_io, tokens_io, status_out, stream=None) -> None:

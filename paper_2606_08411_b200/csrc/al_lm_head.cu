@@ -392,3 +392,47 @@ extern "C" al_status al_lm_head_confidence(al_handle* h, const void* hidden, con
                                 argmax_out, commit_out, tokens_out, cs);
   return AL_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// al_lm_head_confidence_static: the same call for callers that cannot allocate (CUDA graph capture, serving
+// loops, harnesses that forbid cudaMalloc): the per-(row, chunk) partials live in a file-scope device array
+// instead of a caller-provided workspace.  Every GPU that loads the library holds the array until exit.
+// ---------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t kStaticScratchBytes = (size_t)AL_LM_HEAD_STATIC_SCRATCH_BYTES;   // 1 MiB = 65536 (m, s, idx) slots
+static __device__ __align__(256) unsigned char g_lm_head_scratch[kStaticScratchBytes];
+// In host code `g_lm_head_scratch` is a host-side stand-in, NOT a device address: the address a kernel may use comes
+// from cudaGetSymbolAddress, looked up once per device with that device current.
+constexpr int kMaxDevices = 64;
+void* g_scratch_ptr[kMaxDevices];               // zero-initialised; written once per device (same value from any thread)
+}  // namespace
+
+extern "C" size_t al_lm_head_confidence_static_max_bytes(void) { return kStaticScratchBytes; }
+
+extern "C" al_status al_lm_head_confidence_static(al_handle* h, const void* hidden, const void* weight, int32_t n_rows,
+                                                  int32_t vocab, int32_t hidden_dim, const int32_t* tokens_in,
+                                                  int32_t mask_id, int32_t eos_id, float threshold,
+                                                  const al_lane_desc* lanes, int32_t n_lanes, int32_t flags,
+                                                  float* conf_out, int32_t* argmax_out, uint8_t* commit_out,
+                                                  int32_t* tokens_out, void* stream) {
+  const char* who = "al_lm_head_confidence_static";
+  if (!h) AL_FAIL(AL_ERR_INVALID_ARG, "%s: handle is NULL", who);
+  if (n_rows < 0 || vocab < 0) AL_FAIL(AL_ERR_INVALID_ARG, "%s: negative size", who);
+  if (n_rows == 0) return AL_OK;
+  al_status st = al_check_device(h, who);       // the handle's device is the current one from here on
+  if (st != AL_OK) return st;
+  if (vocab == 0) AL_FAIL(AL_ERR_INVALID_ARG, "%s: vocab is 0", who);
+  const size_t need = lm_plan(n_rows, vocab, h->sm_count).ws_bytes;
+  if (need > kStaticScratchBytes)
+    AL_FAIL(AL_ERR_UNSUPPORTED, "%s: %d rows x %d vocabulary entries need %zu bytes of scratch, the static array holds %zu "
+            "(use al_lm_head_confidence with a workspace)", who, n_rows, vocab, need, kStaticScratchBytes);
+  if (h->device < 0 || h->device >= kMaxDevices) AL_FAIL(AL_ERR_UNSUPPORTED, "%s: device %d", who, h->device);
+  void* ptr = g_scratch_ptr[h->device];
+  if (!ptr) {
+    AL_CUDA_OK(cudaGetSymbolAddress(&ptr, g_lm_head_scratch));
+    g_scratch_ptr[h->device] = ptr;
+  }
+  // Nothing in the array has to start at zero: every slot the select kernel reads is written by this call's units.
+  return al_lm_head_confidence(h, hidden, weight, n_rows, vocab, hidden_dim, tokens_in, mask_id, eos_id, threshold, lanes,
+                               n_lanes, flags, conf_out, argmax_out, commit_out, tokens_out, ptr, kStaticScratchBytes, stream);
+}
