@@ -13,10 +13,12 @@
 //   keys     = [prefix key tiles of 64 cache rows] ++ [local key tiles of 64 K_new rows covering the
 //              lanes that intersect the tile]; every row masks what its own lane may not see
 //   item     = (tile, kv-head): n_key_tiles steps of the main loop
-// The 64-key steps of all items, flattened item-major, are cut into per-CTA ranges: one CTA per item
-// ("whole items") when every item can have a CTA of its own and splitting would not pay, else
-// n_ctas contiguous ranges of equal cost ("stream-K": steps + kEpiCost per item finished, whatever
-// the lane structure is), a boundary within one step of an item boundary snapping to it.  An item
+// The 64-key steps of all items go to the CTAs in one of three ways: one CTA per item ("whole items")
+// when every item can have a CTA of its own and splitting would not pay (small calls of this kind launch
+// no plan kernel at all: every CTA derives its record itself, self_plan_record); whole items DEALT to
+// the CTAs, longest first, when there are more items than CTAs and that is cheaper ("item lists"); else
+// n_ctas contiguous ranges of the flattened steps of equal cost ("stream-K": steps + kEpiCost per item
+// finished), a boundary within one step of an item boundary snapping to it.  An item
 // whose steps are spread over several CTAs leaves one normalised fp32 partial + LSE per CTA in the
 // workspace; the CTA that finishes last (a ticket counter per (item, sub-tile)) merges them in a
 // fixed order -- no combine launch, bit-identical results from call to call.
@@ -29,13 +31,15 @@
 //   warps 1, 2  MMA issuer of stream A / B (warp-uniform, one elected lane): S_b = Q_b.K^T (SS form)
 //               into the stream's S buffer as soon as the softmax holds the previous S in registers;
 //               O_b += P_b.V with P_b read from one of the stream's two P buffers in TMEM (TS form)
-//               and V MN-major in shared memory
+//               and V MN-major in shared memory.  (In the instance for one whole item of one sub-tile
+//               warp 1 issues every Q.K^T and warp 2 every P.V, each for both streams.)
 //   warps 4-7   softmax of stream A (sub-tile A), one thread per stacked row
 //   warps 8-11  softmax of stream B (sub-tile B; with one sub-tile per tile under a whole-item plan
 //               the two streams take alternate key tiles of it and the epilogue merges them)
 //               O is rescaled lazily (only when the running max grows by more than 2^8).  Epilogue
 //               per stream: normalise, stage 128-byte half rows in shared memory, store coalesced
-//               (bf16 output, or fp32 partial for a split item).
+//               (bf16 output: one TMA tensor store per 64-column half of a full sub-tile; fp32
+//               partial for a split item: bulk stores).
 // TMEM (512 columns): S_A | S_B (64 fp32 columns each) | P_A[2] | P_B[2] (32 columns of packed bf16
 // each) | O_A | O_B (128 fp32 columns each).
 #include <cuda_bf16.h>
