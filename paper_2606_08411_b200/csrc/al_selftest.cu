@@ -30,7 +30,7 @@ selftest_umma_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_con
                      float* __restrict__ o_out, int variant) {
   extern __shared__ uint8_t smem_raw[];
   SelfSmem& sm = *reinterpret_cast<SelfSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = threadIdx.x >> 5;
 
   if (threadIdx.x == 0) {
     mbar_init(&sm.bar_load, 1);
