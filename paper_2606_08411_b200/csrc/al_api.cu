@@ -48,6 +48,8 @@ extern "C" al_status al_create(al_handle** out, int device) {
   h->encode_tiled = reinterpret_cast<decltype(h->encode_tiled)>(fn);
   const char* sp = getenv("ASYNCLANE_SELF_PLAN");   // "0": small attention calls use the plan kernel too (tests compare the two)
   h->self_plan = !(sp && sp[0] == '0');
+  const char* cs = getenv("ASYNCLANE_CONF_SPREAD");
+  h->conf_spread = !(cs && cs[0] == '0');
   *out = h;
   return AL_OK;
 }

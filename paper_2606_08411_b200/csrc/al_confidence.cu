@@ -436,13 +436,27 @@ int pick_cluster(int n_rows, int vec_total, int sm_count) {
   return k;
 }
 
+constexpr int kSmemPerSm = 228 * 1024;      // shared memory of an sm_100 SM
+
 template <typename T, bool kVector>
 cudaError_t launch_select(int k, int n_rows, cudaStream_t cs, const T* logits, int vocab, long long row_stride,
-                          int eos_id, const al_lane_desc* lanes, int n_lanes, const SelectArgs& out) {
+                          int eos_id, const al_lane_desc* lanes, int n_lanes, const SelectArgs& out, int sm_count, bool spread) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3((unsigned)(n_rows * k));
   cfg.blockDim = dim3(kThreads);
+  // A launch of less than one resident wave (4 CTAs per SM) is as slow as its busiest SM, and the block scheduler
+  // does not spread such a grid evenly: at 384 one-row CTAs on 148 SMs some SMs get four and 384 rows take longer
+  // than 444 (measured: 26.0 us against 22.8 at V = 131072).  Unused dynamic shared memory caps the CTAs an SM
+  // can hold at the even share ceil(CTAs / SMs), which forces the spread.
   cfg.dynamicSmemBytes = 0;
+  const long long n_ctas = (long long)n_rows * k;
+  const int share = (int)((n_ctas + sm_count - 1) / sm_count);
+  if (share < 4 && spread) {
+    cfg.dynamicSmemBytes = (size_t)(kSmemPerSm / share - 2048) & ~(size_t)1023;   // (static shared memory + 1 KB per CTA reserved by the system)
+    const cudaError_t e = cudaFuncSetAttribute(confidence_select_kernel<T, kVector>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                               (int)cfg.dynamicSmemBytes);
+    if (e != cudaSuccess) return e;
+  }
   cfg.stream = cs;
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -521,12 +535,12 @@ extern "C" al_status al_confidence_select(al_handle* h, const void* logits, int3
   cudaError_t e;
   if (dtype == AL_BF16) {
     const __nv_bfloat16* p = static_cast<const __nv_bfloat16*>(logits);
-    e = vec ? launch_select<__nv_bfloat16, true>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out)
-            : launch_select<__nv_bfloat16, false>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out);
+    e = vec ? launch_select<__nv_bfloat16, true>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out, h->sm_count, h->conf_spread)
+            : launch_select<__nv_bfloat16, false>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out, h->sm_count, h->conf_spread);
   } else {
     const float* p = static_cast<const float*>(logits);
-    e = vec ? launch_select<float, true>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out)
-            : launch_select<float, false>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out);
+    e = vec ? launch_select<float, true>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out, h->sm_count, h->conf_spread)
+            : launch_select<float, false>(k, n_rows, cs, p, vocab, row_stride, eos_id, lanes_eff, n_lanes, out, h->sm_count, h->conf_spread);
   }
   if (e != cudaSuccess) AL_FAIL(AL_ERR_CUDA, "al_confidence_select: launch failed: %s", cudaGetErrorString(e));
   h->launches++;

@@ -16,6 +16,7 @@ struct al_handle {
   int cc_major, cc_minor;
   size_t smem_optin;
   mutable std::atomic<uint64_t> launches{0};   // kernels enqueued through this handle
+  bool conf_spread = true; // confidence launches below one wave cap the CTAs per SM at the even share (ASYNCLANE_CONF_SPREAD=0 at al_create: off)
   bool self_plan = true;   // small attention calls plan inside the attention kernel (ASYNCLANE_SELF_PLAN=0 at al_create: always the plan kernel)
   // cuTensorMapEncodeTiled resolved through the runtime (no -lcuda at link time)
   CUresult (*encode_tiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
