@@ -14,8 +14,8 @@
 //     unit = (128-row tile, contiguous chunk of vocabulary tiles); units are numbered chunk-major so that the CTAs
 //     running at the same time share weight tiles through L2; a unit leaves one (m, s, idx) per row in the workspace
 //     and lm_head_select_kernel merges a row's chunks in vocabulary order (first maximiser wins) and applies the
-//     commit rule.  BN = 128 for few rows (the weight stream is HBM-bound and small tiles balance the SMs), 256 else.
-//     Few rows, kCluster = 2: every CTA would re-read the same hidden tile for each of its vocabulary tiles (L2 -> SM
+//     commit rule.  BN = 128 for one row tile (the weight stream is HBM-bound and small tiles balance the SMs), 256 else.
+//     One row tile, kCluster = 2: every CTA would re-read the same hidden tile for each of its vocabulary tiles (L2 -> SM
 //     traffic twice the weight stream), so the two CTAs of a cluster take alternate vocabulary tiles of one unit and
 //     each loads HALF of the hidden tile with TMA multicast into both; a stage is reused once BOTH issuers'
 //     tcgen05.commit (multicast to both CTAs' barriers) have released it.
@@ -61,9 +61,9 @@ __device__ __forceinline__ float ex2f(float x) {
   return y;
 }
 
-// The vocabulary tiles [t0, t0 + step * count) one CTA takes of unit u: the whole chunk (no cluster), or every second
-// tile of the pair's range starting at its rank (cluster of 2; the range is rounded up to an even number of tiles --
-// tiles beyond the vocabulary are loaded as zeros and masked in the epilogue -- so that both ranks run equally long).
+// The vocabulary tiles [t0, t0 + step * count) one CTA takes of unit u: the whole chunk (no cluster), or every
+// kCluster-th tile of the group's range starting at its rank (the range is rounded up to a multiple of the cluster
+// size -- tiles beyond it are masked in the epilogue -- so that all ranks run equally long).
 template <int kCluster>
 __device__ __forceinline__ void unit_tiles(const LmParams& p, int u, int rank, int& chunk, int& mt, int& t0, int& count, int& step,
                                            int& t_end) {
@@ -76,13 +76,13 @@ __device__ __forceinline__ void unit_tiles(const LmParams& p, int u, int rank, i
     count = t_end - t0;
     step = 1;
   } else {
-    const int n_pairs = p.n_chunks / 2;
-    const int a = (int)((long long)group * p.n_tiles / n_pairs), b = (int)((long long)(group + 1) * p.n_tiles / n_pairs);
-    chunk = 2 * group + rank;
+    const int n_groups = p.n_chunks / kCluster;
+    const int a = (int)((long long)group * p.n_tiles / n_groups), b = (int)((long long)(group + 1) * p.n_tiles / n_groups);
+    chunk = kCluster * group + rank;
     t0 = a + rank;
-    count = (b - a + 1) / 2;
-    step = 2;
-    t_end = b;                                             // rank 1's last tile of an odd range is the next unit's: masked
+    count = (b - a + kCluster - 1) / kCluster;
+    step = kCluster;
+    t_end = b;                                             // a rank's last tile may be the next unit's (range not a multiple of the cluster): masked
   }
 }
 
@@ -128,8 +128,8 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
           if (kCluster == 1) {
             tma_load_2d(sm.a[s], &map_a, &sm.full[s], kb * kBK, mt * kBM);
           } else {                                                           // my half of the hidden tile, into both CTAs
-            tma_load_2d_multicast(sm.a[s] + rank * (C::kABytes / 2), &map_a, &sm.full[s], kb * kBK,
-                                  mt * kBM + rank * (kBM / 2), (uint16_t)0x3);
+            tma_load_2d_multicast(sm.a[s] + rank * (C::kABytes / kCluster), &map_a, &sm.full[s], kb * kBK,
+                                  mt * kBM + rank * (kBM / kCluster), (uint16_t)((1u << kCluster) - 1u));
           }
           tma_load_2d(sm.b[s], &map_b, &sm.full[s], kb * kBK, (t0 + j * step) * BN);
         }
@@ -159,7 +159,7 @@ lm_head_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
             if (leader) mma_ss(d, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), idesc, (kb | k) ? 1u : 0u);
           if (leader) {
             if (kCluster == 1) mma_commit(&sm.empty[s]);
-            else mma_commit_multicast(&sm.empty[s], (uint16_t)0x3);      // the stage holds a half the peer loaded: both release it
+            else mma_commit_multicast(&sm.empty[s], (uint16_t)((1u << kCluster) - 1u));   // the stage holds parts the peers loaded: all release it
           }
         }
         if (leader) mma_commit(&sm.acc_full[acc]);
@@ -271,10 +271,12 @@ struct LmPlan {
 LmPlan lm_plan(int n_rows, int vocab, int sm_count) {
   LmPlan L;
   L.m_tiles = (n_rows + kBM - 1) / kBM;
-  // few rows: the weight stream is HBM-bound and what matters is equal bytes per SM -> small vocabulary tiles, and the
-  // hidden tile shared by the two CTAs of a cluster (TMA multicast)
-  L.bn = L.m_tiles <= 4 ? 128 : 256;
-  L.cluster = L.m_tiles <= 4 ? 2 : 1;
+  // one row tile (<= 128 rows): the weight stream is HBM-bound and what matters is equal bytes per SM -> small
+  // vocabulary tiles, and the hidden tile shared by the two CTAs of a cluster (TMA multicast).  From two row tiles on
+  // the wide tile wins (measured, 256 / 384 / 512 rows: 259 / 330 / 423 us against 293 / 407 / 528 us with 128-wide
+  // tiles in clusters of 2, 283 / 373 / 500 us without clusters): half as many hidden-tile reads per weight byte.
+  L.bn = L.m_tiles <= 1 ? 128 : 256;
+  L.cluster = L.m_tiles <= 1 ? 2 : 1;
   L.n_tiles = (vocab + L.bn - 1) / L.bn;
   const int slots = sm_count / L.cluster;                  // CTAs, or clusters, that run at the same time
   // groups (chunks, or pairs of chunks): units = groups * m_tiles should fill whole waves of the slots (a last wave of

@@ -72,6 +72,7 @@ def test_small_rows_ragged_everything(handle):
     run_case(handle, 37, 5003, 200, seed=1)
     run_case(handle, 1, 1000, 64, seed=2)
     run_case(handle, 130, 3000, 72, seed=3)                 # two row tiles, K tail of 8
+    run_case(handle, 390, 2500, 64, seed=7)                 # four row tiles (wide vocabulary tiles, no cluster)
 
 
 def test_llada_shaped_few_rows(handle):
