@@ -457,7 +457,13 @@ lane_plan_kernel(const al_lane_desc* __restrict__ lanes, int n_lanes, int n_kv_h
 // With two sub-tiles per step both streams' softmax warps load each SM sub-partition's MUFU and three
 // of eight pay; when the streams take alternate key tiles (whole-item plans) one of eight is enough and
 // the instruction count matters more (cfg4: 648 -> 617 us with one, cfg5: 88.6 -> 90.9 us).
-constexpr int kPolyMaskTwoSubTiles = 0x52, kPolyMaskAlt = 0x10;
+#ifndef AL_POLY_TWO
+#define AL_POLY_TWO 0x52
+#endif
+#ifndef AL_POLY_ALT
+#define AL_POLY_ALT 0x10
+#endif
+constexpr int kPolyMaskTwoSubTiles = AL_POLY_TWO, kPolyMaskAlt = AL_POLY_ALT;
 #ifdef AL_EPI_NO_TMA_STORE
 constexpr bool kTmaStoreOk = false;        // debug knob: every bf16 sub-tile is copied out by its own warps
 #else
