@@ -326,7 +326,8 @@ def measure_next_rows(h, dev, stream, peaks):
     """SURVEY 8(f) rows, each timed on its own (CUDA events on the stream, inputs resident): the fused LM head at the
     LLaDA-layer and batch-16 shapes (next to the library route it replaces: cuBLAS GEMM + al_confidence_select on
     materialised bf16 logits), al_lane_status on the batch-16 lanes, the Eq.12 refresh forward of one Dream-shaped
-    sequence, and Algorithm 1 end to end with the table-driven stub model."""
+    sequence, the compact refresh on a random sorted subset and on a contiguous run (reading C8), and Algorithm 1 end to
+    end with the table-driven stub model."""
     import numpy as np
     import torch
     from paper_2606_08411_b200 import binding as B, workloads as W
@@ -397,6 +398,25 @@ def measure_next_rows(h, dev, stream, peaks):
     t_rf = timed(lambda: h.al_refresh_forward(shape, q, k, v, kc, vc, ln, 1, Lr, 0, o, None, wsa, stream), 30)
     fl = 4.0 * Hq * d * Lr * Lr
     out["refresh_forward_dream_1024"] = {"us": t_rf, "tflops": fl / t_rf / 1e6, "frac_of_bf16_peak": fl / t_rf / 1e6 / peaks["tensor"]}
+    # compact refresh, both position sets of reading C8: a sorted random subset of the prefix (what the
+    # workloads use) and the contiguous run [0, R) of Eq.12 -- config-4 shape: 32 layers, 320 of 1280 rows, 32 kv-heads.
+    # Two cache sets (2 x 0.8 GB) alternate so that no launch finds its rows in L2.
+    Lc, Hc, R, rows_c = 32, 32, 320, 1536
+    shape_r = B.Handle.make_shape(32, Hc, 128, B.AL_BF16, rows_c)
+    caches = [(torch.zeros(Lc, Hc, rows_c, 128, device=dev, dtype=torch.bfloat16), torch.zeros(Lc, Hc, rows_c, 128, device=dev, dtype=torch.bfloat16)) for _ in range(2)]
+    srcs = [(rnd(Lc, R, Hc, 128).bfloat16(), rnd(Lc, R, Hc, 128).bfloat16()) for _ in range(2)]
+    rngr = np.random.default_rng(20260608)
+    pos_sets = {"random_sorted": np.sort(rngr.choice(1280, size=R, replace=False)).astype(np.int32), "contiguous": np.arange(R, dtype=np.int32)}
+    rbytes = 2 * 2 * R * Hc * 128 * 2 * Lc + 4 * R
+    for nm, pos in pos_sets.items():
+        pd = torch.from_numpy(pos).to(dev)
+        state = {"i": 0}
+        def one():
+            i = state["i"] = state["i"] ^ 1
+            h.al_kv_refresh(shape_r, caches[i][0], caches[i][1], srcs[i][0], srcs[i][1], pd, R, 0, Lc, Hc * rows_c * 128, R * Hc * 128, stream)
+        t = timed(one, 40)
+        out["refresh_cfg4_shape_" + nm] = {"us": t, "gbs": rbytes / t / 1e3, "frac_of_hbm_peak": rbytes / t / 1e3 / peaks["hbm"]}
+    del caches, srcs
     # Algorithm 1 with the stub model (whole decode of 192 tokens, one synchronisation per iteration)
     case = W.scheduler_case(37, gen_len=192)
     t0 = time.perf_counter()
