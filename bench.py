@@ -417,6 +417,22 @@ def measure_next_rows(h, dev, stream, peaks):
         t = timed(one, 40)
         out["refresh_cfg4_shape_" + nm] = {"us": t, "gbs": rbytes / t / 1e3, "frac_of_hbm_peak": rbytes / t / 1e3 / peaks["hbm"]}
     del caches, srcs
+    # launch floor: the smallest launch of this library -- al_kv_refresh of ONE row, one CTA --
+    # back to back inside a CUDA graph, as the steps are timed: what a kernel of a single-layer step costs at least
+    pd1 = torch.zeros(1, dtype=torch.int32, device=dev)
+    kc1, vc1 = torch.zeros(Hkv, 8, d, device=dev, dtype=torch.bfloat16), torch.zeros(Hkv, 8, d, device=dev, dtype=torch.bfloat16)
+    ks1, vs1 = torch.zeros(1, Hkv, d, device=dev, dtype=torch.bfloat16), torch.zeros(1, Hkv, d, device=dev, dtype=torch.bfloat16)
+    shape1 = B.Handle.make_shape(Hq, Hkv, d, B.AL_BF16, 8)
+    gfl = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(stream):
+        h.al_kv_refresh(shape1, kc1, vc1, ks1, vs1, pd1, 1, 0, 1, 0, 0, stream)
+        stream.synchronize()
+        with torch.cuda.graph(gfl, stream=stream):
+            for _ in range(20):
+                h.al_kv_refresh(shape1, kc1, vc1, ks1, vs1, pd1, 1, 0, 1, 0, 0, stream)
+    out["launch_floor"] = {"us_per_launch": timed(lambda: gfl.replay(), 20) / 20,
+                           "what": "al_kv_refresh of one row (one CTA), 20 launches per CUDA-graph replay"}
     # Algorithm 1 with the stub model (whole decode of 192 tokens, one synchronisation per iteration)
     case = W.scheduler_case(37, gen_len=192)
     t0 = time.perf_counter()
