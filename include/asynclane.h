@@ -78,7 +78,10 @@ typedef struct {
 /* ---- life cycle ------------------------------------------------------------------------------- */
 
 /* Creates a handle bound to CUDA device `device` (queries SM count, resolves the tensor-map encoder).
- * Fails with AL_ERR_CUDA when no usable device exists: there is no CPU fallback. */
+ * Fails with AL_ERR_CUDA when no usable device exists: there is no CPU fallback.
+ * Two environment switches are read here, once, for tests and measurements (results are the same either way):
+ * ASYNCLANE_SELF_PLAN=0 (small attention calls launch the plan kernel too) and ASYNCLANE_CONF_SPREAD=0
+ * (confidence launches of less than one resident wave do not cap the CTAs per SM). */
 al_status al_create(al_handle** out_handle, int device);
 al_status al_destroy(al_handle* handle);
 /* Thread-local, never NULL, valid until the next failing call on this thread. */
