@@ -1356,7 +1356,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         // (the streams exchange their running maxima and row sums and work out the merge weights while their
         // last P.V drain; each waits for its own accumulator just before the second barrier)
         if (tid128 == 0) sm.alt_has[b] = n_mine > 0;
-        AL_STAGE_ROUND_BEGIN();                        // the previous piece's bulk stores are done with the staging rows
+        // (an alt CTA holds ONE piece: no earlier bulk store can still be reading the staging rows)
         *reinterpret_cast<float2*>(my_stage) = make_float2(m_used, l_sum);   // exchanged through the staging rows
         bar_sync_both();
         TRACE_E(1);
@@ -1433,10 +1433,10 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         }
         tc_fence_before();
         TRACE_E(6);
-        bar_sync_both();                               // both streams have read both accumulators (and published)
+        // (no barrier, no o_empty arrival: nothing follows the CTA's one piece that could overwrite an accumulator
+        // the other stream is still reading)
         TRACE_E(7);
-        if (n_mine > 0) mbar_arrive(&sm.o_empty[b]);
-        do_ticket = do_ticket && b == 0;               // stream 0 counts and merges for the tile
+        do_ticket = false;
       } else {
       const bool full = kTmaStoreOk && T.n_tok - b * p.tpt >= p.tpt;     // the sub-tile fills its TMA box: no row beyond it may be written
       if (n_mine == 0) {
@@ -1530,7 +1530,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
         bar_sync_stream(b);                            // ticket is reused by the next piece
       }
     }
-    if (tid128 == 0) bulk_wait_all();                  // the staging rows must outlive the bulk stores that read them
+    if (tid128 == 0) bulk_wait_read_all();             // the staging rows must outlive the bulk stores that read them (their writes complete with the grid)
   }
 }
 
