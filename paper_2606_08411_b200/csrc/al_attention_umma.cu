@@ -824,6 +824,10 @@ __device__ __forceinline__ float* part_round_ptr(const AttnParams& p, int slot, 
 // Keeping each mode's code out of the other instance is worth a lot: the general instance got 8 us of 108 at
 // cfg5 in round 1, and making the alt instance alt-ONLY (it used to test the tile at run time) took cfg4 from
 // 616 to 585 us per 32 layers and the cfg3 kernel from 18.4 to 16.7 us.
+// The piece loops run ONCE in the alt instance: an alt CTA holds one whole item, and saying so lets the compiler fold
+// the per-piece ring / phase counters (cfg4 562 -> 555 us per 32 layers, cfg2 kernel 13.3 -> 12.3 us).  (Also telling
+// it that the piece starts at key tile 0 took the gain at cfg4 back: 564 us.)
+#define AL_FOR_PIECES(w) for (bool more_ = (w).next(); more_; more_ = kAltOk ? false : (w).next())
 template <bool kAltOk>
 __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, const CUtensorMap* pmap_q,
                                            const CUtensorMap* pmap_knew, const CUtensorMap* pmap_vnew,
@@ -839,7 +843,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       // ===================== TMA producer of Q and the K tiles =====================
       uint32_t kv_it = 0, piece_it = 0;
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
-      while (w.next()) {
+      AL_FOR_PIECES(w) {
         const TileRec& T = w.T;
         const bool two = T.n_tok > p.tpt;
         auto issue_k = [&](int kt) {
@@ -878,7 +882,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       // must not queue behind it)
       uint32_t kv_it = 0;
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
-      while (w.next()) {
+      AL_FOR_PIECES(w) {
         const TileRec& T = w.T;
         for (int kt = w.kt_begin; kt < w.kt_end; ++kt, ++kv_it) {
           const int sv = kv_it % kStagesV;
@@ -919,7 +923,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       uint32_t c_qk = 0, c_pv = 0;             // key tiles of this stream whose Q.K^T / P.V has been issued (all pieces)
       uint32_t oe = 0;                         // pieces so far in which the stream had key tiles: o_empty phase
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
-      while (w.next()) {
+      AL_FOR_PIECES(w) {
         const int n = w.kt_end - w.kt_begin;
         const bool alt = alt_ok;     // one sub-tile: both streams work on Q of sub-tile A
         const StreamSteps mine(w.T, p.tpt, b, w.kt_begin, alt_ok);
@@ -1059,7 +1063,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       uint32_t kv_it = 0, piece_it = 0;
       uint32_t c_qk0 = 0, c_qk1 = 0;           // key tiles of stream A / B whose Q.K^T has been issued (all pieces)
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
-      while (w.next()) {
+      AL_FOR_PIECES(w) {
         const int n = w.kt_end - w.kt_begin;
         const bool alt = alt_ok;     // one sub-tile: both streams work on Q of sub-tile A
         const StreamSteps mine0(w.T, p.tpt, 0, w.kt_begin, alt_ok), mine1(w.T, p.tpt, 1, w.kt_begin, alt_ok);
@@ -1109,7 +1113,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       uint32_t c_pv0 = 0, c_pv1 = 0;           // key tiles of stream A / B whose P.V has been issued (all pieces)
       uint32_t oe0 = 0, oe1 = 0;               // pieces so far in which the stream had key tiles: o_empty phase
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
-      while (w.next()) {
+      AL_FOR_PIECES(w) {
         const int n = w.kt_end - w.kt_begin;
         const StreamSteps mine0(w.T, p.tpt, 0, w.kt_begin, alt_ok), mine1(w.T, p.tpt, 1, w.kt_begin, alt_ok);
         bool first0 = true, first1 = true;
@@ -1200,7 +1204,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
     uint32_t cnt = 0;                                  // key tiles this stream has processed (all pieces)
     uint32_t pieces_done = 0;                          // pieces in which it had key tiles: o_full phase
     PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
-    while (w.next()) {
+    AL_FOR_PIECES(w) {
       const TileRec& T = w.T;
       const int n = w.kt_end - w.kt_begin;
       const bool alt = alt_ok;     // one sub-tile: this stream takes every other key tile of it
