@@ -845,7 +845,7 @@ __device__ __forceinline__ void attn_roles(AttnSmem& sm, const AttnParams& p, co
       PieceWalk w(p.plan, &sm.cta, p.n_kv_heads, blockIdx.x);
       AL_FOR_PIECES(w) {
         const TileRec& T = w.T;
-        const bool two = T.n_tok > p.tpt;
+        const bool two = !kAltOk && T.n_tok > p.tpt;      // (an alt CTA's item has one sub-tile)
         auto issue_k = [&](int kt) {
           const int sk = kv_it % kStagesK;
           const bool pref = kt < T.n_pref_tiles;
