@@ -346,6 +346,18 @@ def measure_next_rows(h, dev, stream, peaks):
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / n * 1e3
 
+    def timed_graph(fn, n, inner=8):
+        """us per call with `inner` calls captured into one CUDA graph (as the steps are timed: no host launch cost)"""
+        g = torch.cuda.CUDAGraph()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(stream):
+            fn()
+            stream.synchronize()
+            with torch.cuda.graph(g, stream=stream):
+                for _ in range(inner):
+                    fn()
+        return timed(lambda: g.replay(), n) / inner
+
     out = {}
     gen = torch.Generator(device=dev).manual_seed(1)
     rnd = lambda *sh: torch.randn(*sh, device=dev, generator=gen)
@@ -385,8 +397,8 @@ def measure_next_rows(h, dev, stream, peaks):
     cm = torch.zeros(n_r, dtype=torch.uint8, device=dev); to = ti.clone() + 1
     stt = torch.zeros((n_l, 8), dtype=torch.int32, device=dev)
     dl = torch.tensor([13, 30], dtype=torch.int32, device=dev)
-    out["lane_status_batch16"] = {"us": timed(lambda: h.al_lane_status(lanes_d, n_l, n_r, ti, cf, am, 7, 2, 0.9, dl, None, cm, to, stt, stream), 50),
-                                  "lanes": n_l, "rows": n_r}
+    f_status = lambda: h.al_lane_status(lanes_d, n_l, n_r, ti, cf, am, 7, 2, 0.9, dl, None, cm, to, stt, stream)
+    out["lane_status_batch16"] = {"us": timed_graph(f_status, 20), "us_direct_launch": timed(f_status, 50), "lanes": n_l, "rows": n_r}
     # refresh forward (Eq.12) of one Dream-shaped sequence: L_refresh = 1024, 28q / 4kv heads, d = 128
     Lr, Hq, Hkv, d = 1024, 28, 4, 128
     shape = B.Handle.make_shape(Hq, Hkv, d, B.AL_BF16, Lr + 64)
@@ -395,9 +407,12 @@ def measure_next_rows(h, dev, stream, peaks):
     o = torch.zeros_like(q)
     ln = torch.tensor([[0, 0, 0, 0, Lr, 0]], dtype=torch.int32, device=dev)
     wsa = torch.empty(h.al_lane_attention_workspace_bytes(shape, 1, Lr, 0), dtype=torch.uint8, device=dev)
-    t_rf = timed(lambda: h.al_refresh_forward(shape, q, k, v, kc, vc, ln, 1, Lr, 0, o, None, wsa, stream), 30)
+    f_rf = lambda: h.al_refresh_forward(shape, q, k, v, kc, vc, ln, 1, Lr, 0, o, None, wsa, stream)
+    t_rf = timed_graph(f_rf, 20, inner=4)
     fl = 4.0 * Hq * d * Lr * Lr
-    out["refresh_forward_dream_1024"] = {"us": t_rf, "tflops": fl / t_rf / 1e6, "frac_of_bf16_peak": fl / t_rf / 1e6 / peaks["tensor"]}
+    out["refresh_forward_dream_1024"] = {"us": t_rf, "us_direct_launch": timed(f_rf, 30), "tflops": fl / t_rf / 1e6,
+                                         "frac_of_bf16_peak": fl / t_rf / 1e6 / peaks["tensor"],
+                                         "note": "plan + attention + append, 4 calls per CUDA-graph replay; the direct-launch figure includes the host's tensor-map encoding"}
     # compact refresh, both position sets of reading C8: a sorted random subset of the prefix (what the
     # workloads use) and the contiguous run [0, R) of Eq.12 -- config-4 shape: 32 layers, 320 of 1280 rows, 32 kv-heads.
     # Two cache sets (2 x 0.8 GB) alternate so that no launch finds its rows in L2.
